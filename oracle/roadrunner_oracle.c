@@ -165,7 +165,7 @@ int oracle_kepler(double M, double e, double *Eout)
         double f = E - e * sin(E) - M;
         if (f > 0.0) hi = E; else lo = E;
         double En = E - f / (1.0 - e * cos(E));
-        if (!(En > lo && En < hi)) En = 0.5 * (lo + hi);
+        if (!(En >= lo && En <= hi)) En = 0.5 * (lo + hi);   /* Newton left the bracket: bisect */
         double dE = En - E;
         E = En;
         if (fabs(dE) <= 1e-15) { ++it; break; }
