@@ -1,0 +1,191 @@
+/*
+ * roadrunner.h - C-ABI of the B200-native RoadRunner transit-model library
+ *                (libroadrunner_b200.so, sm_100a CUDA kernels behind plain C entry points).
+ *
+ * The method is H. Parviainen, "RoadRunner: a fast and flexible exoplanet transit model"
+ * (arXiv:2009.08500).  Citations below are PAPER.md line numbers (section / equation); readings
+ * of the paper where it is silent are numbered R1..R12 in DESIGN.md section 3.
+ *
+ * The two calls of the problem statement are
+ *     build_ld_table(ldp[npv x npb x nz])                                   -> rr_build_ld_table
+ *     evaluate(times, lc_index, passband_index, supersampling, exposure_time,
+ *              pv[npv x npar]) -> flux[npv x npt]                  -> rr_set_data + rr_evaluate
+ * following the paper's call pattern "set_data once, evaluate many times";
+ * rr_evaluate_flat is the one-call form with the problem statement's flat argument list.
+ *
+ * Conventions (every entry point)
+ *   - extern "C", plain pointers and sizes; no C++ or torch types cross the boundary.
+ *   - A pointer named d_* is a DEVICE pointer, h_* a HOST pointer.  All are owned by the caller;
+ *     the library never frees or keeps them beyond the call unless stated (rr_set_data copies).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls are
+ *     asynchronous on that stream unless stated.
+ *   - Return value: 0 = ok; a negative RR_E* code = argument/state error detected on the host
+ *     before anything was launched; <= -1000 = CUDA error (-1000 - cudaError_t).
+ *     rr_error_string() names any code.  No exception crosses the ABI.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with a CUDA error.
+ *
+ * Per-parameter-vector validity (reading R12): a parameter vector whose k is outside [k0,k1], whose
+ * e is outside [0,1), whose a <= 0 or p <= 0, or that holds a non-finite value gets an all-NaN
+ * flux row and a non-zero status word (bits below); the call itself still returns 0, so that a
+ * sampler does not lose its other walkers.
+ */
+#ifndef ROADRUNNER_B200_H
+#define ROADRUNNER_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- codes ------------------------------------------------------------------------------- */
+#define RR_FP64 0
+#define RR_FP32 1
+
+#define RR_OK            0
+#define RR_ENULL        -1   /* a required pointer is NULL                                     */
+#define RR_ECONFIG      -2   /* rr_config out of range                                         */
+#define RR_ESIZE        -3   /* a size is <= 0 or inconsistent (npar, npv, npt, nlc)           */
+#define RR_EINDEX       -4   /* lc_index / passband_index / supersampling out of range         */
+#define RR_ESTATE       -5   /* call order: evaluate before set_data / build_ld_table, or npv  */
+#define RR_EALLOC       -6   /* device or host allocation failed                               */
+#define RR_ECUDA_BASE   -1000
+
+/* status bits written per parameter vector (reading R12) */
+#define RR_PV_K_RANGE    1   /* some k outside [k0, k1]            */
+#define RR_PV_E_RANGE    2   /* e outside [0, 1)                   */
+#define RR_PV_A_RANGE    4   /* a <= 0                             */
+#define RR_PV_P_RANGE    8   /* p <= 0                             */
+#define RR_PV_NONFINITE 16   /* a NaN or infinity in the row       */
+
+/* supersample reduction layout of the fused flux kernel (rr_set_reduction) */
+#define RR_REDUCE_AUTO    0  /* library picks per light curve from ns and the amount of work    */
+#define RR_REDUCE_THREAD  1  /* one thread per exposure, in-thread loop over its sub-samples    */
+#define RR_REDUCE_SHUFFLE 2  /* sub-samples across lanes, warp-shuffle sum       */
+
+typedef struct rr_ctx rr_ctx;   /* opaque; owned by the library */
+
+/* Resolution of the model: what the paper's RoadRunnerModel constructor fixes
+ * (PAPER.md:83-92 z grid; :116-122 (k,g) weight table).                                        */
+typedef struct {
+  int32_t nzin;      /* radial bins of constant dz  on [0, zcut]                 (>= 1)          */
+  int32_t nzlimb;    /* radial bins of constant dmu on [zcut, 1]; nz = nzin+nzlimb (>= 1)        */
+  double  zcut;      /* 0 < zcut < 1                                                             */
+  int32_t ng;        /* nodes of g = z/(1+k) on [0,1], g_i = i/(ng-1)            (>= 2)          */
+  int32_t nk;        /* nodes of the radius ratio, k_i = k0 + i (k1-k0)/(nk-1)   (>= 2)          */
+  double  k0, k1;    /* 0 < k0 < k1                                                              */
+  int32_t npb;       /* passbands                                                (>= 1)          */
+  int32_t nkpb;      /* 1 = one k per parameter vector; npb = one k per passband  */
+  int32_t precision; /* RR_FP64 or RR_FP32: type of ldp, istar, the table and flux               */
+} rr_config;
+
+/* ---- life cycle ------------------------------------------------------------------------------
+ * rr_create builds, on the current CUDA device, the z grid ze[nz+1], zm[nz], mu[nz]
+ * (zm = edge mean, reading R1) and the geometry weight tensor W[nk][ng][nz]
+ * (g = 1 node = limit, reading R5) in fp64.  Synchronous.          */
+int rr_create(const rr_config *cfg, rr_ctx **out);
+int rr_destroy(rr_ctx *ctx);
+const char *rr_error_string(int code);
+
+/* Grid read-back (host arrays, fp64): the caller samples its limb-darkening law at mu[nz]
+ * (PAPER.md:89, :98).  h_W (optional diagnostics) receives W[nk][ng][nz].  Synchronous.         */
+int rr_get_mu(const rr_ctx *ctx, double *h_mu /*[nz]*/);
+int rr_get_ze(const rr_ctx *ctx, double *h_ze /*[nz+1]*/);
+int rr_get_weights(const rr_ctx *ctx, double *h_W /*[nk][ng][nz]*/);
+
+/* ---- data: paper's tm.set_data(times, lcids, pbids, nsamples, exptimes), PAPER.md:230-236 -----
+ * d_times[npt]          mid-exposure times (days), fp64, any order
+ * d_lc_index[npt]       light-curve index of each exposure, 0 <= . < nlc
+ * h_passband_index[nlc] passband of each light curve, 0 <= . < npb     (reading R11: per light
+ *                       curve, as in the paper; per-point passband = passband_index[lc_index[i]])
+ * h_supersampling[nlc]  sub-samples per exposure, >= 1
+ * h_exposure_time[nlc]  exposure time (days), >= 0; sub-sample s of n sits at
+ *                       t + tau*((s+1/2)/n - 1/2)                               (reading R7)
+ * The library copies all five and runs the heterogeneous-dispatch kernels (DESIGN.md section 6,
+ * kernel 4), which cut the exposure axis into tiles of one light curve each (uniform ns, tau,
+ * passband) with their time range.  Synchronous on `stream` (it reads back the tile count).
+ * RR_EINDEX if any index is out of range (nothing is kept then).                                */
+int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, int64_t npt,
+                const int32_t *h_passband_index, const int32_t *h_supersampling,
+                const double *h_exposure_time, int32_t nlc, void *stream);
+
+/* ---- kernel 1: LD table, PAPER.md:98-99, :127-131 -----------------------------------------------
+ * d_ldp[npv][npb][nz]  the limb-darkening profile sampled at mu[nz] (ctx precision)
+ * d_istar[npv][npb]    optional disk-integrated brightness (ctx precision); NULL = reading R6:
+ *                      Istar = pi sum_j ldp[j] (ze[j+1]^2 - ze[j]^2)            (Eq. (2))
+ * Builds T[npv][npb][nk][ng] = sum_j W[ik][ig][j] ldp[pv][pb][j] and Istar[npv][npb] in buffers
+ * owned by ctx (grown as needed).  fp64 accumulation in both precisions.                        */
+int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64_t npv,
+                      void *stream);
+/* Diagnostics: device pointers to the table and Istar built last (ctx precision), or NULL.      */
+const void *rr_table_ptr(const rr_ctx *ctx);
+const void *rr_istar_ptr(const rr_ctx *ctx);
+/* Copies the table T[npv][npb][nk][ng] and Istar[npv][npb] built last to host arrays (ctx
+ * precision; either may be NULL).  Synchronous (device-wide).                                   */
+int rr_get_table(const rr_ctx *ctx, void *h_T, void *h_istar);
+
+/* ---- kernels 2+3+4: evaluate, PAPER.md:101-107, :128-131, :214, :220 ---------------------------
+ * d_pv[npv][npar]   fp64 rows [k_0..k_{nkpb-1}, t0, p, a, i, e, w], npar = nkpb + 6: the order of
+ *                   the paper's evaluate(k, ldc, t0, p, a, i, e, w) with ldc replaced by ldp.
+ *                   t0 = time of inferior conjunction, p period (days), a = semi-major axis /
+ *                   stellar radius, i inclination and w argument of periastron in radians.
+ * d_flux[npv][npt]  out, ctx precision, row-major, exposure order of d_times.
+ * d_status[npv]     out, optional (NULL): status bits above.
+ * npv must equal the npv of the last rr_build_ld_table.                                         */
+int rr_evaluate(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, void *d_flux,
+                int32_t *d_status, void *stream);
+
+/* One-call form with the problem statement's flat argument list: rr_set_data (synchronous) then
+ * rr_evaluate.                                                                                  */
+int rr_evaluate_flat(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, int64_t npt,
+                     const int32_t *h_passband_index, const int32_t *h_supersampling,
+                     const double *h_exposure_time, int32_t nlc, const double *d_pv, int32_t npar,
+                     int64_t npv, void *d_flux, int32_t *d_status, void *stream);
+
+/* ---- kernel 2 alone: projected separation, for tests and diagnostics -------
+ * d_z[npv][nsub], nsub = sum over exposures of their ns (rr_num_subsamples), sub-samples of an
+ * exposure contiguous, exposure order; fp64 in both precisions of ctx unless fp32_math != 0, in
+ * which case the fp32 orbit arithmetic of the RR_FP32 flux kernel is used and widened.  A
+ * sub-sample with the planet behind the star stores -z.  Rows of invalid pvs are NaN.  Needs
+ * rr_set_data; not rr_build_ld_table.                                                           */
+int rr_orbit_z(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, double *d_z,
+               int32_t fp32_math, void *stream);
+int64_t rr_num_subsamples(const rr_ctx *ctx);   /* < 0: no data set */
+int64_t rr_num_tiles(const rr_ctx *ctx);        /* dispatch tiles of the current data; < 0: none */
+
+/* Dispatch read-back for tests (host arrays of rr_num_tiles entries each): first exposure, number
+ * of exposures and light curve of every tile, and its [tmin, tmax] time range.  Synchronous.    */
+int rr_get_tiles(const rr_ctx *ctx, int32_t *h_start, int32_t *h_count, int32_t *h_lc,
+                 double *h_tmin, double *h_tmax);
+
+/* Supersample reduction layout (RR_REDUCE_*); takes effect at the next rr_set_data.             */
+int rr_set_reduction(rr_ctx *ctx, int32_t mode);
+
+/* ---- whole step with HOST buffers (the end-to-end call) --------------------------------------------
+ * h_ldp[npv][npb][nz], h_pv[npv][npar] -> h_flux[npv][npt], h_status[npv] (optional).  Runs
+ * rr_build_ld_table + rr_evaluate over chunks of parameter vectors on two internal streams so
+ * that the host<->device copies of one chunk overlap the kernels of the next.  Host buffers may be
+ * pageable or pinned (pinned ones copy faster).  Needs rr_set_data.  Synchronous.  Afterwards the
+ * ctx table holds the LAST chunk only.                                                           */
+int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t npar, int64_t npv,
+                     void *h_flux, int32_t *h_status);
+
+/* ---- measurement aids (bench.py) ---------------------------------------------------------------
+ * Counters of the last rr_evaluate on this ctx, filled by the flux kernel when enabled with
+ * rr_enable_counters(ctx, 1) (adds atomics; keep off when timing): h_counts[0] sub-samples skipped
+ * as out of the transit window, [1] evaluated circular, [2] evaluated eccentric, [3] of those with
+ * z < 1+k in front of the star, [4] of those in ingress/egress (lens area), [5] Newton iterations,
+ * [6] (tile, pv) pairs filled without evaluation, [7] (tile, pv) pairs evaluated.  Synchronous. */
+int rr_enable_counters(rr_ctx *ctx, int32_t on);
+int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts /*[8]*/);
+/* Number of kernel launches the library has made on this ctx since creation.                     */
+int64_t rr_launch_count(const rr_ctx *ctx);
+/* FP64 / FP32 FMA pipe peak of the current device, measured with a register-resident FMA chain
+ * (DESIGN.md section 7): returns thread-level FMA instructions per second in *h_fma_per_s.
+ * Synchronous.                                                                                   */
+int rr_measure_fma_peak(int32_t precision, double *h_fma_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ROADRUNNER_B200_H */

@@ -1,0 +1,367 @@
+"""paper_2009_08500_b200 - thin Python binding of libroadrunner_b200.so (include/roadrunner.h).
+
+Argument marshalling only: every step of the path (z grid and geometry weights, LD table, orbit,
+fused flux, heterogeneous dispatch) runs in the library's sm_100a CUDA kernels.  PyTorch supplies
+device memory and the current CUDA stream, nothing else.  There is no CPU fallback: loading fails
+loudly if the library cannot be built or found, and every compute call raises ``RoadRunnerError``
+when CUDA reports an error (e.g. no device).
+
+Module-level ``rr_*`` functions mirror the C entry points one to one (torch tensors in place of
+raw pointers); ``RoadRunner`` is a small convenience wrapper in the shape of the paper's
+``RoadRunnerModel``: ``set_data`` once, ``build_ld_table`` + ``evaluate`` many
+times.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+RR_FP64, RR_FP32 = 0, 1
+RR_REDUCE_AUTO, RR_REDUCE_THREAD, RR_REDUCE_SHUFFLE = 0, 1, 2
+RR_PV_K_RANGE, RR_PV_E_RANGE, RR_PV_A_RANGE, RR_PV_P_RANGE, RR_PV_NONFINITE = 1, 2, 4, 8, 16
+
+# every symbol include/roadrunner.h declares (tests check the library exports each of them)
+SYMBOLS = (
+    "rr_create", "rr_destroy", "rr_error_string", "rr_get_mu", "rr_get_ze", "rr_get_weights",
+    "rr_set_data", "rr_build_ld_table", "rr_table_ptr", "rr_istar_ptr", "rr_get_table",
+    "rr_evaluate",
+    "rr_evaluate_flat", "rr_orbit_z", "rr_num_subsamples", "rr_num_tiles", "rr_get_tiles",
+    "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
+    "rr_launch_count", "rr_measure_fma_peak",
+)
+
+
+class RoadRunnerError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {error_string(code)} (code {code})")
+
+
+class rr_config(C.Structure):
+    _fields_ = [("nzin", C.c_int32), ("nzlimb", C.c_int32), ("zcut", C.c_double),
+                ("ng", C.c_int32), ("nk", C.c_int32), ("k0", C.c_double), ("k1", C.c_double),
+                ("npb", C.c_int32), ("nkpb", C.c_int32), ("precision", C.c_int32)]
+
+
+_lib = None
+_VP, _I64, _I32, _DBL = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load() -> C.CDLL:
+    """Build (if stale) and load the CUDA library.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build() if os.path.exists(_build.NVCC) else _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing and nvcc is not available to build it; "
+                           "there is no CPU fallback")
+    lib = C.CDLL(path)
+    sig = {
+        "rr_create": (C.c_int, [C.POINTER(rr_config), C.POINTER(_VP)]),
+        "rr_destroy": (C.c_int, [_VP]),
+        "rr_error_string": (C.c_char_p, [C.c_int]),
+        "rr_get_mu": (C.c_int, [_VP, _VP]),
+        "rr_get_ze": (C.c_int, [_VP, _VP]),
+        "rr_get_weights": (C.c_int, [_VP, _VP]),
+        "rr_set_data": (C.c_int, [_VP, _VP, _VP, _I64, _VP, _VP, _VP, _I32, _VP]),
+        "rr_build_ld_table": (C.c_int, [_VP, _VP, _VP, _I64, _VP]),
+        "rr_table_ptr": (_VP, [_VP]),
+        "rr_istar_ptr": (_VP, [_VP]),
+        "rr_get_table": (C.c_int, [_VP, _VP, _VP]),
+        "rr_evaluate": (C.c_int, [_VP, _VP, _I32, _I64, _VP, _VP, _VP]),
+        "rr_evaluate_flat": (C.c_int, [_VP, _VP, _VP, _I64, _VP, _VP, _VP, _I32, _VP, _I32, _I64,
+                                       _VP, _VP, _VP]),
+        "rr_orbit_z": (C.c_int, [_VP, _VP, _I32, _I64, _VP, _I32, _VP]),
+        "rr_num_subsamples": (_I64, [_VP]),
+        "rr_num_tiles": (_I64, [_VP]),
+        "rr_get_tiles": (C.c_int, [_VP, _VP, _VP, _VP, _VP, _VP]),
+        "rr_set_reduction": (C.c_int, [_VP, _I32]),
+        "rr_evaluate_host": (C.c_int, [_VP, _VP, _VP, _I32, _I64, _VP, _VP]),
+        "rr_enable_counters": (C.c_int, [_VP, _I32]),
+        "rr_get_counters": (C.c_int, [_VP, _VP]),
+        "rr_launch_count": (_I64, [_VP]),
+        "rr_measure_fma_peak": (C.c_int, [_I32, C.POINTER(_DBL), _VP]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(lib, name)
+        f.restype, f.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def error_string(code: int) -> str:
+    return load().rr_error_string(int(code)).decode()
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise RoadRunnerError(code, where)
+
+
+def _stream(stream=None) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dev(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be contiguous {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _host(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+# ---- one-to-one wrappers of the C entry points ----------------------------------------------------
+def rr_create(nzin=50, nzlimb=50, zcut=0.7, ng=100, nk=50, k0=0.02, k1=0.2, npb=1, nkpb=1,
+              precision=RR_FP64) -> int:
+    cfg = rr_config(nzin, nzlimb, zcut, ng, nk, k0, k1, npb, nkpb, precision)
+    h = _VP()
+    _check(load().rr_create(C.byref(cfg), C.byref(h)), "rr_create")
+    return h.value
+
+
+def rr_destroy(ctx: int):
+    _check(load().rr_destroy(ctx), "rr_destroy")
+
+
+def rr_get_mu(ctx: int, nz: int) -> np.ndarray:
+    out = np.empty(nz)
+    _check(load().rr_get_mu(ctx, out.ctypes.data), "rr_get_mu")
+    return out
+
+
+def rr_get_ze(ctx: int, nz: int) -> np.ndarray:
+    out = np.empty(nz + 1)
+    _check(load().rr_get_ze(ctx, out.ctypes.data), "rr_get_ze")
+    return out
+
+
+def rr_get_weights(ctx: int, nk: int, ng: int, nz: int) -> np.ndarray:
+    out = np.empty((nk, ng, nz))
+    _check(load().rr_get_weights(ctx, out.ctypes.data), "rr_get_weights")
+    return out
+
+
+def rr_set_data(ctx: int, times, lc_index, passband_index, supersampling, exposure_time,
+                stream=None):
+    """times f64 [npt] and lc_index i32 [npt]: CUDA tensors; the per-light-curve arrays: host."""
+    import torch
+    pb, ns, et = _host(passband_index, np.int32), _host(supersampling, np.int32), \
+        _host(exposure_time, np.float64)
+    if not (pb.size == ns.size == et.size):
+        raise ValueError("passband_index, supersampling, exposure_time must have nlc entries each")
+    if times.numel() != lc_index.numel():
+        raise ValueError("times and lc_index must have npt entries each")
+    _check(load().rr_set_data(ctx, _dev(times, torch.float64, "times"),
+                              _dev(lc_index, torch.int32, "lc_index"), times.numel(),
+                              pb.ctypes.data, ns.ctypes.data, et.ctypes.data, pb.size,
+                              _stream(stream)), "rr_set_data")
+
+
+def rr_build_ld_table(ctx: int, ldp, npv: int, istar=None, stream=None):
+    """ldp [npv][npb][nz] CUDA tensor in the ctx precision."""
+    _check(load().rr_build_ld_table(ctx, _dev(ldp, ldp.dtype, "ldp"),
+                                    None if istar is None else _dev(istar, ldp.dtype, "istar"),
+                                    npv, _stream(stream)), "rr_build_ld_table")
+
+
+def rr_evaluate(ctx: int, pv, flux, status=None, stream=None):
+    """pv f64 [npv][npar] -> flux [npv][npt] (ctx precision), status i32 [npv] optional."""
+    import torch
+    npv, npar = pv.shape
+    _check(load().rr_evaluate(ctx, _dev(pv, torch.float64, "pv"), npar, npv,
+                              _dev(flux, flux.dtype, "flux"),
+                              None if status is None else _dev(status, torch.int32, "status"),
+                              _stream(stream)), "rr_evaluate")
+
+
+def rr_evaluate_flat(ctx: int, times, lc_index, passband_index, supersampling, exposure_time, pv,
+                     flux, status=None, stream=None):
+    import torch
+    pb, ns, et = _host(passband_index, np.int32), _host(supersampling, np.int32), \
+        _host(exposure_time, np.float64)
+    npv, npar = pv.shape
+    _check(load().rr_evaluate_flat(ctx, _dev(times, torch.float64, "times"),
+                                   _dev(lc_index, torch.int32, "lc_index"), times.numel(),
+                                   pb.ctypes.data, ns.ctypes.data, et.ctypes.data, pb.size,
+                                   _dev(pv, torch.float64, "pv"), npar, npv,
+                                   _dev(flux, flux.dtype, "flux"),
+                                   None if status is None else _dev(status, torch.int32, "status"),
+                                   _stream(stream)), "rr_evaluate_flat")
+
+
+def rr_orbit_z(ctx: int, pv, z, fp32_math=False, stream=None):
+    import torch
+    npv, npar = pv.shape
+    _check(load().rr_orbit_z(ctx, _dev(pv, torch.float64, "pv"), npar, npv,
+                             _dev(z, torch.float64, "z"), int(bool(fp32_math)), _stream(stream)),
+           "rr_orbit_z")
+
+
+def rr_num_subsamples(ctx: int) -> int:
+    return int(load().rr_num_subsamples(ctx))
+
+
+def rr_num_tiles(ctx: int) -> int:
+    return int(load().rr_num_tiles(ctx))
+
+
+def rr_get_tiles(ctx: int) -> dict:
+    n = rr_num_tiles(ctx)
+    if n < 0:
+        raise RoadRunnerError(-5, "rr_get_tiles")
+    start, count, lc = (np.empty(n, np.int32) for _ in range(3))
+    tmin, tmax = np.empty(n), np.empty(n)
+    _check(load().rr_get_tiles(ctx, start.ctypes.data, count.ctypes.data, lc.ctypes.data,
+                               tmin.ctypes.data, tmax.ctypes.data), "rr_get_tiles")
+    return dict(start=start, count=count, lc=lc, tmin=tmin, tmax=tmax)
+
+
+def rr_set_reduction(ctx: int, mode: int):
+    _check(load().rr_set_reduction(ctx, mode), "rr_set_reduction")
+
+
+def rr_evaluate_host(ctx: int, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray,
+                     status: np.ndarray | None = None):
+    """Whole step from HOST arrays (numpy, or the .numpy() view of a pinned torch tensor)."""
+    if not (ldp.flags.c_contiguous and pv.flags.c_contiguous and flux.flags.c_contiguous):
+        raise TypeError("host arrays must be C-contiguous")
+    if pv.dtype != np.float64 or ldp.dtype != flux.dtype:
+        raise TypeError("pv must be float64; ldp and flux must share the ctx precision")
+    npv, npar = pv.shape
+    _check(load().rr_evaluate_host(ctx, ldp.ctypes.data, pv.ctypes.data, npar, npv,
+                                   flux.ctypes.data,
+                                   None if status is None else status.ctypes.data),
+           "rr_evaluate_host")
+
+
+def rr_enable_counters(ctx: int, on: bool):
+    _check(load().rr_enable_counters(ctx, int(bool(on))), "rr_enable_counters")
+
+
+COUNTER_NAMES = ("skipped", "circular", "eccentric", "occulting", "ingress", "solver_iters",
+                 "tiles_filled", "tiles_evaluated")
+
+
+def rr_get_counters(ctx: int) -> dict:
+    out = np.zeros(8, np.int64)
+    _check(load().rr_get_counters(ctx, out.ctypes.data), "rr_get_counters")
+    return dict(zip(COUNTER_NAMES, (int(x) for x in out)))
+
+
+def rr_launch_count(ctx: int) -> int:
+    return int(load().rr_launch_count(ctx))
+
+
+def rr_measure_fma_peak(precision=RR_FP64, stream=None) -> float:
+    v = _DBL()
+    _check(load().rr_measure_fma_peak(precision, C.byref(v), _stream(stream)),
+           "rr_measure_fma_peak")
+    return v.value
+
+
+# ---- convenience wrapper ----------------------------------------------------------------------------
+class RoadRunner:
+    """The paper's call pattern over the C-ABI.  Holds the ctx handle."""
+
+    def __init__(self, nzin=50, nzlimb=50, zcut=0.7, ng=100, nk=50, k0=0.02, k1=0.2, npb=1,
+                 nkpb=1, precision=RR_FP64):
+        import torch
+        self.nz, self.ng, self.nk, self.npb, self.nkpb = nzin + nzlimb, ng, nk, npb, nkpb
+        self.precision = precision
+        self.dtype = torch.float32 if precision == RR_FP32 else torch.float64
+        self.ctx = rr_create(nzin, nzlimb, zcut, ng, nk, k0, k1, npb, nkpb, precision)
+        self.mu = rr_get_mu(self.ctx, self.nz)
+        self.ze = rr_get_ze(self.ctx, self.nz)
+        self.npt = 0
+        self.npv = 0
+
+    @classmethod
+    def from_config(cls, m, precision=RR_FP64):
+        return cls(m.nzin, m.nzlimb, m.zcut, m.ng, m.nk, m.k0, m.k1, m.npb, m.nkpb, precision)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            rr_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def weights(self) -> np.ndarray:
+        return rr_get_weights(self.ctx, self.nk, self.ng, self.nz)
+
+    def set_data(self, times, lc_index, passband_index, supersampling, exposure_time):
+        import torch
+        t = torch.as_tensor(np.ascontiguousarray(times, np.float64)).cuda()
+        lc = torch.as_tensor(np.ascontiguousarray(lc_index, np.int32)).cuda()
+        rr_set_data(self.ctx, t, lc, passband_index, supersampling, exposure_time)
+        self.npt = t.numel()
+
+    def build_ld_table(self, ldp, istar=None):
+        """ldp: CUDA tensor or array [npv][npb][nz]."""
+        import torch
+        if not isinstance(ldp, torch.Tensor):
+            ldp = torch.as_tensor(np.ascontiguousarray(ldp)).to(self.dtype).cuda()
+        ldp = ldp.reshape(-1, self.npb, self.nz).contiguous()
+        if istar is not None and not isinstance(istar, torch.Tensor):
+            istar = torch.as_tensor(np.ascontiguousarray(istar)).to(self.dtype).cuda()
+        self.npv = ldp.shape[0]
+        rr_build_ld_table(self.ctx, ldp, self.npv, istar)
+
+    def table(self):
+        """Copy of T[npv][npb][nk][ng] and Istar[npv][npb] as numpy arrays (diagnostics)."""
+        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        T = np.empty((self.npv, self.npb, self.nk, self.ng), npdt)
+        I = np.empty((self.npv, self.npb), npdt)
+        _check(load().rr_get_table(self.ctx, T.ctypes.data, I.ctypes.data), "rr_get_table")
+        return T, I
+
+    def evaluate(self, pv, want_status=False):
+        """pv: CUDA tensor or array [npv][nkpb+6] -> flux CUDA tensor [npv][npt]."""
+        import torch
+        if not isinstance(pv, torch.Tensor):
+            pv = torch.as_tensor(np.ascontiguousarray(pv, np.float64)).cuda()
+        pv = pv.reshape(-1, self.nkpb + 6).contiguous()
+        flux = torch.empty((pv.shape[0], self.npt), dtype=self.dtype, device="cuda")
+        status = torch.empty(pv.shape[0], dtype=torch.int32, device="cuda")
+        rr_evaluate(self.ctx, pv, flux, status)
+        return (flux, status) if want_status else flux
+
+    def orbit_z(self, pv, fp32_math=False):
+        import torch
+        if not isinstance(pv, torch.Tensor):
+            pv = torch.as_tensor(np.ascontiguousarray(pv, np.float64)).cuda()
+        pv = pv.reshape(-1, self.nkpb + 6).contiguous()
+        z = torch.empty((pv.shape[0], rr_num_subsamples(self.ctx)), dtype=torch.float64,
+                        device="cuda")
+        rr_orbit_z(self.ctx, pv, z, fp32_math)
+        return z
+
+    def evaluate_host(self, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray | None = None,
+                      status: np.ndarray | None = None):
+        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        ldp = np.ascontiguousarray(ldp, npdt).reshape(-1, self.npb, self.nz)
+        pv = np.ascontiguousarray(pv, np.float64).reshape(-1, self.nkpb + 6)
+        if flux is None:
+            flux = np.empty((pv.shape[0], self.npt), npdt)
+        rr_evaluate_host(self.ctx, ldp, pv, flux, status)
+        return flux

@@ -1,0 +1,133 @@
+// rr_common.cuh - shared declarations of the CUDA library (product code; no oracle code here).
+// Method: H. Parviainen, arXiv:2009.08500 (citations: PAPER.md lines).  Layout: DESIGN.md s5.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/roadrunner.h"
+
+#define RR_PI 3.14159265358979323846264338327950288
+#define RR_TWOPI 6.28318530717958647692528676655900577
+
+// ---- device-resident descriptors -----------------------------------------------------------
+// Per light curve (kernel 4 input): PAPER.md:230-236.
+struct RRLc {
+  double exptime;    // exposure time tau (days)
+  int32_t ns;        // sub-samples per exposure
+  int32_t pb;        // passband
+  int32_t tile_len;  // exposures per dispatch tile
+  int32_t shuffle;   // 1: sub-samples across lanes (warp-shuffle reduction)
+};
+
+// One dispatch tile (kernel 4 output): a run of exposures of ONE light curve.
+struct RRTile {
+  double tmin, tmax;  // range of the mid-exposure times in the tile
+  int64_t sub_off;    // index of the tile's first sub-sample in a [nsub] row (rr_orbit_z)
+  int32_t start;      // first exposure
+  int32_t count;      // exposures in the tile
+  int32_t lc;         // light curve
+  int32_t pad;
+};
+
+// Per parameter vector, orbit part (kernel 2's per-pv work, done once per rr_evaluate).
+// Phases are in turns of the orbit relative to t0; E_tr is the eccentric anomaly at inferior
+// conjunction (true anomaly pi/2 - w, reading R8).
+struct RRPvOrbit {
+  double t0, inv_p;
+  double u_lo, u_hi;   // transit window: z < 1+k and in front is only possible inside it
+  double a2;           // a^2
+  double ci2, omci2;   // cos^2 i, 1 - cos^2 i
+  double e, sE, cE;    // e, sin E_tr, cos E_tr
+  double beta;         // sqrt(1-e^2)
+  double sw, cw;       // sin w, cos w
+  double rho_tr;       // r(t0)/a = (1-e^2)/(1+e sin w)
+  int32_t status;      // RR_PV_* bits; != 0 -> NaN row
+  int32_t circular;    // e == 0
+};
+
+// Per (parameter vector, k-band): radius-ratio constants.
+struct RRPvBand {
+  double k, opk;       // k, 1+k
+  double omk;          // |1-k|: z <= omk -> full overlap
+  double afull;        // pi * min(1,k)^2
+  double k2;           // k^2
+  double gscale;       // (ng-1)/(1+k): y = z*gscale is the g coordinate in table cells
+  double ak;           // weight of table row ik+1
+  int32_t ik;          // lower k row, clamped to nk-2 (reading R10)
+  int32_t pad;
+};
+
+// Per-evaluation device buffers: one set for the device-pointer API, one per slot of the
+// host-buffer path (so that two chunks can be in flight on two streams).
+struct RRWork {
+  void *T, *istar;          // kernel 1 output (ctx precision)
+  int64_t table_npv;        // npv of the table built last; -1 = none
+  int64_t T_cap, istar_cap; // bytes
+  RRPvOrbit *pvo;
+  RRPvBand *pvb;
+  int64_t pv_cap;
+};
+
+// ---- host context -----------------------------------------------------------------------------
+struct rr_ctx {
+  rr_config cfg;
+  int nz;
+  int device;
+  int sm_count;
+  // geometry (a0)
+  double *d_ze, *d_zm, *d_mu, *d_q, *d_W;
+  std::vector<double> h_ze, h_mu;
+  // data (kernel 4)
+  int64_t npt;
+  int32_t nlc;
+  double *d_times;
+  int32_t *d_lc_index;
+  RRLc *d_lc;
+  std::vector<RRLc> h_lc;
+  RRTile *d_tiles;
+  int64_t ntiles, tiles_cap;
+  int64_t nsub;
+  int64_t *d_scratch;   // dispatch scratch
+  int64_t scratch_cap;
+  int32_t reduction;
+  int32_t any_shuffle;
+  // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
+  RRWork work[3];
+  // counters / accounting
+  unsigned long long *d_counters;
+  int32_t counters_on;
+  int64_t launches;
+  // host path
+  cudaStream_t hs[2];
+  cudaEvent_t hev[2];
+  void *d_host_stage[2][4];   // per slot: ldp, pv, flux, status
+  int64_t host_stage_cap[2][4];
+};
+
+// ---- error plumbing -----------------------------------------------------------------------------
+#define RR_CUDA(call)                                          \
+  do {                                                         \
+    cudaError_t _e = (call);                                   \
+    if (_e != cudaSuccess) return RR_ECUDA_BASE - (int)_e;     \
+  } while (0)
+
+#define RR_LAUNCH_CHECK(ctx)                                   \
+  do {                                                         \
+    (ctx)->launches++;                                         \
+    cudaError_t _e = cudaGetLastError();                       \
+    if (_e != cudaSuccess) return RR_ECUDA_BASE - (int)_e;     \
+  } while (0)
+
+// ---- internal entry points of the kernel files ---------------------------------------------------
+int rr_geometry_build(rr_ctx *ctx);                                            // rr_geometry.cu
+int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp,             // rr_ld_table.cu
+                       const void *d_istar, int64_t npv, cudaStream_t st);
+int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu
+int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
+                      int32_t *d_status, cudaStream_t st);                     // rr_flux.cu
+int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStream_t st);
+int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_math,
+                    cudaStream_t st);
+int rr_fma_peak_launch(int precision, double *h_fma_per_s, cudaStream_t st);   // rr_flux.cu

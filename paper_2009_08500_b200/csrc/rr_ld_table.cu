@@ -1,0 +1,172 @@
+// rr_ld_table.cu - kernel 1: the per-call limb-darkening table.
+//   T[row][n] = sum_j W[n][j] * ldp[row][j],   row = pv*npb + pb,  n = ik*ng + ig,  j < nz
+//   Istar[row] = sum_j q[j] * ldp[row][j],     q[j] = pi (ze[j+1]^2 - ze[j]^2)    (reading R6)
+// A "TN" matrix product C[M][N] = A[M][K] . B[N][K]^T with M = npv*npb, N = nk*ng (5000),
+// K = nz (100..200), both operands K-contiguous.  fp64 FMA accumulation in k order for both ctx
+// precisions (the fp32 mode only narrows the operand A on load and C on store).  It is a skinny
+// product worth a few per cent of a step: a register-blocked DFMA kernel, 128x128
+// block tile, 8x8 micro tile, operands staged k-major in shared memory with register prefetch of
+// the next k slab.  B200's DMMA rate equals its DFMA rate, so tensor cores would buy nothing here.
+#include "rr_common.cuh"
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 16, PAD = 2, NT = 256;
+
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+
+template <typename TA, typename TC>
+__global__ void __launch_bounds__(NT, 1)
+rr_ld_table_kernel(const TA *__restrict__ A, const double *__restrict__ B, TC *__restrict__ C,
+                   int64_t M, int N, int K) {
+  __shared__ __align__(16) double As[BK][BM + PAD];
+  __shared__ __align__(16) double Bs[BK][BN + PAD];
+  const int t = threadIdx.x;
+  const int tx = t & 15, ty = t >> 4;
+  const int64_t m0 = (int64_t)blockIdx.y * BM;
+  const int n0 = blockIdx.x * BN;
+  // loader mapping: thread -> (row r of the tile, k half h): 8 consecutive k of one row
+  const int lr = t >> 1, lh = (t & 1) * 8;
+  const int64_t am = m0 + lr;
+  const int bn = n0 + lr;
+  const bool a_ok = am < M, b_ok = bn < N;
+  const TA *ap = A + (a_ok ? am : 0) * (int64_t)K;
+  const double *bp = B + (int64_t)(b_ok ? bn : 0) * K;
+
+  double acc[8][8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[i][j] = 0.0;
+
+  double ra[8], rb[8];
+  auto gload = [&](int kb) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      int k = kb + lh + q;
+      bool kin = k < K;
+      ra[q] = (a_ok && kin) ? (double)ap[k] : 0.0;
+      rb[q] = (b_ok && kin) ? bp[k] : 0.0;
+    }
+  };
+  gload(0);
+  for (int kb = 0; kb < K; kb += BK) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      As[lh + q][lr] = ra[q];
+      Bs[lh + q][lr] = rb[q];
+    }
+    __syncthreads();
+    if (kb + BK < K) gload(kb + BK);
+#pragma unroll
+    for (int kk = 0; kk < BK; ++kk) {
+      double a[8], b[8];
+#pragma unroll
+      for (int i = 0; i < 8; i += 2) {
+        double2 v = *reinterpret_cast<const double2 *>(&As[kk][ty * 8 + i]);
+        a[i] = v.x;
+        a[i + 1] = v.y;
+      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        double2 v = *reinterpret_cast<const double2 *>(&Bs[kk][tx * 2 + 32 * c]);
+        b[2 * c] = v.x;
+        b[2 * c + 1] = v.y;
+      }
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+  // epilogue: 16 lanes x 16 B contiguous per row
+  const bool vec_ok = (N & 1) == 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    int64_t m = m0 + ty * 8 + i;
+    if (m >= M) continue;
+    TC *crow = C + m * (int64_t)N;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      int n = n0 + tx * 2 + 32 * c;
+      if (vec_ok && n + 1 < N) {
+        typename Vec2<TC>::type v;
+        v.x = (TC)acc[i][2 * c];
+        v.y = (TC)acc[i][2 * c + 1];
+        *reinterpret_cast<typename Vec2<TC>::type *>(crow + n) = v;
+      } else {
+        if (n < N) crow[n] = (TC)acc[i][2 * c];
+        if (n + 1 < N) crow[n + 1] = (TC)acc[i][2 * c + 1];
+      }
+    }
+  }
+}
+
+// Istar: one warp per row.
+template <typename TA, typename TC>
+__global__ void rr_istar_kernel(const TA *__restrict__ A, const double *__restrict__ q,
+                                const TC *__restrict__ given, TC *__restrict__ out, int64_t M,
+                                int K) {
+  int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  if (given) {
+    if (lane == 0) out[row] = given[row];
+    return;
+  }
+  double s = 0.0;
+  for (int j = lane; j < K; j += 32) s = fma(q[j], (double)A[row * K + j], s);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane == 0) out[row] = (TC)s;
+}
+
+template <typename TR>
+int launch_typed(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar, int64_t npv,
+                 cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  int64_t M = npv * c.npb;
+  int N = c.nk * c.ng, K = ctx->nz;
+  dim3 grid((N + BN - 1) / BN, (unsigned)((M + BM - 1) / BM));
+  rr_ld_table_kernel<TR, TR><<<grid, NT, 0, st>>>((const TR *)d_ldp, ctx->d_W, (TR *)wk->T, M,
+                                                  N, K);
+  RR_LAUNCH_CHECK(ctx);
+  int64_t threads = M * 32;
+  rr_istar_kernel<TR, TR><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+      (const TR *)d_ldp, ctx->d_q, (const TR *)d_istar, (TR *)wk->istar, M, K);
+  RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
+}  // namespace
+
+// Grows wk->T / wk->istar as needed (cudaMalloc: synchronous, only when a larger npv arrives).
+int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar,
+                       int64_t npv, cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t needT = npv * c.npb * (int64_t)c.nk * c.ng * esz, needI = npv * c.npb * esz;
+  if (needT > wk->T_cap) {
+    if (wk->T) cudaFree(wk->T);
+    wk->T = nullptr;
+    wk->T_cap = 0;
+    wk->table_npv = -1;
+    if (cudaMalloc(&wk->T, needT) != cudaSuccess) { cudaGetLastError(); return RR_EALLOC; }
+    wk->T_cap = needT;
+  }
+  if (needI > wk->istar_cap) {
+    if (wk->istar) cudaFree(wk->istar);
+    wk->istar = nullptr;
+    wk->istar_cap = 0;
+    wk->table_npv = -1;
+    if (cudaMalloc(&wk->istar, needI) != cudaSuccess) { cudaGetLastError(); return RR_EALLOC; }
+    wk->istar_cap = needI;
+  }
+  int rc = c.precision == RR_FP32 ? launch_typed<float>(ctx, wk, d_ldp, d_istar, npv, st)
+                                  : launch_typed<double>(ctx, wk, d_ldp, d_istar, npv, st);
+  wk->table_npv = rc == RR_OK ? npv : -1;
+  return rc;
+}

@@ -1,0 +1,428 @@
+"""GPU parity: the CUDA library (through its C-ABI binding) against the CPU oracle, element by
+element, on the seeded workloads of BASELINE.json at sizes the oracle finishes in seconds that
+still span several dispatch tiles and a ragged tail; plus sampled checks at full size.
+
+Tolerances (BASELINE.json north_star): fp64 |flux_gpu - flux_oracle| <= 1e-9 absolute;
+fp32 <= 2e-7 absolute.  Integer work (dispatch tiles, status words) is bit-exact.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-9
+TOL32 = 2e-7
+
+
+@pytest.fixture(scope="module")
+def rr():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device (there is no CPU fallback)")
+    import paper_2009_08500_b200 as m
+    m.load()
+    return m
+
+
+def gpu_model(rr, wl, precision=0):
+    model = rr.RoadRunner.from_config(wl.model, precision)
+    model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
+    return model
+
+
+def gpu_flux(rr, wl, precision=0, reduction=0, want_status=False):
+    model = gpu_model(rr, wl, precision)
+    if reduction:
+        rr.rr_set_reduction(model.ctx, reduction)
+    model.build_ld_table(wl.ldp(model.mu))
+    flux, status = model.evaluate(wl.pv, want_status=True)
+    out = flux.cpu().numpy().astype(np.float64), status.cpu().numpy()
+    model.close()
+    return out if want_status else out[0]
+
+
+def oracle_flux(wl):
+    flux, status = oracle.evaluate_workload(wl, nthreads=0)
+    return flux, status
+
+
+SMALL = {  # config -> (npv, npt): several tiles per light curve and a ragged tail
+    0: (None, None),
+    1: (48, 5000),
+    2: (12, 3000),
+    3: (10, 6 * 2500),
+    4: (40, 7001),
+}
+
+
+def small_workload(config):
+    npv, npt = SMALL[config]
+    return workloads.make_workload(config, npv=npv, npt=npt)
+
+
+# ---- a0: geometry ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", [dict(), dict(nzin=100, nzlimb=100, npb=4),
+                                 dict(k0=0.01, k1=0.3), dict(nzin=7, nzlimb=5, ng=11, nk=3)])
+def test_geometry_matches_oracle(rr, cfg):
+    mc = workloads.ModelConfig(**cfg)
+    om = oracle.OracleModel.from_config(mc)
+    gm = rr.RoadRunner.from_config(mc)
+    assert np.max(np.abs(gm.ze - om.ze)) <= 4e-16
+    assert np.max(np.abs(gm.mu - om.mu)) <= 4e-16
+    W = gm.weights()
+    assert W.shape == om.W.shape
+    assert np.max(np.abs(W - om.W)) <= 1e-11
+    assert np.max(np.abs(W.sum(axis=2) - 1.0)) <= 1e-12
+    gm.close()
+
+
+# ---- kernel 1: LD table --------------------------------------------------------------------------------
+@pytest.mark.parametrize("config,npv", [(0, None), (1, 300), (3, 37)])
+def test_ld_table_matches_oracle(rr, config, npv):
+    wl = workloads.make_workload(config, npv=npv, npt=600)
+    om = oracle.OracleModel.from_config(wl.model)
+    T_o, I_o = om.build_ld_table(wl.ldp(om.mu))
+    gm = rr.RoadRunner.from_config(wl.model)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    T_g, I_g = gm.table()
+    assert T_g.shape == T_o.shape
+    assert np.max(np.abs(T_g - T_o)) <= 1e-12
+    assert np.max(np.abs(I_g / I_o - 1.0)) <= 1e-13
+    gm.close()
+
+
+def test_ld_table_istar_override(rr):
+    wl = workloads.make_workload(1, npv=5, npt=300)
+    gm = gpu_model(rr, wl)
+    ldp = wl.ldp(gm.mu)
+    given = np.linspace(2.0, 3.0, 5).reshape(5, 1)
+    gm.build_ld_table(ldp, istar=given)
+    _, I_g = gm.table()
+    assert np.array_equal(I_g, given)
+    flux_g = gm.evaluate(wl.pv).cpu().numpy()
+    om = oracle.OracleModel.from_config(wl.model)
+    om.build_ld_table(wl.ldp(om.mu), istar_override=given)
+    flux_o, _ = om.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                            wl.exposure_time, wl.pv)
+    assert np.max(np.abs(flux_g - flux_o)) <= TOL64
+    gm.close()
+
+
+# ---- kernels 2+3+4: flux, fp64 ---------------------------------------------------------------------------
+@pytest.mark.parametrize("config", [0, 1, 2, 3, 4])
+def test_flux_fp64_matches_oracle(rr, config):
+    wl = small_workload(config)
+    want, st_o = oracle_flux(wl)
+    got, st_g = gpu_flux(rr, wl, want_status=True)
+    assert got.shape == want.shape
+    assert np.array_equal(st_g, st_o)
+    err = np.abs(got - want)
+    assert np.max(err) <= TOL64, (config, float(np.max(err)))
+    # out of transit is 1 exactly on both sides
+    assert np.array_equal(got == 1.0, want == 1.0) or np.max(err[(got == 1.0) != (want == 1.0)]) <= 1e-12
+    assert (want < 1.0).sum() > 100 or config == 0
+
+
+@pytest.mark.parametrize("config", [2, 3, 4])
+def test_flux_fp32_matches_oracle(rr, config):
+    wl = small_workload(config)
+    want, _ = oracle_flux(wl)
+    got = gpu_flux(rr, wl, precision=1)
+    err = np.abs(got - want)
+    assert np.max(err) <= TOL32, (config, float(np.max(err)))
+
+
+@pytest.mark.parametrize("config", [2, 3])
+@pytest.mark.parametrize("precision", [0, 1])
+def test_reduction_layouts_agree(rr, config, precision):
+    """Thread-per-exposure loop and lanes-over-sub-samples warp-shuffle sum: same flux."""
+    wl = small_workload(config)
+    want, _ = oracle_flux(wl)
+    a = gpu_flux(rr, wl, precision, reduction=1)
+    b = gpu_flux(rr, wl, precision, reduction=2)
+    tol = TOL32 if precision else TOL64
+    assert np.max(np.abs(a - want)) <= tol
+    assert np.max(np.abs(b - want)) <= tol
+    assert np.max(np.abs(a - b)) <= (1e-6 if precision else 1e-14)
+
+
+# ---- kernel 2 alone ------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config", [1, 3, 4])
+def test_orbit_z_matches_oracle(rr, config):
+    wl = workloads.make_workload(config, npv=24, npt=6 * 200 if config == 3 else 1500)
+    _, _, z_o = oracle.evaluate_workload(wl, want_z=True)
+    gm = gpu_model(rr, wl)
+    assert rr.rr_num_subsamples(gm.ctx) == z_o.shape[1]
+    z_g = gm.orbit_z(wl.pv).cpu().numpy()
+    assert np.max(np.abs(z_g - z_o)) <= 1e-11 * max(1.0, float(np.max(np.abs(z_o))))
+    z32 = gm.orbit_z(wl.pv, fp32_math=True).cpu().numpy()
+    near = np.abs(z_o) < 1.5         # the part of the orbit that matters: relative 1e-6
+    assert np.max(np.abs(np.abs(z32[near]) - np.abs(z_o[near]))) <= 2e-6
+    gm.close()
+
+
+def test_orbit_high_eccentricity_full_phase(rr):
+    """Solver robustness away from the transit window: e up to 0.95, every phase."""
+    rng = np.random.default_rng(7)
+    n = 64
+    pv = np.empty((n, 7))
+    pv[:, 0] = 0.1
+    pv[:, 1] = rng.uniform(-0.5, 0.5, n)
+    pv[:, 2] = rng.uniform(1.0, 5.0, n)
+    pv[:, 3] = rng.uniform(30.0, 60.0, n)
+    pv[:, 4] = rng.uniform(1.3, 1.6, n)
+    pv[:, 5] = np.linspace(0.0, 0.95, n)
+    pv[:, 6] = rng.uniform(0, 2 * np.pi, n)
+    times = np.linspace(-6.0, 6.0, 2400)
+    mc = workloads.ModelConfig()
+    gm = rr.RoadRunner.from_config(mc)
+    gm.set_data(times, np.zeros(times.size, np.int32), [0], [1], [0.0])
+    z_g = gm.orbit_z(pv).cpu().numpy()
+    z_o = np.array([[(lambda zf: zf[0] if zf[1] else -zf[0])(oracle.separation(t, *row[1:]))
+                     for t in times] for row in pv])
+    assert np.max(np.abs(z_g - z_o) / np.maximum(1.0, np.abs(z_o))) <= 1e-11
+    gm.close()
+
+
+# ---- kernel 4: dispatch -----------------------------------------------------------------------------------
+def expected_tiles(lc_index, supersampling):
+    """Runs of equal lc_index cut into tiles of 256*R exposures, R = clamp((8+ns//2)//ns, 1, 8)."""
+    tiles = []
+    n = len(lc_index)
+    b = 0
+    while b < n:
+        e = b
+        while e < n and lc_index[e] == lc_index[b]:
+            e += 1
+        ns = int(supersampling[lc_index[b]])
+        length = 256 * max(1, min(8, (8 + ns // 2) // ns))
+        for s in range(b, e, length):
+            tiles.append((s, min(length, e - s), int(lc_index[b])))
+        b = e
+    return tiles
+
+
+@pytest.mark.parametrize("case", ["config3", "interleaved", "single", "paper"])
+def test_dispatch_tiles(rr, case):
+    rng = np.random.default_rng(11)
+    if case == "config3":
+        wl = workloads.make_workload(3, npv=1, npt=6 * 2500)
+        times, lc, pb, ns, et = wl.times, wl.lc_index, wl.passband_index, wl.supersampling, \
+            wl.exposure_time
+        npb = 4
+    elif case == "interleaved":
+        lc = rng.integers(0, 3, 5000).astype(np.int32)
+        lc[1000:3500] = 2
+        times = rng.uniform(-1, 1, lc.size)
+        pb, ns, et, npb = [0, 1, 0], [1, 7, 30], [0.0, 0.01, 0.02], 2
+    elif case == "single":
+        lc = np.zeros(1, np.int32)
+        times = np.array([0.25])
+        pb, ns, et, npb = [0], [3], [0.01], 1
+    else:
+        d = workloads.paper_dummy_example()
+        times, lc, pb = d["times"], d["lc_index"], d["passband_index"]
+        ns, et, npb = [1, 2, 3], [0.0, 0.1, 0.2], 2
+    gm = rr.RoadRunner(npb=npb)
+    gm.set_data(times, lc, pb, ns, et)
+    got = rr.rr_get_tiles(gm.ctx)
+    want = expected_tiles(lc, ns)
+    assert rr.rr_num_tiles(gm.ctx) == len(want)
+    assert [(int(s), int(c), int(l)) for s, c, l in zip(got["start"], got["count"], got["lc"])] \
+        == want
+    for (s, c, _), lo, hi in zip(want, got["tmin"], got["tmax"]):
+        assert lo == times[s:s + c].min() and hi == times[s:s + c].max()
+    assert rr.rr_num_subsamples(gm.ctx) == int(np.asarray(ns)[lc].sum())
+    gm.close()
+
+
+def test_paper_dummy_example_indexing(rr):
+    """points 0,1,5 use passband 0's table, points 2,3,4 passband 1's."""
+    d = workloads.paper_dummy_example()
+    times = d["times"] * 0.02 - 0.05
+    mc = workloads.ModelConfig(npb=2)
+    pv = np.array([[0.1, 0.0, 3.0, 8.0, np.deg2rad(88.0), 0.0, 0.0],
+                   [0.15, 0.01, 2.0, 6.0, np.deg2rad(87.0), 0.2, 1.0]])
+    coeffs = np.array([[[0.4, 0.2], [0.7, 0.1]], [[0.3, 0.3], [0.1, 0.05]]])
+    ns, et = [1, 3, 2], [0.0, 0.01, 0.02]
+    om = oracle.OracleModel.from_config(mc)
+    om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+    want, _ = om.evaluate(times, d["lc_index"], d["passband_index"], ns, et, pv)
+    gm = rr.RoadRunner.from_config(mc)
+    gm.set_data(times, d["lc_index"], d["passband_index"], ns, et)
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy()
+    assert np.max(np.abs(got - want)) <= TOL64
+    assert (want < 1).all()
+    gm.close()
+
+
+def test_unsorted_times_and_out_of_order_light_curves(rr):
+    wl = workloads.make_workload(3, npv=6, npt=6 * 700)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(wl.npt)
+    wl = wl.subset_times(perm)
+    want, _ = oracle_flux(wl)
+    got = gpu_flux(rr, wl)
+    assert np.max(np.abs(got - want)) <= TOL64
+
+
+# ---- edge cases ---------------------------------------------------------------------------------------------
+def test_invalid_parameter_vectors_give_nan_rows(rr):
+    wl = workloads.make_workload(4, npv=12, npt=900)
+    pv = wl.pv.copy()
+    pv[1, 0] = 0.5          # k above k1
+    pv[2, 5] = 1.0          # e = 1
+    pv[3, 3] = -1.0         # a <= 0
+    pv[4, 2] = 0.0          # p <= 0
+    pv[5, 1] = np.nan
+    pv[6, 0] = 0.001        # k below k0
+    pv[7, 5] = -0.1
+    wl.pv = pv
+    want, st_o = oracle_flux(wl)
+    got, st_g = gpu_flux(rr, wl, want_status=True)
+    assert np.array_equal(st_g, st_o)
+    assert list(st_g[:8]) == [0, 1, 2, 4, 8, 16, 1, 2]
+    assert np.array_equal(np.isnan(got), np.isnan(want))
+    ok = ~np.isnan(want)
+    assert np.max(np.abs(got[ok] - want[ok])) <= TOL64
+
+
+def test_grazing_wide_window_and_secondary_eclipse(rr):
+    """a(1-e) barely above 1+k (window = whole orbit), periods short enough that the time span
+    reaches the secondary-eclipse phase (flux must be 1 there), k at both table edges."""
+    mc = workloads.ModelConfig()
+    pv = np.array([
+        [0.2, 0.0, 1.0, 1.25, np.deg2rad(80.0), 0.0, 0.0],
+        [0.02, 0.1, 0.7, 2.0, np.deg2rad(89.0), 0.45, 4.0],
+        [0.2, -0.2, 0.9, 3.0, np.deg2rad(75.0), 0.55, 1.0],
+        [0.11, 0.0, 1.3, 1.6, np.deg2rad(60.0), 0.1, 2.5],
+        [0.05, 0.3, 5.0, 12.0, np.deg2rad(90.0), 0.0, 0.0],
+    ])
+    times = np.linspace(-1.0, 1.0, 4001)
+    coeffs = np.tile(np.array([[[0.5, 0.1]]]), (pv.shape[0], 1, 1))
+    for ns, tau in ((1, 0.0), (4, 0.03)):
+        om = oracle.OracleModel.from_config(mc)
+        om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+        want, _ = om.evaluate(times, np.zeros(times.size, np.int32), [0], [ns], [tau], pv)
+        gm = rr.RoadRunner.from_config(mc)
+        gm.set_data(times, np.zeros(times.size, np.int32), [0], [ns], [tau])
+        gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+        got = gm.evaluate(pv).cpu().numpy()
+        assert np.max(np.abs(got - want)) <= TOL64
+        gm.close()
+
+
+def test_uniform_disk_closed_form(rr):
+    """ldp = 1: flux = 1 - a(z,k)/pi straight from the CUDA path."""
+    wl = workloads.make_workload(1, npv=8, npt=2000)
+    wl.ld_kind = "uniform"
+    gm = gpu_model(rr, wl)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    flux = gm.evaluate(wl.pv).cpu().numpy()
+    z = np.abs(gm.orbit_z(wl.pv).cpu().numpy())
+    for v in range(wl.npv):
+        k = wl.pv[v, 0]
+        want = np.array([1.0 - oracle.lens_area(1.0, k, zz) / np.pi for zz in z[v]])
+        assert np.max(np.abs(flux[v] - want)) <= 1e-13
+    gm.close()
+
+
+def test_chromatic_k(rr):
+    """k per passband: pv rows carry npb radius ratios."""
+    mc = workloads.ModelConfig(npb=2, nkpb=2)
+    rng = np.random.default_rng(3)
+    base = workloads.make_workload(1, npv=6, npt=10)
+    pv = np.concatenate([base.pv[:, :1], base.pv[:, :1] * rng.uniform(0.9, 1.1, (6, 1)),
+                         base.pv[:, 1:]], axis=1)
+    pv[:, :2] = np.clip(pv[:, :2], 0.02, 0.2)
+    times = np.tile(np.linspace(-0.2, 0.2, 900), 2)
+    lc = np.repeat(np.arange(2, dtype=np.int32), 900)
+    coeffs = rng.uniform(0.1, 0.4, (6, 2, 2))
+    om = oracle.OracleModel.from_config(mc)
+    om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+    want, _ = om.evaluate(times, lc, [0, 1], [1, 3], [0.0, 0.01], pv)
+    gm = rr.RoadRunner.from_config(mc)
+    gm.set_data(times, lc, [0, 1], [1, 3], [0.0, 0.01])
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy()
+    assert np.max(np.abs(got - want)) <= TOL64
+    gm.close()
+
+
+def test_argument_errors(rr):
+    import torch
+    gm = rr.RoadRunner()
+    pv = torch.zeros((2, 7), dtype=torch.float64, device="cuda")
+    flux = torch.zeros((2, 10), dtype=torch.float64, device="cuda")
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_evaluate(gm.ctx, pv, flux)               # no data, no table
+    assert e.value.code == -5
+    t = torch.linspace(-0.1, 0.1, 10, dtype=torch.float64, device="cuda")
+    lc = torch.zeros(10, dtype=torch.int32, device="cuda")
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_set_data(gm.ctx, t, lc, [1], [1], [0.0])  # passband out of range
+    assert e.value.code == -4
+    bad = lc.clone()
+    bad[3] = 2
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_set_data(gm.ctx, t, bad, [0], [1], [0.0])  # lc_index out of range (found on device)
+    assert e.value.code == -4
+    rr.rr_set_data(gm.ctx, t, lc, [0], [1], [0.0])
+    gm.npt = 10
+    gm.build_ld_table(np.ones((3, 1, 100)))
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_evaluate(gm.ctx, pv, flux)               # table npv 3 != 2
+    assert e.value.code == -5
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_evaluate(gm.ctx, torch.zeros((3, 6), dtype=torch.float64, device="cuda"), flux)
+    assert e.value.code == -3
+    with pytest.raises(rr.RoadRunnerError):
+        rr.rr_create(ng=1)
+    gm.close()
+
+
+# ---- host-buffer path -----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", [0, 1])
+def test_host_path_equals_device_path(rr, precision):
+    wl = workloads.make_workload(4, npv=700, npt=60000)      # > 1 chunk of 256 MB flux in fp64
+    gm = gpu_model(rr, wl, precision)
+    ldp = wl.ldp(gm.mu)
+    gm.build_ld_table(ldp)
+    dev, st_dev = gm.evaluate(wl.pv, want_status=True)
+    status = np.empty(wl.npv, np.int32)
+    host = gm.evaluate_host(ldp, wl.pv, status=status)
+    assert np.array_equal(host, dev.cpu().numpy())
+    assert np.array_equal(status, st_dev.cpu().numpy())
+    gm.close()
+
+
+# ---- full size, the launch configuration bench.py times ----------------------------------------------------
+@pytest.mark.parametrize("config,precision", [(4, 0), (4, 1), (3, 0), (2, 0)])
+def test_full_size_sampled(rr, config, precision):
+    """Full BASELINE size on the GPU; the oracle recomputes sampled (pv, exposure) pairs."""
+    wl = workloads.make_workload(config)
+    gm = gpu_model(rr, wl, precision)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    flux = gm.evaluate(wl.pv)
+    rng = np.random.default_rng(100 + config)
+    pvs = np.sort(rng.choice(wl.npv, 48, replace=False))
+    cols = np.sort(rng.choice(wl.npt, 1500, replace=False))
+    # add exposures around each sampled pv's conjunction so that in-transit points are covered
+    t0 = wl.pv[pvs, 1]
+    near = np.unique(np.concatenate([np.argsort(np.abs(wl.times - t))[:40] for t in t0[:8]]))
+    cols = np.unique(np.concatenate([cols, near]))
+    import torch
+    got = flux[torch.as_tensor(pvs, device="cuda")][:, torch.as_tensor(cols, device="cuda")] \
+        .cpu().numpy().astype(np.float64)
+    # property that holds at any size: flux <= 1, finite
+    assert bool(torch.isfinite(flux).all()) and float(flux.max()) <= 1.0
+    sub = wl.subset_pv(pvs).subset_times(cols)
+    want, _ = oracle_flux(sub)
+    tol = TOL32 if precision else TOL64
+    assert np.max(np.abs(got - want)) <= tol
+    assert (want < 1).sum() > 50
+    gm.close()
