@@ -30,9 +30,11 @@ __global__ void rr_zgrid_kernel(double zcut, int nzin, int nzlimb, double *ze, d
   auto edge = [&](int i) -> double {
     if (i <= nzin) return (double)i * zcut / (double)nzin;
     if (i >= nz) return 1.0;
-    double mucut = sqrt(1.0 - zcut * zcut);
+    // __dmul_rn / __dadd_rn: no FMA contraction, so that 1 - x^2 near the limb (where it is
+    // ill-conditioned) rounds exactly as the plain formula does
+    double mucut = sqrt(__dadd_rn(1.0, -__dmul_rn(zcut, zcut)));
     double mue = mucut * (1.0 - (double)(i - nzin) / (double)nzlimb);
-    return sqrt(1.0 - mue * mue);
+    return sqrt(__dadd_rn(1.0, -__dmul_rn(mue, mue)));
   };
   double lo = edge(j);
   ze[j] = lo;
@@ -40,7 +42,7 @@ __global__ void rr_zgrid_kernel(double zcut, int nzin, int nzlimb, double *ze, d
     double hi = edge(j + 1);
     double m = 0.5 * (lo + hi);
     zm[j] = m;
-    mu[j] = sqrt(1.0 - m * m);
+    mu[j] = sqrt(__dadd_rn(1.0, -__dmul_rn(m, m)));
     q[j] = RR_PI * (hi * hi - lo * lo);   // annulus area: Istar = sum_j q_j ldp_j (reading R6)
   }
 }
