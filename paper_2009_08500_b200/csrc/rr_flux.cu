@@ -19,13 +19,15 @@
 // the remaining error by ~2.5e-13 (fp64); anything else (large |d|, e near 1 at periastron) goes to a
 // bracketed Halley/bisection loop.  sin d, cos d - 1 on |d| <= 0.8 are Taylor polynomials with their
 // coefficients in constant memory (operands of the FMAs, no register traffic).
+#include <algorithm>
+
 #include "rr_common.cuh"
 
 namespace {
 
 constexpr int FT = 256;   // threads per flux block
 #ifndef RR_FLUX_MIN_BLOCKS
-#define RR_FLUX_MIN_BLOCKS 4
+#define RR_FLUX_MIN_BLOCKS 4    // resident blocks per SM the register budget is set for
 #endif
 
 // Taylor coefficients: sin x = x + x^3 (S0 + S1 x^2 + ...), cos x - 1 = x^2 (C0 + C1 x^2 + ...).
@@ -164,8 +166,7 @@ __device__ __forceinline__ void rr_sincos(double x, double *s, double *c) { sinc
 __device__ __forceinline__ void rr_sincos(float x, float *s, float *c) { sincosf(x, s, c); }
 __device__ __forceinline__ double rr_sinpi(double x) { return sinpi(x); }
 __device__ __forceinline__ float rr_sinpi(float x) { return sinpif(x); }
-__device__ __forceinline__ double rr_atan2(double y, double x) { return atan2(y, x); }
-__device__ __forceinline__ float rr_atan2(float y, float x) { return atan2f(y, x); }
+__device__ __forceinline__ float rr_atan2_pos(float y, float x) { return atan2f(y, x); }
 __device__ __forceinline__ double rr_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(x); }
 
@@ -176,6 +177,37 @@ __device__ __forceinline__ double rr_rcp(double x) {
   return fma(fma(-x, r, 1.0), r, r);
 }
 __device__ __forceinline__ float rr_rcp(float x) { return __frcp_rn(x); }
+
+// atan2(y, x) for y >= 0, (x, y) != (0, 0): the angle in [0, pi].  Octant reduction
+// t = min/max of (|x|, y), then a turn by pi/4 when t > tan(pi/8) so that |t| <= tan(pi/8); one
+// division (hardware seed, Newton step, residual correction: correctly rounded to ~1 ulp);
+// atan t = t + t u Q(u), u = t^2, Q = degree-10 interpolant at the Chebyshev nodes of
+// [0, tan^2(pi/8)] (max error 6e-17 against 60-digit arithmetic, profiles/ note r01b).
+__constant__ double RR_ATAN_D[11] = {
+    -3.33333333333331205e-01, 1.99999999999408928e-01,  -1.42857142792502445e-01,
+    1.11111107449196583e-01,  -9.09089680906402658e-02, 7.69204533090222520e-02,
+    -6.66295181362919070e-02, 5.84687829733087222e-02,  -5.03510245660155203e-02,
+    3.79652574538659332e-02,  -1.78053972054194459e-02};
+__device__ __forceinline__ double rr_atan2_pos(double y, double x) {
+  const double ax = fabs(x);
+  const double mx = fmax(ax, y), mn = fmin(ax, y);
+  const bool red = mn > 0.41421356237309503 * mx;
+  const double num = red ? mn - mx : mn;
+  const double den = red ? mn + mx : mx;
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
+  r = fma(fma(-den, r, 1.0), r, r);
+  double t = num * r;
+  t = fma(fma(-den, t, num), r, t);
+  const double u = t * t;
+  double q = RR_ATAN_D[10];
+#pragma unroll
+  for (int i = 9; i >= 0; --i) q = fma(q, u, RR_ATAN_D[i]);
+  const double base = fma(t * u, q, t) + (red ? 0.78539816339744831 : 0.0);
+  const bool swap = y > ax, neg = x < 0.0;
+  const double off = swap ? 1.5707963267948966 : (neg ? 3.1415926535897932 : 0.0);
+  return fma((swap != neg) ? -1.0 : 1.0, base, off);
+}
 
 // Nearest integer of |x| < 2^51 as a double (two adds, no conversion instruction).
 __device__ __forceinline__ double rr_round(double x) {
@@ -217,7 +249,9 @@ enum {
   K_ZC0, K_ZC1, K_E, K_SE, K_CE, K_A, K_B, K_C, K_KY, K_C2, K_C3, K_C4, K_TOL, K_X1, K_X2, K_Y0,
   K_Y1, K_Y2, K_ACI2,                                             // orbit
   K_K, K_OPK, K_OPK2, K_OMK, K_AFULL, K_K2, K_GSCALE, K_OMK2,     // radius ratio
-  K_COUNT
+  K_COUNT,
+  K_SCALE = K_COUNT,                                              // 1 / (Istar ns)
+  K_TOTAL
 };
 template <typename R> struct Cst {
   const volatile R *p;
@@ -369,8 +403,8 @@ __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restric
     // two sectors minus the kite, kite = 4 x area of the triangle (1, k, z)
     const R kk = k[K_K], opk = k[K_OPK], k2 = k[K_K2];
     R kite = rr_sqrt(fmax((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk), (R)0));
-    R th1 = rr_atan2(kite, fma(z - kk, z + kk, (R)1));
-    R th2 = rr_atan2(kite, fma(z - (R)1, z + (R)1, k2));
+    R th1 = rr_atan2_pos(kite, fma(z - kk, z + kk, (R)1));
+    R th2 = rr_atan2_pos(kite, fma(z - (R)1, z + (R)1, k2));
     ap = th1 + k2 * th2 - (R)0.5 * kite;
     ++ningress;
   }
@@ -390,6 +424,8 @@ struct FluxParams {
   int64_t npt, npv, ntiles;
   int npb, nkpb, nk, ng;
   int shuffle_min_ns;   // light curves with ns >= this use the lanes-over-sub-samples layout
+  unsigned nchunks;     // blocks per parameter vector
+  unsigned chunk_len;   // dispatch tiles per block
 };
 
 template <typename R> __device__ __forceinline__ R rr_nan();
@@ -398,24 +434,26 @@ template <> __device__ __forceinline__ float rr_nan<float>() { return __int_as_f
 
 // Coalesced, 16-byte-vectorised constant fill of out[0..count).
 template <typename R>
-__device__ __forceinline__ void rr_fill(R *out, int count, R val) {
+__device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
   constexpr int VN = 16 / sizeof(R);
   uintptr_t addr = reinterpret_cast<uintptr_t>(out);
-  int head = (int)(((16 - (addr & 15)) & 15) / sizeof(R));
+  int64_t head = (int64_t)(((16 - (addr & 15)) & 15) / sizeof(R));
   if (head > count) head = count;
-  if ((int)threadIdx.x < head) out[threadIdx.x] = val;
-  int nvec = (count - head) / VN;
+  if ((int64_t)threadIdx.x < head) out[threadIdx.x] = val;
+  const int64_t nvec = (count - head) / VN;
   if (sizeof(R) == 8) {
     double2 v = make_double2((double)val, (double)val);
     double2 *o = reinterpret_cast<double2 *>(out + head);
-    for (int i = threadIdx.x; i < nvec; i += FT) o[i] = v;
+#pragma unroll 4
+    for (int64_t i = threadIdx.x; i < nvec; i += FT) o[i] = v;
   } else {
     float4 v = make_float4((float)val, (float)val, (float)val, (float)val);
     float4 *o = reinterpret_cast<float4 *>(out + head);
-    for (int i = threadIdx.x; i < nvec; i += FT) o[i] = v;
+#pragma unroll 4
+    for (int64_t i = threadIdx.x; i < nvec; i += FT) o[i] = v;
   }
-  int done = head + nvec * VN;
-  if ((int)threadIdx.x < count - done) out[done + threadIdx.x] = val;
+  const int64_t done = head + nvec * VN;
+  if ((int64_t)threadIdx.x < count - done) out[done + threadIdx.x] = val;
 }
 
 // Occulted light of the sub-sample at phase w (turns, measured from the window centre).
@@ -501,8 +539,11 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
   }
 }
 
-// One (tile, pv) pair per block iteration.  Block = FT threads.
-// Shared memory: ldw[ng] (k-collapsed table row) | cst[K_COUNT] (per-(tile,pv) constants).
+// One block per (parameter vector, chunk of consecutive dispatch tiles).  Block = FT threads.
+// The pv's constants are staged once per block, the k-collapsed table row once per light curve the
+// chunk meets; tiles outside the transit window are merged into contiguous runs and written as
+// flux = 1 with 16-byte stores, without touching the orbit.
+// Shared memory: ldw[ng] (k-collapsed table row) | cst[K_COUNT] (constants, working precision).
 template <typename R, bool COUNT>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
@@ -510,23 +551,35 @@ rr_flux_kernel(const FluxParams P) {
   R *ldw = reinterpret_cast<R *>(rr_smem);
   R *cst = ldw + ((P.ng + 1) & ~1);
   const Cst<R> k{cst};
-  const int64_t total = P.ntiles * P.npv;
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
-  for (int64_t wi = blockIdx.x; wi < total; wi += gridDim.x) {
-    const int64_t v = wi / P.ntiles;
-    const int64_t tl = wi - v * P.ntiles;
+  const unsigned v = blockIdx.x / P.nchunks;
+  const unsigned chunk = blockIdx.x - v * P.nchunks;
+  const int64_t tl0 = (int64_t)chunk * P.chunk_len;
+  const int64_t tl1 = min(tl0 + (int64_t)P.chunk_len, P.ntiles);
+  const RRPvOrbit &po = P.pvo[v];
+  R *row = reinterpret_cast<R *>(P.flux) + (int64_t)v * P.npt;
+  if (po.status) {                                     // reading R12: NaN row
+    const RRTile a = P.tiles[tl0], b = P.tiles[tl1 - 1];
+    rr_fill<R>(row + a.start, (int64_t)b.start + b.count - a.start, rr_nan<R>());
+    return;
+  }
+  const double t0 = po.t0, inv_p = po.inv_p, u_mid = po.u_mid, hwid = po.hwid;
+  const int circular = po.circular;
+  int desc_lc = -1, staged_lc = -1;                    // light curve of lc / of the staged table
+  RRLc lc;
+  double hw = 0.0;                                     // half an exposure, in turns
+  R scale = (R)0;
+  int64_t f0 = -1, f1 = 0;                             // pending run of exposures with flux 1
+
+  for (int64_t tl = tl0; tl < tl1; ++tl) {
     const RRTile tile = P.tiles[tl];
-    const RRLc lc = P.lcs[tile.lc];
-    const RRPvOrbit &po = P.pvo[v];
-    R *out = reinterpret_cast<R *>(P.flux) + v * P.npt + tile.start;
-    if (po.status) {                                   // reading R12: NaN row
-      rr_fill<R>(out, tile.count, rr_nan<R>());
-      continue;
+    if (tile.lc != desc_lc) {
+      lc = P.lcs[tile.lc];
+      desc_lc = tile.lc;
+      hw = 0.5 * lc.exptime * inv_p;
     }
-    const double t0 = po.t0, inv_p = po.inv_p, u_mid = po.u_mid, hwid = po.hwid;
-    const double hw = 0.5 * lc.exptime * inv_p;        // half an exposure, in turns
     {
       // whole tile outside the transit window (modulo one turn) -> flux 1, no evaluation:
       // phases of the tile, measured from the window centre, lie in [wa, wb]
@@ -534,35 +587,43 @@ rr_flux_kernel(const FluxParams P) {
       const double wb = fma(tile.tmax - t0, inv_p, -u_mid) + hw;
       const double n = ceil(wa - hwid);                // first turn whose window can end after wa
       if (n - hwid > wb) {
-        rr_fill<R>(out, tile.count, (R)1);
+        if (f0 < 0) f0 = tile.start;
+        f1 = (int64_t)tile.start + tile.count;
         if (COUNT) { cfill += (threadIdx.x == 0); cnt[0] += (threadIdx.x == 0) ? (unsigned long long)tile.count * lc.ns : 0; }
         continue;
       }
     }
+    if (f0 >= 0) {
+      rr_fill<R>(row + f0, f1 - f0, (R)1);
+      f0 = -1;
+    }
     if (COUNT) ceval += (threadIdx.x == 0);
-    // stage the k-collapsed table row ldw[ng] and the constants in shared memory
-    const int kb = (P.nkpb == 1) ? 0 : lc.pb;
-    const RRPvBand &pb = P.pvb[v * P.nkpb + kb];
-    {
-      const R *T0 = reinterpret_cast<const R *>(P.T) +
-                    ((v * P.npb + lc.pb) * P.nk + pb.ik) * (int64_t)P.ng;
+    if (tile.lc != staged_lc) {
+      // stage the k-collapsed table row ldw[ng] and the constants in shared memory
+      const int kb = (P.nkpb == 1) ? 0 : lc.pb;
+      const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
+      const int64_t trow = (int64_t)v * P.npb + lc.pb;
+      const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
       const R *T1 = T0 + P.ng;
       const R ak = (R)pb.ak;
       __syncthreads();
       for (int ig = threadIdx.x; ig < P.ng; ig += FT) ldw[ig] = fma(ak, T1[ig] - T0[ig], T0[ig]);
       rr_stage_constants<R>(cst, po, pb);
+      if (threadIdx.x == K_COUNT)
+        cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
       __syncthreads();
+      scale = k[K_SCALE];
+      staged_lc = tile.lc;
     }
-    const int ns = lc.ns;
-    const R scale = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[v * P.npb + lc.pb] * ns));
-    const int shuffle = ns >= P.shuffle_min_ns;
-    if (po.circular)
-      rr_tile<R, COUNT, true>(P.times + tile.start, out, tile.count, ns, shuffle, t0, inv_p, u_mid,
-                              hwid, hw, scale, k, ldw, P.ng, cnt);
+    const int shuffle = lc.ns >= P.shuffle_min_ns;
+    if (circular)
+      rr_tile<R, COUNT, true>(P.times + tile.start, row + tile.start, tile.count, lc.ns, shuffle,
+                              t0, inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
     else
-      rr_tile<R, COUNT, false>(P.times + tile.start, out, tile.count, ns, shuffle, t0, inv_p,
-                               u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+      rr_tile<R, COUNT, false>(P.times + tile.start, row + tile.start, tile.count, lc.ns, shuffle,
+                               t0, inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
   }
+  if (f0 >= 0) rr_fill<R>(row + f0, f1 - f0, (R)1);
   if (COUNT) {
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
@@ -721,10 +782,20 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   if (ctx->reduction == RR_REDUCE_THREAD) P.shuffle_min_ns = 0x7fffffff;
   else if (ctx->reduction == RR_REDUCE_SHUFFLE) P.shuffle_min_ns = 2;
   else P.shuffle_min_ns = (npv * ctx->npt < 2 * resident) ? 4 : 0x7fffffff;
-  const int64_t total = ctx->ntiles * npv;
-  if (total <= 0) return RR_OK;
-  const unsigned grid = rr_grid_for(total);
-  const size_t smem = (size_t)(((c.ng + 1) & ~1) + K_COUNT) * (c.precision == RR_FP32 ? 4 : 8);
+  if (ctx->ntiles <= 0 || npv <= 0) return RR_OK;
+  // Blocks: one per (pv, chunk of consecutive tiles).  One chunk per pv when the population alone
+  // gives every SM several waves of blocks (table row and constants staged once per pv);
+  // otherwise the tile axis is cut so that about 8 waves of blocks exist.
+  const int64_t want = (int64_t)ctx->sm_count * RR_FLUX_MIN_BLOCKS * 8;
+  int64_t nchunks = (want + npv - 1) / npv;
+  nchunks = std::max<int64_t>(1, std::min<int64_t>(nchunks, ctx->ntiles));
+  const int64_t chunk_len = (ctx->ntiles + nchunks - 1) / nchunks;
+  nchunks = (ctx->ntiles + chunk_len - 1) / chunk_len;
+  if (npv * nchunks > 0x7fffffffLL) return RR_ESIZE;
+  P.nchunks = (unsigned)nchunks;
+  P.chunk_len = (unsigned)chunk_len;
+  const unsigned grid = (unsigned)(npv * nchunks);
+  const size_t smem = (size_t)(((c.ng + 1) & ~1) + K_TOTAL) * (c.precision == RR_FP32 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
     if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);
