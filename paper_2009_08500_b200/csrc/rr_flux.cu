@@ -167,7 +167,21 @@ __device__ __forceinline__ void rr_sincos(float x, float *s, float *c) { sincosf
 __device__ __forceinline__ double rr_sinpi(double x) { return sinpi(x); }
 __device__ __forceinline__ float rr_sinpi(float x) { return sinpif(x); }
 __device__ __forceinline__ float rr_atan2_pos(float y, float x) { return atan2f(y, x); }
-__device__ __forceinline__ double rr_sqrt(double x) { return sqrt(x); }
+// sqrt(x) for x >= 0 (0 and normal numbers): hardware reciprocal-square-root seed (~2^-20), two
+// Goldschmidt steps (g -> sqrt x, h -> 1/(2 sqrt x)) and a final residual correction; <= 1 ulp.
+__device__ __forceinline__ double rr_sqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double r = fma(-h, g, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-h, g, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  g = fma(fma(-g, g, x), h, g);
+  return x > 0.0 ? g : 0.0;
+}
 __device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(x); }
 
 // 1/x to ~1e-12 (fp64: hardware seed + one Newton step) / ~1e-7 (fp32).  x normal, non-zero.
@@ -246,16 +260,37 @@ __device__ __forceinline__ void rr_sincosm1_small(float x, float &s, float &cm1)
 // issue slots the half-rate FP64 pipe leaves free, and keeping ~25 of them out of registers is what
 // lets 4 blocks of 256 threads share an SM.
 enum {
-  K_ZC0, K_ZC1, K_E, K_SE, K_CE, K_A, K_B, K_C, K_KY, K_C2, K_C3, K_C4, K_TOL, K_X1, K_X2, K_Y0,
-  K_Y1, K_Y2, K_ACI2,                                             // orbit
-  K_K, K_OPK, K_OPK2, K_OMK, K_AFULL, K_K2, K_GSCALE, K_OMK2,     // radius ratio
+  K_ZC0, K_ZC1,           // circular (pair)
+  K_C4, K_C3,             // starter (pair)
+  K_C2, K_KY,             // (pair)
+  K_B, K_C,               // (pair)
+  K_A, K_TOL,             // (pair)
+  K_X1, K_X2,             // (pair)
+  K_Y1, K_Y2,             // (pair)
+  K_Y0, K_ACI2,           // (pair)
+  K_E, K_SE, K_CE,        // robust solver path
+  K_OPK2,                 // radius ratio
+  K_OMK2, K_AFULL,        // (pair)
+  K_GSCALE, K_K,          // (pair)
+  K_OPK, K_K2,            // (pair)
+  K_OMK,
   K_COUNT,
-  K_SCALE = K_COUNT,                                              // 1 / (Istar ns)
+  K_SCALE = K_COUNT,      // 1 / (Istar ns)
   K_TOTAL
 };
+static_assert(K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
 template <typename R> struct Cst {
   const volatile R *p;
   __device__ __forceinline__ R operator[](int i) const { return p[i]; }
+  // two neighbouring constants (i even) with one 16-/8-byte shared load
+  __device__ __forceinline__ void pair(int i, double &a, double &b) const {
+    unsigned addr = (unsigned)__cvta_generic_to_shared(const_cast<const R *>(p) + i);
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr));
+  }
+  __device__ __forceinline__ void pair(int i, float &a, float &b) const {
+    unsigned addr = (unsigned)__cvta_generic_to_shared(const_cast<const R *>(p) + i);
+    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a), "=f"(b) : "r"(addr));
+  }
 };
 
 template <typename R>
@@ -334,39 +369,54 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
       s = rr_sinpi((R)(2.0 * ur));
     }
     front = fabs(ur) < 0.25;
-    return fma(s * s, k[K_ZC1], k[K_ZC0]);
+    R zc0, zc1;
+    k.pair(K_ZC0, zc0, zc1);
+    return fma(s * s, zc1, zc0);
   }
   const R dM = (R)(RR_TWOPI * ur);
   R s2, cm2;
   bool done = false;
   {
-    const R y = (R)ur * k[K_KY];                       // dM / A
-    const R d = y * fma(y, fma(y, fma(y, k[K_C4], k[K_C3]), k[K_C2]), (R)1);
-    if (fabs(d) <= (R)RR_TRIG_SMALL) {
+    R c4, c3, c2, ky, B, C, A, tol;
+    k.pair(K_C4, c4, c3);
+    k.pair(K_C2, c2, ky);
+    const R y = (R)ur * ky;                            // dM / A
+    R d = y * fma(y, fma(y, fma(y, c4, c3), c2), (R)1);
+    k.pair(K_B, B, C);
+    k.pair(K_A, A, tol);
+    // Halley steps from the series starter while d stays in the polynomial range; the first one
+    // is accepted for ~94 % of config 4's eccentric sub-samples
+#pragma unroll 1
+    for (int it = 0; it < 3 && fabs(d) <= (R)RR_TRIG_SMALL; ++it) {
       R s, cm1;
       rr_sincosm1_small(d, s, cm1);
-      const R B = k[K_B], C = k[K_C];
       const R t = fma(B, cm1, C * s);              // e [sin E - sin E_tr]
       const R g = (d - dM) - t;
-      const R gp = k[K_A] - fma(C, cm1, -B * s);   // 1 - e cos E
+      const R gp = A - fma(C, cm1, -B * s);        // 1 - e cos E
       const R gpp = B + t;                         // e sin E
       const R dd = (R)-2 * g * gp * rr_rcp(fma((R)2 * gp, gp, -g * gpp));   // Halley
-      if (fabs(dd) <= k[K_TOL]) {
+      iters += 1;
+      if (fabs(dd) <= tol) {
         // (sin, cos - 1) of d + dd, third order in dd
         const R c = (R)1 + cm1;
         const R h2 = (R)0.5 * dd * dd, h3 = h2 * dd * (R)(1.0 / 3.0);
         s2 = fma(c, dd, s) - fma(s, h2, c * h3);
         cm2 = fma(-s, dd, cm1) - fma(c, h2, -s * h3);
         done = true;
-        iters += 1;
+        break;
       }
+      d += dd;
     }
   }
   if (!done) rr_kepler_robust<R>(k[K_E], k[K_SE], k[K_CE], dM, &s2, &cm2, &iters);
-  const R xs = fma(k[K_X1], cm2, k[K_X2] * s2);
-  const R ys = k[K_Y0] + fma(k[K_Y1], cm2, k[K_Y2] * s2);
+  R X1, X2, Y1, Y2, Y0, aci2;
+  k.pair(K_X1, X1, X2);
+  k.pair(K_Y1, Y1, Y2);
+  k.pair(K_Y0, Y0, aci2);
+  const R xs = fma(X1, cm2, X2 * s2);
+  const R ys = Y0 + fma(Y1, cm2, Y2 * s2);
   front = ys > (R)0;
-  return fma(xs, xs, k[K_ACI2] * (ys * ys));
+  return fma(xs, xs, aci2 * (ys * ys));
 }
 
 // ---- kernel 3 core: occulted light ip * ap of one sub-sample with z < 1+k ------
@@ -392,16 +442,21 @@ __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restric
   R z = rr_sqrt(z2);
   int ig;
   R ag;
-  rr_cell(z * k[K_GSCALE], ng, ig, ag);
+  R gscale, kk;
+  k.pair(K_GSCALE, gscale, kk);
+  rr_cell(z * gscale, ng, ig, ag);
   R l0 = ldw[ig], l1 = ldw[ig + 1];
   R ip = fma(ag, l1 - l0, l0);              // mean occulted brightness
   R ap;
-  if (z2 <= k[K_OMK2]) {
-    ap = k[K_AFULL];                        // planet (or star) fully inside the other disc
+  R omk2, afull;
+  k.pair(K_OMK2, omk2, afull);
+  if (z2 <= omk2) {
+    ap = afull;                             // planet (or star) fully inside the other disc
   } else {
     // lens of the unit disc and the disc of radius k at distance z (reading R9, atan2 form):
     // two sectors minus the kite, kite = 4 x area of the triangle (1, k, z)
-    const R kk = k[K_K], opk = k[K_OPK], k2 = k[K_K2];
+    R opk, k2;
+    k.pair(K_OPK, opk, k2);
     R kite = rr_sqrt(fmax((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk), (R)0));
     R th1 = rr_atan2_pos(kite, fma(z - kk, z + kk, (R)1));
     R th2 = rr_atan2_pos(kite, fma(z - (R)1, z + (R)1, k2));
@@ -644,7 +699,7 @@ __global__ void __launch_bounds__(FT)
 rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ tiles,
                 const RRLc *__restrict__ lcs, const RRPvOrbit *__restrict__ pvo, int64_t ntiles,
                 int64_t npv, int64_t nsub, double *__restrict__ zout) {
-  __shared__ R cst[K_COUNT];
+  __shared__ __align__(16) R cst[K_TOTAL];
   const Cst<R> k{cst};
   const int64_t total = ntiles * npv;
   for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
