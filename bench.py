@@ -35,12 +35,14 @@ METRIC = "transit-model evaluations/sec (pv x time x supersample)"
 UNIT = "evaluations/s"
 # B200 FP64 FMA pipe = 64 lanes/clk/SM (37.2 TFLOP/s nominal at 148 SMs, 1965 MHz)
 FP64_LANES_PER_SM, FP32_LANES_PER_SM, SM_COUNT = 64, 128, 148
-# algorithmic FMA-pipe instructions per unit of each class of the flux kernel
+# algorithmic FMA-pipe instructions (DFMA/DMUL/DADD; fp32 mode: FFMA-class, with the
+# fp64 phase instructions counted twice) per unit of each class of the flux kernel.  Sub-samples in
+# merged out-of-window fill runs cost no arithmetic.
 ALG_OPS = {
-    "fp64": dict(skipped=5, circular=34, eccentric_fixed=46, solver_iter=62, occulting=30,
-                 ingress=150),
-    "fp32": dict(skipped=5, circular=24, eccentric_fixed=40, solver_iter=40, occulting=16,
-                 ingress=60),
+    "fp64": dict(skipped=2, circular=17, eccentric_fixed=32, solver_iter=33, occulting=18,
+                 ingress=68),
+    "fp32": dict(skipped=4, circular=20, eccentric_fixed=38, solver_iter=26, occulting=11,
+                 ingress=61),
 }
 
 

@@ -172,10 +172,12 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
 
 /* ---- measurement aids (bench.py) ---------------------------------------------------------------
  * Counters of the last rr_evaluate on this ctx, filled by the flux kernel when enabled with
- * rr_enable_counters(ctx, 1) (adds atomics; keep off when timing): h_counts[0] sub-samples skipped
- * as out of the transit window, [1] evaluated circular, [2] evaluated eccentric, [3] of those with
- * z < 1+k in front of the star, [4] of those in ingress/egress (lens area), [5] Newton iterations,
- * [6] (tile, pv) pairs filled without evaluation, [7] (tile, pv) pairs evaluated.  Synchronous. */
+ * rr_enable_counters(ctx, 1) (adds atomics; keep off when timing): h_counts[0] sub-samples of
+ * evaluated tiles skipped as out of the transit window (sub-samples of tiles filled whole are not
+ * counted: total - [0] - [1] - [2]), [1] evaluated circular, [2] evaluated eccentric, [3] of those
+ * with z < 1+k in front of the star, [4] of those in ingress/egress (lens area), [5] sincos
+ * evaluations of the Kepler solver, [6] tiles (per pv) filled without evaluation, [7] tiles (per
+ * pv) evaluated.  Synchronous. */
 int rr_enable_counters(rr_ctx *ctx, int32_t on);
 int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts /*[8]*/);
 /* Number of kernel launches the library has made on this ctx since creation.                     */

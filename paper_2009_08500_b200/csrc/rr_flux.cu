@@ -644,7 +644,7 @@ rr_flux_kernel(const FluxParams P) {
       if (n - hwid > wb) {
         if (f0 < 0) f0 = tile.start;
         f1 = (int64_t)tile.start + tile.count;
-        if (COUNT) { cfill += (threadIdx.x == 0); cnt[0] += (threadIdx.x == 0) ? (unsigned long long)tile.count * lc.ns : 0; }
+        if (COUNT) cfill += (threadIdx.x == 0);
         continue;
       }
     }
