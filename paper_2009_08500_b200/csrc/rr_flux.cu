@@ -204,7 +204,8 @@ __constant__ double RR_ATAN_D[11] = {
     3.79652574538659332e-02,  -1.78053972054194459e-02};
 __device__ __forceinline__ double rr_atan2_pos(double y, double x) {
   const double ax = fabs(x);
-  const double mx = fmax(ax, y), mn = fmin(ax, y);
+  const bool swap = y > ax;
+  const double mx = swap ? y : ax, mn = swap ? ax : y;
   const bool red = mn > 0.41421356237309503 * mx;
   const double num = red ? mn - mx : mn;
   const double den = red ? mn + mx : mx;
@@ -218,7 +219,7 @@ __device__ __forceinline__ double rr_atan2_pos(double y, double x) {
 #pragma unroll
   for (int i = 9; i >= 0; --i) q = fma(q, u, RR_ATAN_D[i]);
   const double base = fma(t * u, q, t) + (red ? 0.78539816339744831 : 0.0);
-  const bool swap = y > ax, neg = x < 0.0;
+  const bool neg = x < 0.0;
   const double off = swap ? 1.5707963267948966 : (neg ? 3.1415926535897932 : 0.0);
   return fma((swap != neg) ? -1.0 : 1.0, base, off);
 }
@@ -276,7 +277,8 @@ enum {
   K_OMK,
   K_COUNT,
   K_SCALE = K_COUNT,      // 1 / (Istar ns)
-  K_TOTAL
+  K_TOTAL,
+  K_SMEM = (K_TOTAL + 3) & ~3   // 16-byte multiple in both precisions
 };
 static_assert(K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
 template <typename R> struct Cst {
@@ -598,14 +600,15 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
 // The pv's constants are staged once per block, the k-collapsed table row once per light curve the
 // chunk meets; tiles outside the transit window are merged into contiguous runs and written as
 // flux = 1 with 16-byte stores, without touching the orbit.
-// Shared memory: ldw[ng] (k-collapsed table row) | cst[K_COUNT] (constants, working precision).
+// Shared memory: cst[K_SMEM] (constants, working precision) | ldw[ng] (k-collapsed table row).
 template <typename R, bool COUNT>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
   extern __shared__ __align__(16) unsigned char rr_smem[];
-  R *ldw = reinterpret_cast<R *>(rr_smem);
-  R *cst = ldw + ((P.ng + 1) & ~1);
+  R *cst = reinterpret_cast<R *>(rr_smem);             // fixed offsets: immediates in the loads
+  R *ldw = cst + K_SMEM;
   const Cst<R> k{cst};
+  __shared__ unsigned tflags[FT / 32];
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
@@ -628,55 +631,77 @@ rr_flux_kernel(const FluxParams P) {
   R scale = (R)0;
   int64_t f0 = -1, f1 = 0;                             // pending run of exposures with flux 1
 
-  for (int64_t tl = tl0; tl < tl1; ++tl) {
-    const RRTile tile = P.tiles[tl];
-    if (tile.lc != desc_lc) {
-      lc = P.lcs[tile.lc];
-      desc_lc = tile.lc;
-      hw = 0.5 * lc.exptime * inv_p;
+  for (int64_t base = tl0; base < tl1; base += FT) {
+    const int ngrp = (int)min((int64_t)FT, tl1 - base);
+    // Each thread tests ONE tile of the group against the transit window (modulo one turn): the
+    // phases of the tile, measured from the window centre, lie in [wa, wb]; n = first turn whose
+    // window can end after wa.  Out-of-window tiles get flux 1 without evaluation.
+    bool in = false;
+    if ((int)threadIdx.x < ngrp) {
+      const RRTile *tp = P.tiles + base + threadIdx.x;
+      const double hwt = 0.5 * P.lcs[tp->lc].exptime * inv_p;
+      const double wa = fma(tp->tmin - t0, inv_p, -u_mid) - hwt;
+      const double wb = fma(tp->tmax - t0, inv_p, -u_mid) + hwt;
+      in = !(ceil(wa - hwid) - hwid > wb);
     }
-    {
-      // whole tile outside the transit window (modulo one turn) -> flux 1, no evaluation:
-      // phases of the tile, measured from the window centre, lie in [wa, wb]
-      const double wa = fma(tile.tmin - t0, inv_p, -u_mid) - hw;
-      const double wb = fma(tile.tmax - t0, inv_p, -u_mid) + hw;
-      const double n = ceil(wa - hwid);                // first turn whose window can end after wa
-      if (n - hwid > wb) {
-        if (f0 < 0) f0 = tile.start;
-        f1 = (int64_t)tile.start + tile.count;
-        if (COUNT) cfill += (threadIdx.x == 0);
-        continue;
+    const unsigned mask = __ballot_sync(0xffffffffu, in);
+    __syncthreads();                                   // the previous group's flags are consumed
+    if ((threadIdx.x & 31) == 0) tflags[threadIdx.x >> 5] = mask;
+    __syncthreads();
+    const int nwords = (ngrp + 31) >> 5;
+    int pos = 0;
+    while (pos < ngrp) {
+      int q = ngrp;                                    // next in-window tile at or after pos
+      for (int w = pos >> 5; w < nwords; ++w) {
+        unsigned bits = tflags[w];
+        if (w == (pos >> 5)) bits &= 0xffffffffu << (pos & 31);
+        if (bits) { q = (w << 5) + __ffs(bits) - 1; break; }
       }
+      if (q > pos) {                                   // tiles pos .. q-1: extend the pending run
+        const RRTile *ta = P.tiles + base + pos, *tb = P.tiles + base + q - 1;
+        if (f0 < 0) f0 = ta->start;
+        f1 = (int64_t)tb->start + tb->count;
+        if (COUNT) cfill += (threadIdx.x == 0) ? (unsigned long long)(q - pos) : 0ull;
+      }
+      if (q >= ngrp) break;
+      pos = q + 1;
+      if (f0 >= 0) {
+        rr_fill<R>(row + f0, f1 - f0, (R)1);
+        f0 = -1;
+      }
+      const RRTile *tp = P.tiles + base + q;
+      const int tstart = tp->start, tcount = tp->count, tlc = tp->lc;
+      if (tlc != desc_lc) {
+        lc = P.lcs[tlc];
+        desc_lc = tlc;
+        hw = 0.5 * lc.exptime * inv_p;
+      }
+      if (COUNT) ceval += (threadIdx.x == 0);
+      if (tlc != staged_lc) {
+        // stage the k-collapsed table row ldw[ng] and the constants in shared memory
+        const int kb = (P.nkpb == 1) ? 0 : lc.pb;
+        const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
+        const int64_t trow = (int64_t)v * P.npb + lc.pb;
+        const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
+        const R *T1 = T0 + P.ng;
+        const R ak = (R)pb.ak;
+        __syncthreads();
+        for (int ig = threadIdx.x; ig < P.ng; ig += FT) ldw[ig] = fma(ak, T1[ig] - T0[ig], T0[ig]);
+        rr_stage_constants<R>(cst, po, pb);
+        if (threadIdx.x == K_COUNT)
+          cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
+        __syncthreads();
+        scale = k[K_SCALE];
+        staged_lc = tlc;
+      }
+      const int shuffle = lc.ns >= P.shuffle_min_ns;
+      if (circular)
+        rr_tile<R, COUNT, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0, inv_p,
+                                u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+      else
+        rr_tile<R, COUNT, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0, inv_p,
+                                 u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
     }
-    if (f0 >= 0) {
-      rr_fill<R>(row + f0, f1 - f0, (R)1);
-      f0 = -1;
-    }
-    if (COUNT) ceval += (threadIdx.x == 0);
-    if (tile.lc != staged_lc) {
-      // stage the k-collapsed table row ldw[ng] and the constants in shared memory
-      const int kb = (P.nkpb == 1) ? 0 : lc.pb;
-      const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
-      const int64_t trow = (int64_t)v * P.npb + lc.pb;
-      const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
-      const R *T1 = T0 + P.ng;
-      const R ak = (R)pb.ak;
-      __syncthreads();
-      for (int ig = threadIdx.x; ig < P.ng; ig += FT) ldw[ig] = fma(ak, T1[ig] - T0[ig], T0[ig]);
-      rr_stage_constants<R>(cst, po, pb);
-      if (threadIdx.x == K_COUNT)
-        cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
-      __syncthreads();
-      scale = k[K_SCALE];
-      staged_lc = tile.lc;
-    }
-    const int shuffle = lc.ns >= P.shuffle_min_ns;
-    if (circular)
-      rr_tile<R, COUNT, true>(P.times + tile.start, row + tile.start, tile.count, lc.ns, shuffle,
-                              t0, inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
-    else
-      rr_tile<R, COUNT, false>(P.times + tile.start, row + tile.start, tile.count, lc.ns, shuffle,
-                               t0, inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
   }
   if (f0 >= 0) rr_fill<R>(row + f0, f1 - f0, (R)1);
   if (COUNT) {
@@ -850,7 +875,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(((c.ng + 1) & ~1) + K_TOTAL) * (c.precision == RR_FP32 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + c.ng) * (c.precision == RR_FP32 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
     if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);
