@@ -167,9 +167,11 @@ __device__ __forceinline__ void rr_sincos(float x, float *s, float *c) { sincosf
 __device__ __forceinline__ double rr_sinpi(double x) { return sinpi(x); }
 __device__ __forceinline__ float rr_sinpi(float x) { return sinpif(x); }
 __device__ __forceinline__ float rr_atan2_pos(float y, float x) { return atan2f(y, x); }
-// sqrt(x) for x >= 0 (0 and normal numbers): hardware reciprocal-square-root seed (~2^-20), two
-// Goldschmidt steps (g -> sqrt x, h -> 1/(2 sqrt x)) and a final residual correction; <= 1 ulp.
-__device__ __forceinline__ double rr_sqrt(double x) {
+// sqrt(x): hardware reciprocal-square-root seed (~2^-20), two Goldschmidt steps (g -> sqrt x,
+// h -> 1/(2 sqrt x)) and a final residual correction; <= 1 ulp.  rr_sqrt: any x, 0 for x <= 0
+// (a product of rounded factors that should be >= 0); rr_sqrt_pos: x >= 0, adds 1e-300 so that the
+// seed of x = 0 is finite (no effect on any other x).
+__device__ __forceinline__ double rr_sqrt_core(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double g = x * y, h = 0.5 * y;
@@ -179,11 +181,15 @@ __device__ __forceinline__ double rr_sqrt(double x) {
   r = fma(-h, g, 0.5);
   g = fma(g, r, g);
   h = fma(h, r, h);
-  g = fma(fma(-g, g, x), h, g);
+  return fma(fma(-g, g, x), h, g);
+}
+__device__ __forceinline__ double rr_sqrt(double x) {
+  const double g = rr_sqrt_core(x);
   return x > 0.0 ? g : 0.0;
 }
-__device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(x); }
-
+__device__ __forceinline__ double rr_sqrt_pos(double x) { return rr_sqrt_core(x + 1e-300); }
+__device__ __forceinline__ float rr_sqrt_pos(float x) { return sqrtf(x); }
+__device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(fmaxf(x, 0.0f)); }
 // 1/x to ~1e-12 (fp64: hardware seed + one Newton step) / ~1e-7 (fp32).  x normal, non-zero.
 __device__ __forceinline__ double rr_rcp(double x) {
   double r;
@@ -215,9 +221,16 @@ __device__ __forceinline__ double rr_atan2_pos(double y, double x) {
   double t = num * r;
   t = fma(fma(-den, t, num), r, t);
   const double u = t * t;
-  double q = RR_ATAN_D[10];
+  // Q(u) = Qe(u^2) + u Qo(u^2): two half-length Horner chains in flight
+  const double u2 = u * u;
+  double qe = RR_ATAN_D[10], qo = RR_ATAN_D[9];
 #pragma unroll
-  for (int i = 9; i >= 0; --i) q = fma(q, u, RR_ATAN_D[i]);
+  for (int i = 8; i >= 2; i -= 2) {
+    qe = fma(qe, u2, RR_ATAN_D[i]);
+    qo = fma(qo, u2, RR_ATAN_D[i - 1]);
+  }
+  qe = fma(qe, u2, RR_ATAN_D[0]);
+  const double q = fma(qo, u, qe);
   const double base = fma(t * u, q, t) + (red ? 0.78539816339744831 : 0.0);
   const bool neg = x < 0.0;
   const double off = swap ? 1.5707963267948966 : (neg ? 3.1415926535897932 : 0.0);
@@ -422,31 +435,31 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
 }
 
 // ---- kernel 3 core: occulted light ip * ap of one sub-sample with z < 1+k ------
-// Table cell of y = g/dg >= 0: lower node ig (clamped to ng-2, reading R10) and weight ag = y - ig.
+// Table cell of y = g/dg in [0, ng-1]: lower node ig and weight ag = y - ig.  The staged row carries
+// one extra node ldw[ng] = ldw[ng-1], so that y = ng-1 (z = 1+k to rounding) needs no clamp: it
+// lands in cell ng-1 with ag = 0 (reading R10: the same value as cell ng-2 with ag = 1).
 // fp64: floor by adding 2^52+2^51 to y - 1/2 (the integer lands in the low word); a tie or a
 // rounding across a node picks the neighbouring cell with ag = 1 or 0, the same interpolant.
-__device__ __forceinline__ void rr_cell(double y, int ng, int &ig, double &ag) {
+__device__ __forceinline__ void rr_cell(double y, int &ig, double &ag) {
   const double M = 6755399441055744.0;
   const double t = __dadd_rn(y - 0.5, M);
-  const int raw = __double2loint(t);
-  ig = min(max(raw, 0), ng - 2);
+  ig = __double2loint(t);
   ag = y - __dadd_rn(t, -M);
-  if (raw != ig) ag = y - (double)ig;
 }
-__device__ __forceinline__ void rr_cell(float y, int ng, int &ig, float &ag) {
-  ig = min((int)y, ng - 2);
+__device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
+  ig = (int)y;
   ag = y - (float)ig;
 }
 
 template <typename R>
 __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restrict__ ldw, int ng,
                                         int &ningress) {
-  R z = rr_sqrt(z2);
+  R z = rr_sqrt_pos(z2);
   int ig;
   R ag;
   R gscale, kk;
   k.pair(K_GSCALE, gscale, kk);
-  rr_cell(z * gscale, ng, ig, ag);
+  rr_cell(z * gscale, ig, ag);
   R l0 = ldw[ig], l1 = ldw[ig + 1];
   R ip = fma(ag, l1 - l0, l0);              // mean occulted brightness
   R ap;
@@ -459,7 +472,7 @@ __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restric
     // two sectors minus the kite, kite = 4 x area of the triangle (1, k, z)
     R opk, k2;
     k.pair(K_OPK, opk, k2);
-    R kite = rr_sqrt(fmax((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk), (R)0));
+    R kite = rr_sqrt((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk));
     R th1 = rr_atan2_pos(kite, fma(z - kk, z + kk, (R)1));
     R th2 = rr_atan2_pos(kite, fma(z - (R)1, z + (R)1, k2));
     ap = th1 + k2 * th2 - (R)0.5 * kite;
@@ -548,8 +561,11 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
   const double hskip = hwid + hw;
   if (!shuffle) {
     // ---- one thread per exposure, in-thread loop over its sub-samples ----
+    double tnext = ((int)threadIdx.x < count) ? times[threadIdx.x] : 0.0;
     for (int i = threadIdx.x; i < count; i += FT) {
-      const double wc = fma(times[i] - t0, inv_p, -u_mid);
+      const double tcur = tnext;
+      if (i + FT < count) tnext = times[i + FT];     // in flight while this exposure is evaluated
+      const double wc = fma(tcur - t0, inv_p, -u_mid);
       const double wr = wc - rr_round(wc);           // exposure centre from the window centre
       R f;
       if (fabs(wr) > hskip) {
@@ -559,10 +575,9 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
         f = rr_nan<R>();
       } else {
         R acc = (R)0;
-        const double w0 = wr + off0;
-        double sd = 0.0;
-        for (int s = 0; s < ns; ++s, sd += 1.0)
-          acc += rr_subsample<R, COUNT, CIRC>(fma(du, sd, w0), u_mid, hwid, k, ldw, ng, cnt);
+        double w = wr + off0;
+        for (int s = 0; s < ns; ++s, w += du)
+          acc += rr_subsample<R, COUNT, CIRC>(w, u_mid, hwid, k, ldw, ng, cnt);
         f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
       out[i] = f;
@@ -600,7 +615,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
 // The pv's constants are staged once per block, the k-collapsed table row once per light curve the
 // chunk meets; tiles outside the transit window are merged into contiguous runs and written as
 // flux = 1 with 16-byte stores, without touching the orbit.
-// Shared memory: cst[K_SMEM] (constants, working precision) | ldw[ng] (k-collapsed table row).
+// Shared memory: cst[K_SMEM] (constants, working precision) | ldw[ng+1] (k-collapsed table row).
 template <typename R, bool COUNT>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
@@ -686,7 +701,10 @@ rr_flux_kernel(const FluxParams P) {
         const R *T1 = T0 + P.ng;
         const R ak = (R)pb.ak;
         __syncthreads();
-        for (int ig = threadIdx.x; ig < P.ng; ig += FT) ldw[ig] = fma(ak, T1[ig] - T0[ig], T0[ig]);
+        for (int ig = threadIdx.x; ig <= P.ng; ig += FT) {
+          const int jg = min(ig, P.ng - 1);          // ldw[ng] = ldw[ng-1]: see rr_cell
+          ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
+        }
         rr_stage_constants<R>(cst, po, pb);
         if (threadIdx.x == K_COUNT)
           cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
@@ -875,7 +893,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + c.ng) * (c.precision == RR_FP32 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + c.ng + 1) * (c.precision == RR_FP32 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
     if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);
