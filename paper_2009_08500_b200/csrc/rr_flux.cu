@@ -29,18 +29,20 @@ constexpr int FT = 256;   // threads per flux block
 #ifndef RR_FLUX_MIN_BLOCKS
 #define RR_FLUX_MIN_BLOCKS 4    // resident blocks per SM the register budget is set for
 #endif
+#ifndef RR_FLUX_WAVES
+#define RR_FLUX_WAVES 32        // waves of blocks wanted before the tile axis is left uncut
+#endif
 
 // Taylor coefficients: sin x = x + x^3 (S0 + S1 x^2 + ...), cos x - 1 = x^2 (C0 + C1 x^2 + ...).
-// Truncation on |x| <= 0.8: fp64 0.8^17/17! = 6e-17, 0.8^18/18! = 3e-18; fp32 0.8^11/11! = 2e-9.
-__constant__ double RR_SIN_D[7] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0,
-                                   -1.0 / 39916800.0, 1.0 / 6227020800.0, -1.0 / 1307674368000.0};
-__constant__ double RR_COS_D[8] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0,
-                                   -1.0 / 3628800.0, 1.0 / 479001600.0, -1.0 / 87178291200.0,
-                                   1.0 / 20922789888000.0};
-__constant__ float RR_SIN_F[4] = {-1.0f / 6.0f, 1.0f / 120.0f, -1.0f / 5040.0f, 1.0f / 362880.0f};
-__constant__ float RR_COS_F[5] = {-1.0f / 2.0f, 1.0f / 24.0f, -1.0f / 720.0f, 1.0f / 40320.0f,
-                                  -1.0f / 3628800.0f};
-constexpr double RR_TRIG_SMALL = 0.8;
+// Truncation on |x| <= 0.5: fp64 sin 0.5^14/15! = 5e-17 relative, cos-1 2 0.5^14/16! = 6e-18;
+// fp32 0.5^8/9! = 1e-8.
+__constant__ double RR_SIN_D[6] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0,
+                                   -1.0 / 39916800.0, 1.0 / 6227020800.0};
+__constant__ double RR_COS_D[7] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0,
+                                   -1.0 / 3628800.0, 1.0 / 479001600.0, -1.0 / 87178291200.0};
+__constant__ float RR_SIN_F[3] = {-1.0f / 6.0f, 1.0f / 120.0f, -1.0f / 5040.0f};
+__constant__ float RR_COS_F[4] = {-1.0f / 2.0f, 1.0f / 24.0f, -1.0f / 720.0f, 1.0f / 40320.0f};
+constexpr double RR_TRIG_SMALL = 0.5;
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
 __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, int nkpb, int nk,
@@ -117,9 +119,10 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     po.c3 = 0.5 * b * b - c / 6.0;
     po.c4 = -0.625 * b * b * b + (5.0 / 12.0) * b * c + b / 24.0;
   }
-  // Halley's error after a step of size s is ~K s^3, K <= (e/(1-e))^2/4 + e/(6(1-e)): with
-  // s <= 1e-4 (1-e) that is below 2.5e-13 (fp64); fp32 works to 1e-3 (1-e) -> 2.5e-10.
-  po.tol = (fp32 ? 1e-3 : 1e-4) * (1.0 - e);
+  // Halley's error after a step of size s is ~K s^3, K <= (e/(1-e))^2/4 + e/(6(1-e)), and the
+  // accepted step is applied to (sin, cos - 1) to second order (error s^3/6): with
+  // s <= 2e-5 (1-e) both are below 2e-15 (fp64); fp32 works to 1e-3 (1-e) -> 4e-10.
+  po.tol = (fp32 ? 1e-3 : 2e-5) * (1.0 - e);
   // sky position from (cm, s) = (cos d - 1, sin d):  sin E - sin E_tr = sE cm + cE s,
   // cos E - cos E_tr = cE cm - sE s;  x/a = cw dC - beta sw dS,  y/a = rho_tr + beta cw dS + sw dC
   const double bsw = beta * sw, bcw = beta * cw;
@@ -246,10 +249,10 @@ __device__ __forceinline__ double rr_round(double x) {
 // sin x and cos x - 1 on |x| <= RR_TRIG_SMALL.
 __device__ __forceinline__ void rr_sincosm1_small(double x, double &s, double &cm1) {
   const double x2 = x * x;
-  double ps = RR_SIN_D[6], pc = RR_COS_D[7];
-  pc = fma(pc, x2, RR_COS_D[6]);
+  double ps = RR_SIN_D[5], pc = RR_COS_D[6];
+  pc = fma(pc, x2, RR_COS_D[5]);
 #pragma unroll
-  for (int i = 5; i >= 0; --i) {
+  for (int i = 4; i >= 0; --i) {
     ps = fma(ps, x2, RR_SIN_D[i]);
     pc = fma(pc, x2, RR_COS_D[i]);
   }
@@ -258,10 +261,10 @@ __device__ __forceinline__ void rr_sincosm1_small(double x, double &s, double &c
 }
 __device__ __forceinline__ void rr_sincosm1_small(float x, float &s, float &cm1) {
   const float x2 = x * x;
-  float ps = RR_SIN_F[3], pc = RR_COS_F[4];
-  pc = fmaf(pc, x2, RR_COS_F[3]);
+  float ps = RR_SIN_F[2], pc = RR_COS_F[3];
+  pc = fmaf(pc, x2, RR_COS_F[2]);
 #pragma unroll
-  for (int i = 2; i >= 0; --i) {
+  for (int i = 1; i >= 0; --i) {
     ps = fmaf(ps, x2, RR_SIN_F[i]);
     pc = fmaf(pc, x2, RR_COS_F[i]);
   }
@@ -377,9 +380,9 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
   if (CIRC) {
     // e = 0: z^2 = a^2 (sin^2 phi + cos^2 phi cos^2 i) = a^2 cos^2 i + a^2 sin^2 i sin^2 phi
     R s;
-    if (fabs(ur) <= 0.125) {
+    if (fabs(ur) <= 0.0795) {
       R cm1;
-      rr_sincosm1_small((R)(RR_TWOPI * ur), s, cm1);   // |x| <= pi/4 < 0.8
+      rr_sincosm1_small((R)(RR_TWOPI * ur), s, cm1);   // |x| <= 0.4995
     } else {
       s = rr_sinpi((R)(2.0 * ur));
     }
@@ -412,11 +415,11 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
       const R dd = (R)-2 * g * gp * rr_rcp(fma((R)2 * gp, gp, -g * gpp));   // Halley
       iters += 1;
       if (fabs(dd) <= tol) {
-        // (sin, cos - 1) of d + dd, third order in dd
+        // (sin, cos - 1) of d + dd, second order in dd
         const R c = (R)1 + cm1;
-        const R h2 = (R)0.5 * dd * dd, h3 = h2 * dd * (R)(1.0 / 3.0);
-        s2 = fma(c, dd, s) - fma(s, h2, c * h3);
-        cm2 = fma(-s, dd, cm1) - fma(c, h2, -s * h3);
+        const R h2 = (R)0.5 * dd * dd;
+        s2 = fma(-s, h2, fma(c, dd, s));
+        cm2 = fma(-c, h2, fma(-s, dd, cm1));
         done = true;
         break;
       }
@@ -884,7 +887,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   // Blocks: one per (pv, chunk of consecutive tiles).  One chunk per pv when the population alone
   // gives every SM several waves of blocks (table row and constants staged once per pv);
   // otherwise the tile axis is cut so that about 8 waves of blocks exist.
-  const int64_t want = (int64_t)ctx->sm_count * RR_FLUX_MIN_BLOCKS * 8;
+  const int64_t want = (int64_t)ctx->sm_count * RR_FLUX_MIN_BLOCKS * RR_FLUX_WAVES;
   int64_t nchunks = (want + npv - 1) / npv;
   nchunks = std::max<int64_t>(1, std::min<int64_t>(nchunks, ctx->ntiles));
   const int64_t chunk_len = (ctx->ntiles + nchunks - 1) / nchunks;
