@@ -58,6 +58,11 @@ extern "C" {
 #define RR_PV_P_RANGE    8   /* p <= 0                             */
 #define RR_PV_NONFINITE 16   /* a NaN or infinity in the row       */
 
+/* how rr_build_ld_table / rr_evaluate share kernel 1's work (rr_set_table_mode) */
+#define RR_TABLE_LAZY     0  /* default: keep the profile, build at rr_evaluate only the two
+                                bracketing k rows each pv's k needs, collapsed */
+#define RR_TABLE_FULL     1  /* rr_build_ld_table builds the whole T[npv][npb][nk][ng]            */
+
 /* supersample reduction layout of the fused flux kernel (rr_set_reduction) */
 #define RR_REDUCE_AUTO    0  /* library picks per light curve from ns and the amount of work    */
 #define RR_REDUCE_THREAD  1  /* one thread per exposure, in-thread loop over its sub-samples    */
@@ -113,16 +118,27 @@ int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, i
  * d_ldp[npv][npb][nz]  the limb-darkening profile sampled at mu[nz] (ctx precision)
  * d_istar[npv][npb]    optional disk-integrated brightness (ctx precision); NULL = reading R6:
  *                      Istar = pi sum_j ldp[j] (ze[j+1]^2 - ze[j]^2)            (Eq. (2))
- * Builds T[npv][npb][nk][ng] = sum_j W[ik][ig][j] ldp[pv][pb][j] and Istar[npv][npb] in buffers
- * owned by ctx (grown as needed).  fp64 accumulation in both precisions.                        */
+ * The table is T[npv][npb][nk][ng] = sum_j W[ik][ig][j] ldp[pv][pb][j]; fp64 accumulation in both
+ * precisions.  The paper's evaluate needs, per (pv, passband), only the two rows that bracket the
+ * pv's k: ldw = (1-ak) dot(w[ik], ldp) + ak dot(w[ik+1], ldp).  This call does
+ * not receive k, so:
+ *   RR_TABLE_LAZY (default)  copies ldp into a buffer owned by ctx and computes Istar; the next
+ *                            rr_evaluate, which knows k, builds exactly those collapsed rows
+ *                            ldw[npv][npb][ng] (2/nk of the table's arithmetic) before the flux kernel;
+ *   RR_TABLE_FULL            builds all of T here (a [npv npb] x [nk ng] x [nz] product) and
+ *                            rr_evaluate collapses the two rows while staging them.
+ * Both give the same flux to rounding (tested).  Buffers are owned by ctx and grown as needed.   */
 int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64_t npv,
                       void *stream);
-/* Diagnostics: device pointers to the table and Istar built last (ctx precision), or NULL.      */
-const void *rr_table_ptr(const rr_ctx *ctx);
+/* RR_TABLE_*; takes effect at the next rr_build_ld_table.                                        */
+int rr_set_table_mode(rr_ctx *ctx, int32_t mode);
+/* Diagnostics: device pointers to the full table (built on demand in lazy mode; synchronous) and
+ * Istar of the last rr_build_ld_table (ctx precision), or NULL.                                 */
+const void *rr_table_ptr(rr_ctx *ctx);
 const void *rr_istar_ptr(const rr_ctx *ctx);
-/* Copies the table T[npv][npb][nk][ng] and Istar[npv][npb] built last to host arrays (ctx
- * precision; either may be NULL).  Synchronous (device-wide).                                   */
-int rr_get_table(const rr_ctx *ctx, void *h_T, void *h_istar);
+/* Copies the full table T[npv][npb][nk][ng] (built on demand in lazy mode) and Istar[npv][npb] to
+ * host arrays (ctx precision; either may be NULL).  Synchronous (device-wide).                   */
+int rr_get_table(rr_ctx *ctx, void *h_T, void *h_istar);
 
 /* ---- kernels 2+3+4: evaluate, PAPER.md:101-107, :128-131, :214, :220 ---------------------------
  * d_pv[npv][npar]   fp64 rows [k_0..k_{nkpb-1}, t0, p, a, i, e, w], npar = nkpb + 6: the order of
@@ -182,6 +198,13 @@ int rr_enable_counters(rr_ctx *ctx, int32_t on);
 int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts /*[8]*/);
 /* Number of kernel launches the library has made on this ctx since creation.                     */
 int64_t rr_launch_count(const rr_ctx *ctx);
+/* Device time of the kernels inside rr_evaluate, by CUDA events recorded on the caller's stream
+ * around them (rr_enable_kernel_timing(ctx, 1); at most 4096 calls are kept between reads).
+ * rr_get_kernel_times sums, over the rr_evaluate calls since the last read, h_ms[0] = the lazy row
+ * builder (kernel 1's share at evaluate time; 0 in RR_TABLE_FULL mode) and h_ms[1] = the fused
+ * flux kernel, and returns the number of calls in *h_calls.  Synchronous.                        */
+int rr_enable_kernel_timing(rr_ctx *ctx, int32_t on);
+int rr_get_kernel_times(rr_ctx *ctx, double *h_ms /*[2]*/, int64_t *h_calls);
 /* FP64 / FP32 FMA pipe peak of the current device, measured with a register-resident FMA chain
  * (DESIGN.md section 7): returns thread-level FMA instructions per second in *h_fma_per_s.
  * Synchronous.                                                                                   */

@@ -22,6 +22,7 @@ from . import build as _build
 
 RR_FP64, RR_FP32 = 0, 1
 RR_REDUCE_AUTO, RR_REDUCE_THREAD, RR_REDUCE_SHUFFLE = 0, 1, 2
+RR_TABLE_LAZY, RR_TABLE_FULL = 0, 1
 RR_PV_K_RANGE, RR_PV_E_RANGE, RR_PV_A_RANGE, RR_PV_P_RANGE, RR_PV_NONFINITE = 1, 2, 4, 8, 16
 
 # every symbol include/roadrunner.h declares (tests check the library exports each of them)
@@ -31,7 +32,8 @@ SYMBOLS = (
     "rr_evaluate",
     "rr_evaluate_flat", "rr_orbit_z", "rr_num_subsamples", "rr_num_tiles", "rr_get_tiles",
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
-    "rr_launch_count", "rr_measure_fma_peak",
+    "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
+    "rr_get_kernel_times",
 )
 
 
@@ -90,6 +92,9 @@ def load() -> C.CDLL:
         "rr_get_counters": (C.c_int, [_VP, _VP]),
         "rr_launch_count": (_I64, [_VP]),
         "rr_measure_fma_peak": (C.c_int, [_I32, C.POINTER(_DBL), _VP]),
+        "rr_set_table_mode": (C.c_int, [_VP, _I32]),
+        "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
+        "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
     for name, (res, args) in sig.items():
         f = getattr(lib, name)
@@ -234,6 +239,22 @@ def rr_get_tiles(ctx: int) -> dict:
 
 def rr_set_reduction(ctx: int, mode: int):
     _check(load().rr_set_reduction(ctx, mode), "rr_set_reduction")
+
+
+def rr_set_table_mode(ctx: int, mode: int):
+    _check(load().rr_set_table_mode(ctx, mode), "rr_set_table_mode")
+
+
+def rr_enable_kernel_timing(ctx: int, on: bool):
+    _check(load().rr_enable_kernel_timing(ctx, int(bool(on))), "rr_enable_kernel_timing")
+
+
+def rr_get_kernel_times(ctx: int) -> dict:
+    """Summed device ms of the lazy row builder and of the flux kernel since the last read."""
+    ms = np.zeros(2)
+    calls = _I64(0)
+    _check(load().rr_get_kernel_times(ctx, ms.ctypes.data, C.byref(calls)), "rr_get_kernel_times")
+    return {"rows_ms": float(ms[0]), "flux_ms": float(ms[1]), "calls": int(calls.value)}
 
 
 def rr_evaluate_host(ctx: int, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray,

@@ -18,6 +18,8 @@ void free_work(RRWork *w) {
   if (w->istar) cudaFree(w->istar);
   if (w->pvo) cudaFree(w->pvo);
   if (w->pvb) cudaFree(w->pvb);
+  if (w->ldp) cudaFree(w->ldp);
+  if (w->rows) cudaFree(w->rows);
   memset(w, 0, sizeof(*w));
   w->table_npv = -1;
 }
@@ -42,6 +44,9 @@ int tile_len_for(int ns) {
   r = std::max(1, std::min(8, r));
   return 256 * r;
 }
+
+// The lazy row builder keeps one profile (nz doubles) in shared memory.
+bool lazy_ok(const rr_ctx *ctx) { return ctx->table_mode == RR_TABLE_LAZY && ctx->nz <= 4096; }
 
 int grow(void **p, int64_t *cap, int64_t need) {
   if (need <= *cap) return RR_OK;
@@ -93,6 +98,7 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   ctx->nsub = -1;
   for (auto &w : ctx->work) w.table_npv = -1;
   ctx->reduction = RR_REDUCE_AUTO;
+  ctx->table_mode = RR_TABLE_LAZY;
   int rc = RR_OK;
   cudaError_t e = cudaGetDevice(&ctx->device);
   if (e == cudaSuccess)
@@ -113,6 +119,8 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
 int rr_destroy(rr_ctx *ctx) {
   if (!ctx) return RR_ENULL;
   cudaDeviceSynchronize();
+  for (auto e : ctx->tev) cudaEventDestroy(e);
+  ctx->tev.clear();
   free_data(ctx);
   for (auto &w : ctx->work) free_work(&w);
   void *bufs[] = {ctx->d_ze, ctx->d_zm, ctx->d_mu, ctx->d_q, ctx->d_W, ctx->d_tiles,
@@ -208,22 +216,39 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
                       void *stream) {
   if (!ctx || !d_ldp) return RR_ENULL;
   if (npv <= 0) return RR_ESIZE;
+  if (lazy_ok(ctx))
+    return rr_ld_profile_launch(ctx, &ctx->work[0], d_ldp, d_istar, npv, 1, (cudaStream_t)stream);
   return rr_ld_table_launch(ctx, &ctx->work[0], d_ldp, d_istar, npv, (cudaStream_t)stream);
 }
 
-const void *rr_table_ptr(const rr_ctx *ctx) {
-  return (ctx && ctx->work[0].table_npv > 0) ? ctx->work[0].T : nullptr;
+int rr_set_table_mode(rr_ctx *ctx, int32_t mode) {
+  if (!ctx) return RR_ENULL;
+  if (mode != RR_TABLE_LAZY && mode != RR_TABLE_FULL) return RR_ECONFIG;
+  ctx->table_mode = mode;
+  return RR_OK;
+}
+
+const void *rr_table_ptr(rr_ctx *ctx) {
+  if (!ctx || ctx->work[0].table_npv <= 0) return nullptr;
+  if (rr_ld_full_from_profile(ctx, &ctx->work[0], nullptr) != RR_OK) return nullptr;
+  if (cudaDeviceSynchronize() != cudaSuccess) return nullptr;
+  return ctx->work[0].T;
 }
 
 const void *rr_istar_ptr(const rr_ctx *ctx) {
   return (ctx && ctx->work[0].table_npv > 0) ? ctx->work[0].istar : nullptr;
 }
 
-int rr_get_table(const rr_ctx *ctx, void *h_T, void *h_istar) {
+int rr_get_table(rr_ctx *ctx, void *h_T, void *h_istar) {
   if (!ctx) return RR_ENULL;
-  const RRWork &w = ctx->work[0];
+  RRWork &w = ctx->work[0];
   if (w.table_npv <= 0) return RR_ESTATE;
   RR_CUDA(cudaDeviceSynchronize());
+  if (h_T) {
+    int rc = rr_ld_full_from_profile(ctx, &w, nullptr);
+    if (rc != RR_OK) return rc;
+    RR_CUDA(cudaDeviceSynchronize());
+  }
   const size_t rows = (size_t)w.table_npv * ctx->cfg.npb, es = (size_t)esize(ctx);
   if (h_T)
     RR_CUDA(cudaMemcpy(h_T, w.T, rows * ctx->cfg.nk * ctx->cfg.ng * es, cudaMemcpyDeviceToHost));
@@ -239,7 +264,18 @@ int rr_evaluate(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, void
   cudaStream_t st = (cudaStream_t)stream;
   int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, d_status, st);
   if (rc != RR_OK) return rc;
-  return rr_flux_launch(ctx, &ctx->work[0], npv, d_flux, st);
+  cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+  const bool timed = ctx->timing_on && ctx->tev.size() < 3 * 4096;
+  if (timed) {
+    for (auto &e : ev) RR_CUDA(cudaEventCreate(&e));
+    for (auto e : ev) ctx->tev.push_back(e);
+    RR_CUDA(cudaEventRecord(ev[0], st));
+  }
+  if (ctx->work[0].lazy && (rc = rr_ld_rows_launch(ctx, &ctx->work[0], npv, st)) != RR_OK) return rc;
+  if (timed) RR_CUDA(cudaEventRecord(ev[1], st));
+  rc = rr_flux_launch(ctx, &ctx->work[0], npv, d_flux, st);
+  if (timed) RR_CUDA(cudaEventRecord(ev[2], st));
+  return rc;
 }
 
 int rr_evaluate_flat(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, int64_t npt,
@@ -322,8 +358,13 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
     RR_CUDA(cudaMemcpyAsync(d_pv, (const char *)h_pv + v0 * pv_row, nv * pv_row,
                             cudaMemcpyHostToDevice, st));
     RRWork *wk = &ctx->work[1 + s];
-    if ((rc = rr_ld_table_launch(ctx, wk, d_ldp, nullptr, nv, st)) != RR_OK) break;
+    if (lazy_ok(ctx)) {   // the staging buffer lives until this chunk's kernels are done
+      if ((rc = rr_ld_profile_launch(ctx, wk, d_ldp, nullptr, nv, 0, st)) != RR_OK) break;
+    } else if ((rc = rr_ld_table_launch(ctx, wk, d_ldp, nullptr, nv, st)) != RR_OK) {
+      break;
+    }
     if ((rc = rr_pv_prep_launch(ctx, wk, d_pv, nv, d_status, st)) != RR_OK) break;
+    if (wk->lazy && (rc = rr_ld_rows_launch(ctx, wk, nv, st)) != RR_OK) break;
     if ((rc = rr_flux_launch(ctx, wk, nv, d_flux, st)) != RR_OK) break;
     RR_CUDA(cudaMemcpyAsync((char *)h_flux + v0 * flux_row, d_flux, nv * flux_row,
                             cudaMemcpyDeviceToHost, st));
@@ -351,6 +392,36 @@ int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts) {
 }
 
 int64_t rr_launch_count(const rr_ctx *ctx) { return ctx ? ctx->launches : -1; }
+
+int rr_enable_kernel_timing(rr_ctx *ctx, int32_t on) {
+  if (!ctx) return RR_ENULL;
+  ctx->timing_on = on ? 1 : 0;
+  return RR_OK;
+}
+
+int rr_get_kernel_times(rr_ctx *ctx, double *h_ms, int64_t *h_calls) {
+  if (!ctx || !h_ms || !h_calls) return RR_ENULL;
+  h_ms[0] = h_ms[1] = 0.0;
+  *h_calls = 0;
+  int rc = RR_OK;
+  for (size_t i = 0; i + 2 < ctx->tev.size(); i += 3) {
+    cudaEvent_t *e = &ctx->tev[i];
+    float a = 0.f, b = 0.f;
+    cudaError_t err = cudaEventSynchronize(e[2]);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&a, e[0], e[1]);
+    if (err == cudaSuccess) err = cudaEventElapsedTime(&b, e[1], e[2]);
+    if (err == cudaSuccess) {
+      h_ms[0] += a;
+      h_ms[1] += b;
+      ++*h_calls;
+    } else if (rc == RR_OK) {
+      rc = RR_ECUDA_BASE - (int)err;
+    }
+    for (int q = 0; q < 3; ++q) cudaEventDestroy(e[q]);
+  }
+  ctx->tev.clear();
+  return rc;
+}
 
 int rr_measure_fma_peak(int32_t precision, double *h_fma_per_s, void *stream) {
   if (!h_fma_per_s) return RR_ENULL;

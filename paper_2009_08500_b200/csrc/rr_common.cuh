@@ -66,8 +66,17 @@ struct RRPvBand {
 // host-buffer path (so that two chunks can be in flight on two streams).
 struct RRWork {
   void *T, *istar;          // kernel 1 output (ctx precision)
-  int64_t table_npv;        // npv of the table built last; -1 = none
+  int64_t table_npv;        // npv of the table / profile set last; -1 = none
   int64_t T_cap, istar_cap; // bytes
+  // lazy table mode (RR_TABLE_LAZY): the profile is kept and rr_evaluate builds, for every
+  // (pv, passband), only the k-collapsed row its k needs
+  void *ldp;                // owned copy of the caller's ldp (device API)
+  int64_t ldp_cap;
+  const void *ldp_src;      // profile the row builder reads: ldp, or the host path's staging
+  void *rows;               // ldw[npv][npb][ng], ctx precision
+  int64_t rows_cap;
+  int32_t lazy;             // 1: evaluate from rows; 0: evaluate from T
+  int32_t have_full;        // T holds the full table of the current profile
   RRPvOrbit *pvo;
   RRPvBand *pvb;
   int64_t pv_cap;
@@ -96,12 +105,17 @@ struct rr_ctx {
   int64_t scratch_cap;
   int32_t reduction;
   int32_t any_shuffle;
+  int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL
   // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
   RRWork work[3];
   // counters / accounting
   unsigned long long *d_counters;
   int32_t counters_on;
   int64_t launches;
+  // per-kernel device timing of rr_evaluate (rr_enable_kernel_timing): event triples
+  // (before rows, before flux, after flux) of the calls since the last read
+  int32_t timing_on;
+  std::vector<cudaEvent_t> tev;
   // host path
   cudaStream_t hs[2];
   cudaEvent_t hev[2];
@@ -127,6 +141,10 @@ struct rr_ctx {
 int rr_geometry_build(rr_ctx *ctx);                                            // rr_geometry.cu
 int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp,             // rr_ld_table.cu
                        const void *d_istar, int64_t npv, cudaStream_t st);
+int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar,
+                         int64_t npv, int copy, cudaStream_t st);              // rr_ld_table.cu
+int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_ld_table.cu
+int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st);         // rr_ld_table.cu
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
                       int32_t *d_status, cudaStream_t st);                     // rr_flux.cu

@@ -490,7 +490,8 @@ struct FluxParams {
   const RRLc *lcs;
   const RRPvOrbit *pvo;
   const RRPvBand *pvb;
-  const void *T;
+  const void *T;        // full table (RR_TABLE_FULL) or NULL
+  const void *rows;     // collapsed rows ldw[npv][npb][ng] (RR_TABLE_LAZY) or NULL
   const void *istar;
   void *flux;
   unsigned long long *counters;
@@ -700,13 +701,18 @@ rr_flux_kernel(const FluxParams P) {
         const int kb = (P.nkpb == 1) ? 0 : lc.pb;
         const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
         const int64_t trow = (int64_t)v * P.npb + lc.pb;
-        const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
-        const R *T1 = T0 + P.ng;
-        const R ak = (R)pb.ak;
         __syncthreads();
-        for (int ig = threadIdx.x; ig <= P.ng; ig += FT) {
-          const int jg = min(ig, P.ng - 1);          // ldw[ng] = ldw[ng-1]: see rr_cell
-          ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
+        if (P.rows) {                                  // lazy mode: the row was collapsed for this k
+          const R *rw = reinterpret_cast<const R *>(P.rows) + trow * (int64_t)P.ng;
+          for (int ig = threadIdx.x; ig <= P.ng; ig += FT) ldw[ig] = rw[min(ig, P.ng - 1)];
+        } else {
+          const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
+          const R *T1 = T0 + P.ng;
+          const R ak = (R)pb.ak;
+          for (int ig = threadIdx.x; ig <= P.ng; ig += FT) {
+            const int jg = min(ig, P.ng - 1);          // ldw[ng] = ldw[ng-1]: see rr_cell
+            ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
+          }
         }
         rr_stage_constants<R>(cst, po, pb);
         if (threadIdx.x == K_COUNT)
@@ -865,7 +871,8 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.lcs = ctx->d_lc;
   P.pvo = wk->pvo;
   P.pvb = wk->pvb;
-  P.T = wk->T;
+  P.T = wk->lazy ? nullptr : wk->T;
+  P.rows = wk->lazy ? wk->rows : nullptr;
   P.istar = wk->istar;
   P.flux = d_flux;
   P.counters = ctx->d_counters;

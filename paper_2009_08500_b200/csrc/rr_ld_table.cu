@@ -124,6 +124,46 @@ __global__ void rr_istar_kernel(const TA *__restrict__ A, const double *__restri
   if (lane == 0) out[row] = (TC)s;
 }
 
+// Lazy mode: the k-collapsed row of one (pv, passband),
+//   ldw[ig] = (1 - ak) sum_j W[ik][ig][j] ldp[j] + ak sum_j W[ik+1][ig][j] ldp[j]
+// for the pv's own k (ik, ak from the per-pv prep).  One block per (pv, passband); the profile sits
+// in shared memory; one warp per g node, lanes over j (coalesced reads of W, which stays in L2:
+// the two rows are 2 ng nz 8 B = 160 kB), shuffle sums.  fp64 accumulation in both precisions.
+constexpr int RT = 256;
+template <typename TR>
+__global__ void __launch_bounds__(RT)
+rr_ld_rows_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
+                  const RRPvBand *__restrict__ pvb, TR *__restrict__ rows, int npb, int nkpb,
+                  int ng, int nz) {
+  extern __shared__ double prof[];
+  const int64_t row = blockIdx.x;                 // pv * npb + pb
+  const int64_t v = row / npb;
+  const int pb = (int)(row - v * npb);
+  const RRPvBand &b = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)];
+  const int ik = b.ik;
+  const double ak = b.ak;
+  for (int j = threadIdx.x; j < nz; j += RT) prof[j] = (double)ldp[row * nz + j];
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const double *W0 = W + (int64_t)ik * ng * nz;
+  const double *W1 = W0 + (int64_t)ng * nz;
+  for (int ig = warp; ig < ng; ig += RT / 32) {
+    const double *w0 = W0 + (int64_t)ig * nz, *w1 = W1 + (int64_t)ig * nz;
+    double s0 = 0.0, s1 = 0.0;
+    for (int j = lane; j < nz; j += 32) {
+      const double p = prof[j];
+      s0 = fma(w0[j], p, s0);
+      s1 = fma(w1[j], p, s1);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+      s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    }
+    if (lane == 0) rows[row * ng + ig] = (TR)fma(ak, s1 - s0, s0);
+  }
+}
+
 template <typename TR>
 int launch_typed(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar, int64_t npv,
                  cudaStream_t st) {
@@ -168,5 +208,93 @@ int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d
   int rc = c.precision == RR_FP32 ? launch_typed<float>(ctx, wk, d_ldp, d_istar, npv, st)
                                   : launch_typed<double>(ctx, wk, d_ldp, d_istar, npv, st);
   wk->table_npv = rc == RR_OK ? npv : -1;
+  wk->lazy = 0;
+  wk->have_full = rc == RR_OK;
+  wk->ldp_src = nullptr;
   return rc;
+}
+
+static int grow_buf(void **p, int64_t *cap, int64_t need) {
+  if (need <= *cap) return RR_OK;
+  if (*p) cudaFree(*p);
+  *p = nullptr;
+  *cap = 0;
+  if (cudaMalloc(p, (size_t)need) != cudaSuccess) { cudaGetLastError(); return RR_EALLOC; }
+  *cap = need;
+  return RR_OK;
+}
+
+// Lazy mode, at rr_build_ld_table: keep the profile (copy = 1: into a buffer of ours; 0: the
+// caller guarantees d_ldp lives until the evaluation, the host path's staging) and compute Istar.
+int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar,
+                         int64_t npv, int copy, cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t M = npv * c.npb, needP = M * ctx->nz * esz, needI = M * esz;
+  wk->table_npv = -1;
+  int rc = grow_buf(&wk->istar, &wk->istar_cap, needI);
+  if (rc == RR_OK && copy) rc = grow_buf(&wk->ldp, &wk->ldp_cap, needP);
+  if (rc != RR_OK) return rc;
+  if (copy) {
+    RR_CUDA(cudaMemcpyAsync(wk->ldp, d_ldp, (size_t)needP, cudaMemcpyDeviceToDevice, st));
+    wk->ldp_src = wk->ldp;
+  } else {
+    wk->ldp_src = d_ldp;
+  }
+  const int64_t threads = M * 32;
+  if (c.precision == RR_FP32)
+    rr_istar_kernel<float, float><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+        (const float *)d_ldp, ctx->d_q, (const float *)d_istar, (float *)wk->istar, M, ctx->nz);
+  else
+    rr_istar_kernel<double, double><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+        (const double *)d_ldp, ctx->d_q, (const double *)d_istar, (double *)wk->istar, M, ctx->nz);
+  RR_LAUNCH_CHECK(ctx);
+  wk->table_npv = npv;
+  wk->lazy = 1;
+  wk->have_full = 0;
+  return RR_OK;
+}
+
+// Lazy mode, at rr_evaluate (after the per-pv prep): the rows the flux kernel stages.
+int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t M = npv * c.npb;
+  if (M > 0x7fffffffLL) return RR_ESIZE;
+  int rc = grow_buf(&wk->rows, &wk->rows_cap, M * c.ng * esz);
+  if (rc != RR_OK) return rc;
+  const size_t smem = sizeof(double) * ctx->nz;
+  if (c.precision == RR_FP32)
+    rr_ld_rows_kernel<float><<<(unsigned)M, RT, smem, st>>>(
+        (const float *)wk->ldp_src, ctx->d_W, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
+        ctx->nz);
+  else
+    rr_ld_rows_kernel<double><<<(unsigned)M, RT, smem, st>>>(
+        (const double *)wk->ldp_src, ctx->d_W, wk->pvb, (double *)wk->rows, c.npb, c.nkpb, c.ng,
+        ctx->nz);
+  RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
+// Diagnostics in lazy mode: the full table of the kept profile, built on demand.
+int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st) {
+  if (wk->have_full) return RR_OK;
+  if (wk->table_npv <= 0 || wk->ldp_src != wk->ldp || !wk->ldp) return RR_ESTATE;
+  const rr_config &c = ctx->cfg;
+  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t npv = wk->table_npv;
+  int rc = grow_buf(&wk->T, &wk->T_cap, npv * c.npb * (int64_t)c.nk * c.ng * esz);
+  if (rc != RR_OK) return rc;
+  const int64_t M = npv * c.npb;
+  const int N = c.nk * c.ng, K = ctx->nz;
+  dim3 grid((N + BN - 1) / BN, (unsigned)((M + BM - 1) / BM));
+  if (c.precision == RR_FP32)
+    rr_ld_table_kernel<float, float><<<grid, NT, 0, st>>>((const float *)wk->ldp, ctx->d_W,
+                                                          (float *)wk->T, M, N, K);
+  else
+    rr_ld_table_kernel<double, double><<<grid, NT, 0, st>>>((const double *)wk->ldp, ctx->d_W,
+                                                            (double *)wk->T, M, N, K);
+  RR_LAUNCH_CHECK(ctx);
+  wk->have_full = 1;
+  return RR_OK;
 }

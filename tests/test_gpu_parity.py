@@ -149,6 +149,39 @@ def test_reduction_layouts_agree(rr, config, precision):
     assert np.max(np.abs(a - b)) <= (1e-6 if precision else 1e-14)
 
 
+@pytest.mark.parametrize("config,precision", [(1, 0), (3, 0), (3, 1), (4, 0)])
+def test_table_modes_agree(rr, config, precision):
+    """RR_TABLE_LAZY (rows for each pv's k at evaluate time) and RR_TABLE_FULL
+    (whole T, rows collapsed while staging): same flux to rounding, both within tolerance."""
+    wl = small_workload(config)
+    want, _ = oracle_flux(wl)
+    out = {}
+    for mode in (rr.RR_TABLE_LAZY, rr.RR_TABLE_FULL):
+        gm = rr.RoadRunner.from_config(wl.model, precision)
+        rr.rr_set_table_mode(gm.ctx, mode)
+        gm.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
+        gm.build_ld_table(wl.ldp(gm.mu))
+        out[mode] = gm.evaluate(wl.pv).cpu().numpy().astype(np.float64)
+        gm.close()
+    tol = TOL32 if precision else TOL64
+    for got in out.values():
+        assert np.max(np.abs(got - want)) <= tol
+    assert np.max(np.abs(out[rr.RR_TABLE_LAZY] - out[rr.RR_TABLE_FULL])) <= (2e-7 if precision else 1e-14)
+
+
+def test_kernel_timing_counts_calls(rr):
+    wl = small_workload(1)
+    gm = gpu_model(rr, wl)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    rr.rr_enable_kernel_timing(gm.ctx, True)
+    for _ in range(3):
+        gm.evaluate(wl.pv)
+    t = rr.rr_get_kernel_times(gm.ctx)
+    assert t["calls"] == 3 and t["flux_ms"] > 0 and t["rows_ms"] > 0
+    assert rr.rr_get_kernel_times(gm.ctx)["calls"] == 0
+    gm.close()
+
+
 # ---- kernel 2 alone ------------------------------------------------------------------------------------
 @pytest.mark.parametrize("config", [1, 3, 4])
 def test_orbit_z_matches_oracle(rr, config):
