@@ -20,6 +20,7 @@ void free_work(RRWork *w) {
   if (w->pvb) cudaFree(w->pvb);
   if (w->ldp) cudaFree(w->ldp);
   if (w->rows) cudaFree(w->rows);
+  if (w->bk) cudaFree(w->bk);
   memset(w, 0, sizeof(*w));
   w->table_npv = -1;
 }

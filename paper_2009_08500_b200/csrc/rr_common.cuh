@@ -75,6 +75,8 @@ struct RRWork {
   const void *ldp_src;      // profile the row builder reads: ldp, or the host path's staging
   void *rows;               // ldw[npv][npb][ng], ctx precision
   int64_t rows_cap;
+  int32_t *bk;              // row buckets by ik: hist[nk] | cursor[nk] | offs[nk+1] | tileoff[nk+1] | list[M]
+  int64_t bk_cap;
   int32_t lazy;             // 1: evaluate from rows; 0: evaluate from T
   int32_t have_full;        // T holds the full table of the current profile
   RRPvOrbit *pvo;

@@ -164,6 +164,106 @@ rr_ld_rows_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
   }
 }
 
+// Lazy mode at scale: rows (pv, passband) are bucketed by their lower k row ik (counting sort:
+// histogram, scan, scatter), and one block builds RB rows of ONE bucket, so that the two weight rows
+// W[ik], W[ik+1] are read once per RB profiles (warp-uniform loads served by L1) instead of once per
+// profile from L2 (2.6 GB of L2 reads at config 4 otherwise).  Lane = row, warp = g nodes.
+constexpr int RB = 32;
+
+__device__ __forceinline__ int rr_row_ik(const RRPvBand *__restrict__ pvb, int64_t row, int npb,
+                                         int nkpb) {
+  const int64_t v = row / npb;
+  const int pb = (int)(row - v * npb);
+  return pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].ik;
+}
+
+__global__ void rr_rows_hist(const RRPvBand *__restrict__ pvb, int64_t M, int npb, int nkpb,
+                             int *__restrict__ hist) {
+  const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (row < M) atomicAdd(&hist[rr_row_ik(pvb, row, npb, nkpb)], 1);
+}
+
+// One block: exclusive scans of the bucket sizes and of their tile counts (nb <= 4096 buckets).
+__global__ void rr_rows_scan(int nb, const int *__restrict__ hist, int *__restrict__ offs,
+                             int *__restrict__ tileoff) {
+  if (threadIdx.x == 0) {
+    int o = 0, t = 0;
+    for (int b = 0; b < nb; ++b) {
+      offs[b] = o;
+      tileoff[b] = t;
+      o += hist[b];
+      t += (hist[b] + RB - 1) / RB;
+    }
+    offs[nb] = o;
+    tileoff[nb] = t;
+  }
+}
+
+__global__ void rr_rows_scatter(const RRPvBand *__restrict__ pvb, int64_t M, int npb, int nkpb,
+                                const int *__restrict__ offs, int *__restrict__ cursor,
+                                int *__restrict__ list) {
+  const int64_t row = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (row >= M) return;
+  const int ik = rr_row_ik(pvb, row, npb, nkpb);
+  list[offs[ik] + atomicAdd(&cursor[ik], 1)] = (int)row;
+}
+
+template <typename TR>
+__global__ void __launch_bounds__(256)
+rr_ld_rows_bucket_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
+                         const RRPvBand *__restrict__ pvb, const int *__restrict__ list,
+                         const int *__restrict__ offs, const int *__restrict__ tileoff, int nb,
+                         TR *__restrict__ rows, int npb, int nkpb, int ng, int nz, int stride) {
+  extern __shared__ double prof[];                 // [RB][stride], stride odd: conflict-free
+  __shared__ int rid[RB];
+  __shared__ double akr[RB];
+  const int b = blockIdx.x;
+  if (b >= tileoff[nb]) return;
+  int lo = 0, hi = nb - 1;                         // last bucket whose first tile is <= b
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (tileoff[mid] <= b) lo = mid; else hi = mid - 1;
+  }
+  const int ik = lo;
+  const int r0 = offs[ik] + (b - tileoff[ik]) * RB;
+  const int nr = min(RB, offs[ik + 1] - r0);
+  if (threadIdx.x < RB) {
+    int row = -1;
+    double ak = 0.0;
+    if ((int)threadIdx.x < nr) {
+      row = list[r0 + threadIdx.x];
+      const int64_t v = row / npb;
+      const int pb = (int)(row - v * npb);
+      ak = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].ak;
+    }
+    rid[threadIdx.x] = row;
+    akr[threadIdx.x] = ak;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < RB * nz; idx += 256) {
+    const int r = idx / nz, j = idx - r * nz;
+    prof[r * stride + j] = (r < nr) ? (double)ldp[(int64_t)rid[r] * nz + j] : 0.0;
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const double *W0 = W + (int64_t)ik * ng * nz;
+  const double *W1 = W0 + (int64_t)ng * nz;
+  const double *pr = prof + lane * stride;
+  const double ak = akr[lane];
+  const int64_t orow = (int64_t)rid[lane] * ng;
+  for (int ig = warp; ig < ng; ig += 8) {
+    const double *w0 = W0 + (int64_t)ig * nz, *w1 = W1 + (int64_t)ig * nz;
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll 4
+    for (int j = 0; j < nz; ++j) {
+      const double p = pr[j];
+      s0 = fma(__ldg(w0 + j), p, s0);
+      s1 = fma(__ldg(w1 + j), p, s1);
+    }
+    if (lane < nr) rows[orow + ig] = (TR)fma(ak, s1 - s0, s0);
+  }
+}
+
 template <typename TR>
 int launch_typed(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar, int64_t npv,
                  cudaStream_t st) {
@@ -263,6 +363,43 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
   if (M > 0x7fffffffLL) return RR_ESIZE;
   int rc = grow_buf(&wk->rows, &wk->rows_cap, M * c.ng * esz);
   if (rc != RR_OK) return rc;
+  const int nb = c.nk - 1;                         // buckets: lower k row ik in [0, nk-2]
+  const int stride = ctx->nz | 1;
+  const size_t smem_b = sizeof(double) * RB * stride;
+  if (M >= 2048 && nb <= 4096 && smem_b <= 96 * 1024) {
+    // bucketed builder
+    const int64_t need = sizeof(int32_t) * (4 * (int64_t)nb + 4 + M);
+    rc = grow_buf((void **)&wk->bk, &wk->bk_cap, need);
+    if (rc != RR_OK) return rc;
+    int *hist = wk->bk, *cursor = hist + nb, *offs = cursor + nb, *tileoff = offs + nb + 1,
+        *list = tileoff + nb + 1;
+    RR_CUDA(cudaMemsetAsync(hist, 0, sizeof(int32_t) * 2 * nb, st));
+    const unsigned gb = (unsigned)((M + 255) / 256);
+    rr_rows_hist<<<gb, 256, 0, st>>>(wk->pvb, M, c.npb, c.nkpb, hist);
+    RR_LAUNCH_CHECK(ctx);
+    rr_rows_scan<<<1, 32, 0, st>>>(nb, hist, offs, tileoff);
+    RR_LAUNCH_CHECK(ctx);
+    rr_rows_scatter<<<gb, 256, 0, st>>>(wk->pvb, M, c.npb, c.nkpb, offs, cursor, list);
+    RR_LAUNCH_CHECK(ctx);
+    const unsigned tiles_max = (unsigned)((M + RB - 1) / RB + nb);
+    if (c.precision == RR_FP32) {
+      if (smem_b > 48 * 1024)
+        RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<float>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+      rr_ld_rows_bucket_kernel<float><<<tiles_max, 256, smem_b, st>>>(
+          (const float *)wk->ldp_src, ctx->d_W, wk->pvb, list, offs, tileoff, nb, (float *)wk->rows,
+          c.npb, c.nkpb, c.ng, ctx->nz, stride);
+    } else {
+      if (smem_b > 48 * 1024)
+        RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<double>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+      rr_ld_rows_bucket_kernel<double><<<tiles_max, 256, smem_b, st>>>(
+          (const double *)wk->ldp_src, ctx->d_W, wk->pvb, list, offs, tileoff, nb,
+          (double *)wk->rows, c.npb, c.nkpb, c.ng, ctx->nz, stride);
+    }
+    RR_LAUNCH_CHECK(ctx);
+    return RR_OK;
+  }
   const size_t smem = sizeof(double) * ctx->nz;
   if (c.precision == RR_FP32)
     rr_ld_rows_kernel<float><<<(unsigned)M, RT, smem, st>>>(

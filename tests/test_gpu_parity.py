@@ -149,11 +149,15 @@ def test_reduction_layouts_agree(rr, config, precision):
     assert np.max(np.abs(a - b)) <= (1e-6 if precision else 1e-14)
 
 
-@pytest.mark.parametrize("config,precision", [(1, 0), (3, 0), (3, 1), (4, 0)])
-def test_table_modes_agree(rr, config, precision):
-    """RR_TABLE_LAZY (rows for each pv's k at evaluate time) and RR_TABLE_FULL
-    (whole T, rows collapsed while staging): same flux to rounding, both within tolerance."""
-    wl = small_workload(config)
+@pytest.mark.parametrize("config,precision,shape", [
+    (1, 0, None), (3, 0, None), (3, 1, None), (4, 0, None),
+    (4, 0, (2500, 400)), (3, 0, (700, 6 * 60)), (3, 1, (700, 6 * 60))])   # >= 2048 rows: bucketed builder
+def test_table_modes_agree(rr, config, precision, shape):
+    """RR_TABLE_LAZY (rows for each pv's k at evaluate time; per-row builder
+    below 2048 (pv, passband) rows, ik-bucketed builder above) and RR_TABLE_FULL (whole T, rows
+    collapsed while staging): same flux to rounding, both within tolerance."""
+    wl = small_workload(config) if shape is None else \
+        workloads.make_workload(config, npv=shape[0], npt=shape[1])
     want, _ = oracle_flux(wl)
     out = {}
     for mode in (rr.RR_TABLE_LAZY, rr.RR_TABLE_FULL):
