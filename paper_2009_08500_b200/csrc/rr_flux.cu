@@ -337,10 +337,9 @@ __device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, c
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
-// Returns (sin d, cos d - 1) of the root; iters counts sincos evaluations.
+// Stores (sin d, cos d - 1) of the root; returns the number of sincos evaluations.
 template <typename R>
-__device__ __noinline__ void rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out, R *cm1_out,
-                                              int *iters) {
+__device__ __noinline__ int rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out, R *cm1_out) {
   // root bracketed by E in [M - e, M + e]  <=>  d in [dM - e sE - e, dM - e sE + e]
   const R mid = fma(-e, sE, dM);
   R lo = mid - e, hi = mid + e;
@@ -366,11 +365,11 @@ __device__ __noinline__ void rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out, R
     d = dn;
     if (fabs(dd) <= tol) { ++it; break; }
   }
-  *iters += it;
   // rotate (sin, cos - 1) of the last evaluated d by the last small step dd, to second order
   const R hdd2 = (R)0.5 * dd * dd;
   *s_out = s + c * dd - s * hdd2;
   *cm1_out = cm1 - s * dd - c * hdd2;
+  return it;
 }
 
 // ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
@@ -426,7 +425,7 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
       d += dd;
     }
   }
-  if (!done) rr_kepler_robust<R>(k[K_E], k[K_SE], k[K_CE], dM, &s2, &cm2, &iters);
+  if (!done) iters += rr_kepler_robust<R>(k[K_E], k[K_SE], k[K_CE], dM, &s2, &cm2);
   R X1, X2, Y1, Y2, Y0, aci2;
   k.pair(K_X1, X1, X2);
   k.pair(K_Y1, Y1, Y2);
@@ -533,8 +532,8 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 // Occulted light of the sub-sample at phase w (turns, measured from the window centre).
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
 template <typename R, bool COUNT, bool CIRC>
-__device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid, const Cst<R> k,
-                                          const R *__restrict__ ldw, int ng,
+__device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
+                                          const Cst<R> k, const R *__restrict__ ldw, int ng,
                                           unsigned long long *cnt) {
   const double wr = w - rr_round(w);
   R def = (R)0;
