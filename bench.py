@@ -75,6 +75,19 @@ def workload_config(wl, precision, extra=None):
     return cfg
 
 
+def ncu_traffic(workload: str, precision: str):
+    """dram read + write bytes per launch of rr_flux_kernel from the committed ncu capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "flux_kernel_dram_traffic.csv")) as f:
+            for line in f.read().splitlines()[1:]:
+                w, p, rd, wr, _ = line.split(",")
+                if w == workload and p == precision:
+                    return int(rd) + int(wr)
+    except (OSError, ValueError):
+        pass
+    return None
+
+
 # ---- clocks ------------------------------------------------------------------------------------
 CLOCK_FIELDS = ["clocks.sm", "clocks.max.sm", "power.draw",
                 "clocks_event_reasons.hw_slowdown", "clocks_event_reasons.hw_thermal_slowdown",
@@ -328,6 +341,7 @@ def run_ours(args):
                     "unit": "TFLOP/s", "frac": alu_achieved / alu_peak_tflops, "traffic": None,
                     "peak_source": f"{lanes} FMA lanes/clk/SM x {SM_COUNT} SMs x {sm_max:.0f} MHz "
                                    "x 2 (DESIGN.md s7)"}
+    roofline["traffic"] = ncu_traffic(wl.name, args.precision)
     roofline.update({
         "kernel": "rr_flux_kernel", "kernel_ms": ms_flux, "ld_table_kernel_ms": ms_table + ms_rows,
         "ld_table_parts_ms": {"rr_build_ld_table": ms_table, "rows_in_rr_evaluate": ms_rows},
