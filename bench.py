@@ -56,8 +56,9 @@ def parse_args():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
     ap.add_argument("--npv", type=int, default=None, help="shrink the population (debugging)")
     ap.add_argument("--npt", type=int, default=None, help="shrink the time axis (debugging)")
-    ap.add_argument("--table-mode", default="lazy", choices=["lazy", "full"],
-                    help="kernel 1: rows for each pv's k at evaluate time (default) or the full table")
+    ap.add_argument("--table-mode", default="lazy", choices=["lazy", "full", "direct"],
+                    help="kernel 1: rows for each pv's k at evaluate time (default), the full table, "
+                         "or the paper's direct model (weights at each pv's own k, no k grid)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -215,7 +216,8 @@ def run_ours(args):
         wl.ld_coeffs = np.ascontiguousarray(np.roll(wl.ld_coeffs, sh, axis=0))
 
     model = rr.RoadRunner.from_config(wl.model, precision)
-    rr.rr_set_table_mode(model.ctx, rr.RR_TABLE_FULL if args.table_mode == "full" else rr.RR_TABLE_LAZY)
+    rr.rr_set_table_mode(model.ctx, {"lazy": rr.RR_TABLE_LAZY, "full": rr.RR_TABLE_FULL,
+                                     "direct": rr.RR_TABLE_DIRECT}[args.table_mode])
     model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
     ldp_h = np.ascontiguousarray(wl.ldp(model.mu), dtype=npdt)
     ldp = torch.as_tensor(ldp_h).to(dev)

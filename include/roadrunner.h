@@ -62,6 +62,9 @@ extern "C" {
 #define RR_TABLE_LAZY     0  /* default: keep the profile, build at rr_evaluate only the two
                                 bracketing k rows each pv's k needs, collapsed */
 #define RR_TABLE_FULL     1  /* rr_build_ld_table builds the whole T[npv][npb][nk][ng]            */
+#define RR_TABLE_DIRECT   2  /* the paper's direct model: no k grid; at
+                                rr_evaluate the weights are computed at each pv's own k and contracted
+                                with its profile (g interpolation only); any k > 0 is valid        */
 
 /* supersample reduction layout of the fused flux kernel (rr_set_reduction) */
 #define RR_REDUCE_AUTO    0  /* library picks per light curve from ns and the amount of work    */
@@ -130,7 +133,7 @@ int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, i
  * Both give the same flux to rounding (tested).  Buffers are owned by ctx and grown as needed.   */
 int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64_t npv,
                       void *stream);
-/* RR_TABLE_*; takes effect at the next rr_build_ld_table.                                        */
+/* RR_TABLE_*; takes effect at the next rr_build_ld_table.  RR_TABLE_DIRECT needs nz <= 2000.     */
 int rr_set_table_mode(rr_ctx *ctx, int32_t mode);
 /* Diagnostics: device pointers to the full table (built on demand in lazy mode; synchronous) and
  * Istar of the last rr_build_ld_table (ctx precision), or NULL.                                 */
@@ -139,6 +142,9 @@ const void *rr_istar_ptr(const rr_ctx *ctx);
 /* Copies the full table T[npv][npb][nk][ng] (built on demand in lazy mode) and Istar[npv][npb] to
  * host arrays (ctx precision; either may be NULL).  Synchronous (device-wide).                   */
 int rr_get_table(rr_ctx *ctx, void *h_T, void *h_istar);
+/* Diagnostics (lazy / direct mode, after an rr_evaluate): the collapsed rows ldw[npv][npb][ng] the
+ * flux kernel staged (ctx precision) -> host array.  Synchronous (device-wide).                  */
+int rr_get_rows(const rr_ctx *ctx, void *h_rows);
 
 /* ---- kernels 2+3+4: evaluate, PAPER.md:101-107, :128-131, :214, :220 ---------------------------
  * d_pv[npv][npar]   fp64 rows [k_0..k_{nkpb-1}, t0, p, a, i, e, w], npar = nkpb + 6: the order of

@@ -61,6 +61,14 @@ def load():
                                     C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32,
                                     _D, _I, _D, C.c_int32]
     lib.oracle_evaluate.restype = None
+    lib.oracle_direct_rows.argtypes = [_D, C.c_int, C.c_int, _D, _D, C.c_int64, _D]
+    lib.oracle_direct_rows.restype = None
+    lib.oracle_flux_from_row.argtypes = [C.c_double, C.c_double, _D, C.c_int, C.c_double]
+    lib.oracle_flux_from_row.restype = C.c_double
+    lib.oracle_evaluate_direct.argtypes = [_D, _I, C.c_int64, _I, _I, _D, _D, C.c_int32,
+                                           C.c_int64, _D, _D, C.c_int32, C.c_int32, _D, _I,
+                                           C.c_int32]
+    lib.oracle_evaluate_direct.restype = None
     _lib = lib
     return lib
 
@@ -178,6 +186,56 @@ class OracleModel:
                                self.npb, self.nk, self.k0, self.k1, self.ng,
                                _dp(flux), _ip(status), _dp(z) if want_z else None, int(nthreads))
         return (flux, status, z) if want_z else (flux, status)
+
+
+class OracleDirectModel:
+    """Direct RoadRunner model: weights at each pv's own k, g interpolation
+    only.  Marshalling only; the arithmetic is oracle_direct_rows / oracle_evaluate_direct."""
+
+    def __init__(self, nzin=50, nzlimb=50, zcut=0.7, ng=100, npb=1, nkpb=1):
+        self.nzin, self.nzlimb, self.zcut = int(nzin), int(nzlimb), float(zcut)
+        self.ng, self.npb, self.nkpb = int(ng), int(npb), int(nkpb)
+        self.nz = self.nzin + self.nzlimb
+        self.ze, self.zm, self.mu = z_grid(self.zcut, self.nzin, self.nzlimb)
+
+    @classmethod
+    def from_config(cls, m):
+        return cls(m.nzin, m.nzlimb, m.zcut, m.ng, m.npb, m.nkpb)
+
+    def rows(self, ldp, pv):
+        """ldw[npv][npb][ng] and Istar[npv][npb] for the k of every (pv, passband)."""
+        ldp = _f64(ldp).reshape(-1, self.npb, self.nz)
+        pv = _f64(pv).reshape(-1, self.nkpb + 6)
+        npv = ldp.shape[0]
+        kcol = [0] * self.npb if self.nkpb == 1 else list(range(self.npb))
+        k = _f64(pv[:, kcol])                                   # [npv][npb]
+        out = np.empty((npv, self.npb, self.ng))
+        load().oracle_direct_rows(_dp(self.ze), self.nz, self.ng, _dp(k), _dp(ldp),
+                                  npv * self.npb, _dp(out))
+        return out, istar(self.ze, ldp)
+
+    def evaluate(self, times, lc_index, passband_index, supersampling, exposure_time, pv, ldp,
+                 nthreads=1):
+        times, pv = _f64(times), _f64(pv).reshape(-1, self.nkpb + 6)
+        lc_index, passband_index = _i32(lc_index), _i32(passband_index)
+        supersampling, exposure_time = _i32(supersampling), _f64(exposure_time)
+        ok = np.all(np.isfinite(pv[:, :self.nkpb]) & (pv[:, :self.nkpb] > 0), axis=1)
+        safe = pv.copy()
+        safe[~ok, :self.nkpb] = 0.1                              # rows of invalid pvs are not used
+        rows, ist = self.rows(ldp, safe)
+        npv, npt = pv.shape[0], times.size
+        flux = np.empty((npv, npt))
+        status = np.empty(npv, np.int32)
+        load().oracle_evaluate_direct(_dp(times), _ip(lc_index), npt, _ip(passband_index),
+                                      _ip(supersampling), _dp(exposure_time), _dp(pv), self.nkpb,
+                                      npv, _dp(rows), _dp(ist), self.npb, self.ng, _dp(flux),
+                                      _ip(status), int(nthreads))
+        return flux, status
+
+
+def flux_from_row(z, k, ldw, istar_value):
+    ldw = _f64(ldw)
+    return load().oracle_flux_from_row(float(z), float(k), _dp(ldw), ldw.size, float(istar_value))
 
 
 def evaluate_workload(wl, nthreads=1, want_z=False):

@@ -290,3 +290,82 @@ void oracle_evaluate(const double *times, const int32_t *lc_index, int64_t npt,
         }
     }
 }
+
+/* ==== direct model ==========================================
+ * The paper's default: no k grid.  Per (pv, passband) the weights are computed at the pv's own k,
+ * `dg, w = calculate_weights(k, ze, ng)`, and `ldw = dot(w, ldp)`; per point only
+ * the g interpolation of PAPER.md:101-105 remains.  Same g nodes and g = 1 limit (R5) as the table
+ * model; any k > 0 is valid. */
+void oracle_direct_rows(const double *ze, int nz, int ng, const double *k /*[nrows]*/,
+                        const double *ldp /*[nrows][nz]*/, int64_t nrows, double *rows /*[nrows][ng]*/)
+{
+    double dg = 1.0 / (double)(ng - 1);
+    double *w = (double *)malloc(sizeof(double) * (size_t)nz);
+    for (int64_t r = 0; r < nrows; ++r)
+        for (int ig = 0; ig < ng; ++ig) {
+            double g = (ig == ng - 1) ? 1.0 : ig * dg;
+            oracle_weights(g * (1.0 + k[r]), k[r], ze, nz, w);
+            double s = 0.0;
+            for (int j = 0; j < nz; ++j) s += w[j] * ldp[r * nz + j];
+            rows[r * ng + ig] = s;                      /* ldw = dot(w, ldp) */
+        }
+    free(w);
+}
+
+/* One sub-sample's flux from a direct-model row (reading R10 for the last cell). */
+double oracle_flux_from_row(double z, double k, const double *ldw /*[ng]*/, int ng, double istar)
+{
+    if (z >= 1.0 + k) return 1.0;
+    double dg = 1.0 / (double)(ng - 1);
+    double y = (z / (1.0 + k)) / dg;
+    int ig = (int)floor(y);
+    if (ig > ng - 2) ig = ng - 2;
+    double ag = y - ig;
+    double ip = (1.0 - ag) * ldw[ig] + ag * ldw[ig + 1];
+    double ap = oracle_lens_area(1.0, k, z);
+    return (istar - ip * ap) / istar;
+}
+
+/* The whole direct-model evaluation: as oracle_evaluate, with rows[npv][npb][ng] from
+ * oracle_direct_rows in place of the table, and k > 0 the only limit on k (status bit 0). */
+void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_t npt,
+                            const int32_t *passband_index, const int32_t *supersampling,
+                            const double *exposure_time, const double *pv, int32_t nkpb,
+                            int64_t npv, const double *rows, const double *istar, int32_t npb,
+                            int32_t ng, double *flux, int32_t *status, int32_t nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t v = 0; v < npv; ++v) {
+        const double *row = pv + v * (nkpb + 6);
+        const double *o = row + nkpb;
+        double t0 = o[0], p = o[1], a = o[2], inc = o[3], e = o[4], w = o[5];
+        int st = oracle_pv_status(row, nkpb, 1e-300, 1e300);
+        if (status) status[v] = st;
+        if (st) {
+            for (int64_t i = 0; i < npt; ++i) flux[v * npt + i] = NAN;
+            continue;
+        }
+        for (int64_t i = 0; i < npt; ++i) {
+            int l = lc_index[i];
+            int pb = passband_index[l];
+            int ns = supersampling[l];
+            double tau = exposure_time[l];
+            double k = row[nkpb == 1 ? 0 : pb];
+            const double *ldw = rows + ((size_t)v * npb + pb) * (size_t)ng;
+            double is = istar[v * npb + pb];
+            double sum = 0.0;
+            for (int s = 0; s < ns; ++s) {
+                double t = times[i] + tau * ((s + 0.5) / (double)ns - 0.5);
+                int front;
+                double z = oracle_separation(t, t0, p, a, inc, e, w, &front);
+                sum += front ? oracle_flux_from_row(z, k, ldw, ng, is) : 1.0;
+            }
+            flux[v * npt + i] = sum / (double)ns;
+        }
+    }
+}

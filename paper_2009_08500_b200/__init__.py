@@ -22,7 +22,7 @@ from . import build as _build
 
 RR_FP64, RR_FP32 = 0, 1
 RR_REDUCE_AUTO, RR_REDUCE_THREAD, RR_REDUCE_SHUFFLE = 0, 1, 2
-RR_TABLE_LAZY, RR_TABLE_FULL = 0, 1
+RR_TABLE_LAZY, RR_TABLE_FULL, RR_TABLE_DIRECT = 0, 1, 2
 RR_PV_K_RANGE, RR_PV_E_RANGE, RR_PV_A_RANGE, RR_PV_P_RANGE, RR_PV_NONFINITE = 1, 2, 4, 8, 16
 
 # every symbol include/roadrunner.h declares (tests check the library exports each of them)
@@ -33,7 +33,7 @@ SYMBOLS = (
     "rr_evaluate_flat", "rr_orbit_z", "rr_num_subsamples", "rr_num_tiles", "rr_get_tiles",
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
-    "rr_get_kernel_times",
+    "rr_get_kernel_times", "rr_get_rows",
 )
 
 
@@ -93,6 +93,7 @@ def load() -> C.CDLL:
         "rr_launch_count": (_I64, [_VP]),
         "rr_measure_fma_peak": (C.c_int, [_I32, C.POINTER(_DBL), _VP]),
         "rr_set_table_mode": (C.c_int, [_VP, _I32]),
+        "rr_get_rows": (C.c_int, [_VP, _VP]),
         "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
         "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
@@ -355,6 +356,13 @@ class RoadRunner:
         I = np.empty((self.npv, self.npb), npdt)
         _check(load().rr_get_table(self.ctx, T.ctypes.data, I.ctypes.data), "rr_get_table")
         return T, I
+
+    def rows(self):
+        """Copy of the collapsed rows ldw[npv][npb][ng] of the last evaluate (lazy / direct mode)."""
+        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        out = np.empty((self.npv, self.npb, self.ng), npdt)
+        _check(load().rr_get_rows(self.ctx, out.ctypes.data), "rr_get_rows")
+        return out
 
     def evaluate(self, pv, want_status=False):
         """pv: CUDA tensor or array [npv][nkpb+6] -> flux CUDA tensor [npv][npt]."""

@@ -47,7 +47,7 @@ int tile_len_for(int ns) {
 }
 
 // The lazy row builder keeps one profile (nz doubles) in shared memory.
-bool lazy_ok(const rr_ctx *ctx) { return ctx->table_mode == RR_TABLE_LAZY && ctx->nz <= 4096; }
+bool lazy_ok(const rr_ctx *ctx) { return ctx->table_mode != RR_TABLE_FULL && ctx->nz <= 2000; }
 
 int grow(void **p, int64_t *cap, int64_t need) {
   if (need <= *cap) return RR_OK;
@@ -224,7 +224,8 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
 
 int rr_set_table_mode(rr_ctx *ctx, int32_t mode) {
   if (!ctx) return RR_ENULL;
-  if (mode != RR_TABLE_LAZY && mode != RR_TABLE_FULL) return RR_ECONFIG;
+  if (mode != RR_TABLE_LAZY && mode != RR_TABLE_FULL && mode != RR_TABLE_DIRECT) return RR_ECONFIG;
+  if (mode == RR_TABLE_DIRECT && ctx->nz > 2000) return RR_ECONFIG;
   ctx->table_mode = mode;
   return RR_OK;
 }
@@ -254,6 +255,16 @@ int rr_get_table(rr_ctx *ctx, void *h_T, void *h_istar) {
   if (h_T)
     RR_CUDA(cudaMemcpy(h_T, w.T, rows * ctx->cfg.nk * ctx->cfg.ng * es, cudaMemcpyDeviceToHost));
   if (h_istar) RR_CUDA(cudaMemcpy(h_istar, w.istar, rows * es, cudaMemcpyDeviceToHost));
+  return RR_OK;
+}
+
+int rr_get_rows(const rr_ctx *ctx, void *h_rows) {
+  if (!ctx || !h_rows) return RR_ENULL;
+  const RRWork &w = ctx->work[0];
+  if (w.table_npv <= 0 || !w.lazy || !w.rows) return RR_ESTATE;
+  RR_CUDA(cudaDeviceSynchronize());
+  RR_CUDA(cudaMemcpy(h_rows, w.rows, (size_t)w.table_npv * ctx->cfg.npb * ctx->cfg.ng * esize(ctx),
+                     cudaMemcpyDeviceToHost));
   return RR_OK;
 }
 

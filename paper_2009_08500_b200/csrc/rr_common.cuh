@@ -77,7 +77,7 @@ struct RRWork {
   int64_t rows_cap;
   int32_t *bk;              // row buckets by ik: hist[nk] | cursor[nk] | offs[nk+1] | tileoff[nk+1] | list[M]
   int64_t bk_cap;
-  int32_t lazy;             // 1: evaluate from rows; 0: evaluate from T
+  int32_t lazy;             // 0: evaluate from T; 1: from lazy rows; 2: from direct-model rows
   int32_t have_full;        // T holds the full table of the current profile
   RRPvOrbit *pvo;
   RRPvBand *pvb;
@@ -147,6 +147,7 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
                          int64_t npv, int copy, cudaStream_t st);              // rr_ld_table.cu
 int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_ld_table.cu
 int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st);         // rr_ld_table.cu
+int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_geometry.cu
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
                       int32_t *d_status, cudaStream_t st);                     // rr_flux.cu

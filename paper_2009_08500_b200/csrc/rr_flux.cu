@@ -46,7 +46,8 @@ constexpr double RR_TRIG_SMALL = 0.5;
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
 __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, int nkpb, int nk,
-                                  double k0, double k1, int ng, int fp32,
+                                  double k0, double k1, double kmin, double kmax_ok, int ng,
+                                  int fp32,
                                   RRPvOrbit *__restrict__ pvo, RRPvBand *__restrict__ pvb,
                                   int32_t *__restrict__ status_out) {
   int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -60,7 +61,7 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     if (!isfinite(row[q])) st |= RR_PV_NONFINITE;
   if (!st) {
     for (int q = 0; q < nkpb; ++q)
-      if (row[q] < k0 || row[q] > k1) st |= RR_PV_K_RANGE;
+      if (row[q] < kmin || row[q] > kmax_ok) st |= RR_PV_K_RANGE;
     if (e < 0.0 || e >= 1.0) st |= RR_PV_E_RANGE;
     if (a <= 0.0) st |= RR_PV_A_RANGE;
     if (p <= 0.0) st |= RR_PV_P_RANGE;
@@ -850,9 +851,11 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
     }
     wk->pv_cap = npv;
   }
+  // direct model (no k grid): any k > 0 is valid
+  const bool direct = wk->lazy == 2;
   rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
-      d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, c.ng, c.precision == RR_FP32, wk->pvo, wk->pvb,
-      d_status);
+      d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, direct ? 1e-300 : c.k0, direct ? 1e300 : c.k1, c.ng,
+      c.precision == RR_FP32, wk->pvo, wk->pvb, d_status);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }

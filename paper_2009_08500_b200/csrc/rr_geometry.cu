@@ -72,6 +72,67 @@ __global__ void rr_weights_kernel(int nk, double k0, double k1, int ng, int nz,
   W[idx] = w;
 }
 
+// ---- direct model on the device -------------------------------
+// The paper's default setting: no k grid.  For every (pv, passband) row the weights are computed at
+// the pv's OWN k, `dg, w = calculate_weights(k, ze, ng)`, and contracted at once with the profile,
+// `ldw = dot(w, ldp)`:
+//   ldw[ig] = sum_j [A(ze[j+1]) - A(ze[j])] ldp[j] / a(c,k),   c = g_ig (1+k),  A(r) = lens(r, k, c)
+//           = sum_{e=1..nz} A(ze[e]) D_e / a(c,k),   D_e = ldp[e-1] - ldp[e] (e < nz), D_nz = ldp[nz-1]
+// (summation by parts: one lens area per annulus EDGE, no neighbour exchange).  ig = ng-1 takes the
+// limit of reading R5.  One block per row, one warp per g node, lanes over edges; fp64 throughout.
+// The result has the layout of the lazy rows, so the flux kernel is unchanged; there is no k
+// interpolation error and no [k0, k1] limit.
+template <typename TR>
+__global__ void __launch_bounds__(256)
+rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ ze,
+                         const RRPvBand *__restrict__ pvb, TR *__restrict__ rows, int npb, int nkpb,
+                         int ng, int nz) {
+  extern __shared__ double sh[];                 // D[nz+1] (index = edge) | ze[nz+1]
+  double *D = sh, *zes = sh + nz + 1;
+  const int64_t row = blockIdx.x;
+  const int64_t v = row / npb;
+  const int pb = (int)(row - v * npb);
+  const double k = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].k;
+  const TR *pr = ldp + row * nz;
+  for (int e = threadIdx.x; e <= nz; e += 256) {
+    zes[e] = ze[e];
+    D[e] = (e == 0) ? 0.0 : (e < nz ? (double)pr[e - 1] - (double)pr[e] : (double)pr[nz - 1]);
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int ig = warp; ig < ng; ig += 8) {
+    double out;
+    if (ig == ng - 1) {
+      out = (double)pr[nz - 1];                  // reading R5: all weight in the outermost annulus
+    } else {
+      const double c = ((double)ig / (double)(ng - 1)) * (1.0 + k);
+      double s = 0.0;
+      for (int e = 1 + lane; e <= nz; e += 32) s = fma(rr_lens_area(zes[e], k, c), D[e], s);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      out = s / rr_lens_area(1.0, k, c);
+    }
+    if (lane == 0) rows[row * ng + ig] = (TR)out;
+  }
+}
+
+int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t M = npv * c.npb;
+  if (M > 0x7fffffffLL) return RR_ESIZE;
+  const size_t smem = sizeof(double) * 2 * (ctx->nz + 1);
+  if (c.precision == RR_FP32)
+    rr_ld_rows_direct_kernel<float><<<(unsigned)M, 256, smem, st>>>(
+        (const float *)wk->ldp_src, ctx->d_ze, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
+        ctx->nz);
+  else
+    rr_ld_rows_direct_kernel<double><<<(unsigned)M, 256, smem, st>>>(
+        (const double *)wk->ldp_src, ctx->d_ze, wk->pvb, (double *)wk->rows, c.npb, c.nkpb, c.ng,
+        ctx->nz);
+  RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
 int rr_geometry_build(rr_ctx *ctx) {
   const rr_config &c = ctx->cfg;
   int nz = ctx->nz;

@@ -350,7 +350,7 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
         (const double *)d_ldp, ctx->d_q, (const double *)d_istar, (double *)wk->istar, M, ctx->nz);
   RR_LAUNCH_CHECK(ctx);
   wk->table_npv = npv;
-  wk->lazy = 1;
+  wk->lazy = ctx->table_mode == RR_TABLE_DIRECT ? 2 : 1;
   wk->have_full = 0;
   return RR_OK;
 }
@@ -363,6 +363,7 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
   if (M > 0x7fffffffLL) return RR_ESIZE;
   int rc = grow_buf(&wk->rows, &wk->rows_cap, M * c.ng * esz);
   if (rc != RR_OK) return rc;
+  if (wk->lazy == 2) return rr_ld_rows_direct_launch(ctx, wk, npv, st);
   const int nb = c.nk - 1;                         // buckets: lower k row ik in [0, nk-2]
   const int stride = ctx->nz | 1;
   const size_t smem_b = sizeof(double) * RB * stride;

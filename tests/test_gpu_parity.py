@@ -173,6 +173,53 @@ def test_table_modes_agree(rr, config, precision, shape):
     assert np.max(np.abs(out[rr.RR_TABLE_LAZY] - out[rr.RR_TABLE_FULL])) <= (2e-7 if precision else 1e-14)
 
 
+# ---- direct model on the device (NEXT-1) ---------------------------------------------------------------
+def _direct_gpu(rr, wl, precision, pv=None):
+    gm = rr.RoadRunner.from_config(wl.model, precision)
+    rr.rr_set_table_mode(gm.ctx, rr.RR_TABLE_DIRECT)
+    gm.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    flux, status = gm.evaluate(wl.pv if pv is None else pv, want_status=True)
+    rows = gm.rows().astype(np.float64)
+    out = flux.cpu().numpy().astype(np.float64), status.cpu().numpy(), rows
+    gm.close()
+    return out
+
+
+@pytest.mark.parametrize("config,precision", [(1, 0), (2, 0), (3, 0), (4, 0), (3, 1), (4, 1)])
+def test_direct_model_matches_oracle(rr, config, precision):
+    """RR_TABLE_DIRECT: rows = weights at the pv's own k contracted with the
+    profile, then the same flux kernel; against the oracle's direct model."""
+    wl = small_workload(config)
+    om = oracle.OracleDirectModel.from_config(wl.model)
+    rows_o, _ = om.rows(wl.ldp(om.mu), wl.pv)
+    want, st_o = om.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                             wl.exposure_time, wl.pv, wl.ldp(om.mu), nthreads=0)
+    got, st_g, rows_g = _direct_gpu(rr, wl, precision)
+    assert np.array_equal(st_g, st_o)
+    assert np.max(np.abs(rows_g - rows_o)) <= (2e-7 if precision else 1e-12)
+    assert np.max(np.abs(got - want)) <= (TOL32 if precision else TOL64)
+    assert (want < 1.0).sum() > 100
+
+
+def test_direct_model_has_no_k_limits(rr):
+    wl = workloads.make_workload(1, npv=6, npt=1500)
+    pv = wl.pv.copy()
+    pv[0, 0] = 0.45            # far above the table's k1: valid in the direct model
+    pv[1, 0] = 0.004           # below k0: valid
+    pv[2, 0] = -0.1            # k <= 0: invalid
+    pv[3, 0] = np.nan
+    om = oracle.OracleDirectModel.from_config(wl.model)
+    want, st_o = om.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                             wl.exposure_time, pv, wl.ldp(om.mu))
+    got, st_g, _ = _direct_gpu(rr, wl, 0, pv=pv)
+    assert np.array_equal(st_g, st_o) and list(st_g[:4]) == [0, 0, 1, 16]
+    assert np.array_equal(np.isnan(got), np.isnan(want))
+    ok = ~np.isnan(want)
+    assert np.max(np.abs(got[ok] - want[ok])) <= TOL64
+    assert want[0].min() < 0.85
+
+
 def test_kernel_timing_counts_calls(rr):
     wl = small_workload(1)
     gm = gpu_model(rr, wl)

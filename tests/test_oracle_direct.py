@@ -1,0 +1,90 @@
+"""Pins for the oracle's DIRECT model: weights at the pv's own
+k, g interpolation only.  CPU only."""
+import math
+
+import numpy as np
+
+import oracle
+import workloads
+from oracle import truth
+
+
+def test_direct_row_on_g_nodes_equals_l1():
+    """At z = g_ig (1+k) the interpolation weight is 0: flux from the row is Eq. (5) with the weight
+    vector at exactly that (c, k) - the L1 function, which is pinned against Eq. (2)."""
+    m = oracle.OracleDirectModel()
+    ld = truth.quadratic(0.4, 0.2)(m.mu)
+    for k in (0.013, 0.1, 0.27, 0.5):
+        pv = np.array([[k, 0, 3, 8, 1.5, 0, 0]])
+        rows, ist = m.rows(ld, pv)
+        for ig in range(0, m.ng - 1, 7):
+            c = ig / (m.ng - 1) * (1 + k)
+            assert abs(oracle.flux_from_row(c, k, rows[0, 0], ist[0, 0])
+                       - oracle.direct_flux(k, c, m.ze, ld, ist[0, 0])) < 1e-15
+
+
+def test_direct_uniform_disc_exact():
+    """ldp = 1: every weight vector sums to 1, the row is 1, flux = 1 - a(z,k)/pi."""
+    m = oracle.OracleDirectModel()
+    ld = np.ones(m.nz)
+    for k in (0.05, 0.3):
+        rows, ist = m.rows(ld, np.array([[k, 0, 3, 8, 1.5, 0, 0]]))
+        assert np.max(np.abs(rows - 1.0)) < 1e-13
+        assert ist[0, 0] == np.pi or abs(ist[0, 0] - math.pi) < 1e-15
+        for z in np.linspace(0, 1 + k, 23):
+            want = 1 - oracle.lens_area(1.0, k, z) / math.pi
+            assert abs(oracle.flux_from_row(z, k, rows[0, 0], ist[0, 0]) - want) < 1e-14
+
+
+def test_direct_last_node_is_limb_sample_and_rows_are_dot_products():
+    m = oracle.OracleDirectModel(nzin=7, nzlimb=5, ng=11)
+    rng = np.random.default_rng(2)
+    ld = rng.uniform(0.2, 1.0, m.nz)
+    k = 0.17
+    rows, _ = m.rows(ld, np.array([[k, 0, 3, 8, 1.5, 0, 0]]))
+    assert rows[0, 0, -1] == ld[-1]                               # reading R5
+    for ig in range(m.ng - 1):
+        w = oracle.weights(ig / (m.ng - 1) * (1 + k), k, m.ze)
+        assert abs(rows[0, 0, ig] - float(np.dot(w, ld))) < 1e-15
+
+
+def test_direct_is_closer_to_l0_than_the_interpolated_model():
+    """No k interpolation: 'small reduction in accuracy' of the interpolated model
+    read the other way round.  Both against Eq. (2) by 20-digit quadrature."""
+    ldf = truth.quadratic(0.4, 0.2)
+    md, mi = oracle.OracleDirectModel(), oracle.OracleModel()
+    lib = oracle.load()
+    k = 0.1037                                                     # between two k nodes
+    rows, ist = md.rows(ldf(md.mu), np.array([[k, 0, 3, 8, 1.5, 0, 0]]))
+    T, ist2 = mi.build_ld_table(ldf(mi.mu)[None, None, :])
+    ed, ei = [], []
+    for z in np.linspace(0, 1 + k, 31):
+        want = float(truth.flux_radial_mp(k, z, ldf, dps=20))
+        ed.append(abs(oracle.flux_from_row(z, k, rows[0, 0], ist[0, 0]) - want))
+        ei.append(abs(lib.oracle_flux_from_table(z, k, T.ctypes.data_as(oracle._D), mi.nk, mi.k0,
+                                                 mi.k1, mi.ng, ist2[0, 0]) - want))
+    assert max(ed) < 12e-6 and np.mean(ed) < 1.5e-6
+    assert np.mean(ed) <= np.mean(ei) * 1.05
+
+
+def test_direct_evaluate_equals_table_model_on_a_k_node_and_allows_any_k():
+    """On a k node of the table the interpolated model has ak = 0: both models use the same weight
+    vectors, so whole light curves agree to rounding; k outside the table's range is fine."""
+    wl = workloads.make_workload(3, npv=4, npt=6 * 50)
+    mi = oracle.OracleModel.from_config(wl.model)
+    dk = (mi.k1 - mi.k0) / (mi.nk - 1)
+    wl.pv[:, 0] = mi.k0 + dk * np.array([3, 17, 30, 48])
+    mi.build_ld_table(wl.ldp(mi.mu))
+    want, _ = mi.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                          wl.exposure_time, wl.pv)
+    md = oracle.OracleDirectModel.from_config(wl.model)
+    got, st = md.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                          wl.exposure_time, wl.pv, wl.ldp(md.mu))
+    assert np.all(st == 0) and np.max(np.abs(got - want)) < 1e-13 and (want < 1).sum() > 50
+    pv = wl.pv.copy()
+    pv[0, 0] = 0.45                    # above the table's k1 = 0.2
+    pv[1, 0] = -0.1                    # invalid
+    got, st = md.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                          wl.exposure_time, pv, wl.ldp(md.mu))
+    assert list(st) == [0, 1, 0, 0] and np.all(np.isnan(got[1])) and np.all(np.isfinite(got[0]))
+    assert got[0].min() < 0.9          # a k = 0.45 transit is deep
