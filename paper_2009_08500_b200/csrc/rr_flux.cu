@@ -22,6 +22,7 @@
 #include <algorithm>
 
 #include "rr_common.cuh"
+#include "rr_math.cuh"
 
 namespace {
 
@@ -32,17 +33,6 @@ constexpr int FT = 256;   // threads per flux block
 #ifndef RR_FLUX_WAVES
 #define RR_FLUX_WAVES 32        // waves of blocks wanted before the tile axis is left uncut
 #endif
-
-// Taylor coefficients: sin x = x + x^3 (S0 + S1 x^2 + ...), cos x - 1 = x^2 (C0 + C1 x^2 + ...).
-// Truncation on |x| <= 0.5: fp64 sin 0.5^14/15! = 5e-17 relative, cos-1 2 0.5^14/16! = 6e-18;
-// fp32 0.5^8/9! = 1e-8.
-__constant__ double RR_SIN_D[6] = {-1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0,
-                                   -1.0 / 39916800.0, 1.0 / 6227020800.0};
-__constant__ double RR_COS_D[7] = {-1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0,
-                                   -1.0 / 3628800.0, 1.0 / 479001600.0, -1.0 / 87178291200.0};
-__constant__ float RR_SIN_F[3] = {-1.0f / 6.0f, 1.0f / 120.0f, -1.0f / 5040.0f};
-__constant__ float RR_COS_F[4] = {-1.0f / 2.0f, 1.0f / 24.0f, -1.0f / 720.0f, 1.0f / 40320.0f};
-constexpr double RR_TRIG_SMALL = 0.5;
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
 __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, int nkpb, int nk,
@@ -163,114 +153,6 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   po.u_mid = 0.5 * (u_lo + u_hi);
   po.hwid = 0.5 * (u_hi - u_lo);
   pvo[v] = po;
-}
-
-// ---- working-precision math ------------------------------------------------------------------------
-__device__ __forceinline__ void rr_sincos(double x, double *s, double *c) { sincos(x, s, c); }
-__device__ __forceinline__ void rr_sincos(float x, float *s, float *c) { sincosf(x, s, c); }
-__device__ __forceinline__ double rr_sinpi(double x) { return sinpi(x); }
-__device__ __forceinline__ float rr_sinpi(float x) { return sinpif(x); }
-__device__ __forceinline__ float rr_atan2_pos(float y, float x) { return atan2f(y, x); }
-// sqrt(x): hardware reciprocal-square-root seed (~2^-20), two Goldschmidt steps (g -> sqrt x,
-// h -> 1/(2 sqrt x)) and a final residual correction; <= 1 ulp.  rr_sqrt: any x, 0 for x <= 0
-// (a product of rounded factors that should be >= 0); rr_sqrt_pos: x >= 0, adds 1e-300 so that the
-// seed of x = 0 is finite (no effect on any other x).
-__device__ __forceinline__ double rr_sqrt_core(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double g = x * y, h = 0.5 * y;
-  double r = fma(-h, g, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
-  r = fma(-h, g, 0.5);
-  g = fma(g, r, g);
-  h = fma(h, r, h);
-  return fma(fma(-g, g, x), h, g);
-}
-__device__ __forceinline__ double rr_sqrt(double x) {
-  const double g = rr_sqrt_core(x);
-  return x > 0.0 ? g : 0.0;
-}
-__device__ __forceinline__ double rr_sqrt_pos(double x) { return rr_sqrt_core(x + 1e-300); }
-__device__ __forceinline__ float rr_sqrt_pos(float x) { return sqrtf(x); }
-__device__ __forceinline__ float rr_sqrt(float x) { return sqrtf(fmaxf(x, 0.0f)); }
-// 1/x to ~1e-12 (fp64: hardware seed + one Newton step) / ~1e-7 (fp32).  x normal, non-zero.
-__device__ __forceinline__ double rr_rcp(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  return fma(fma(-x, r, 1.0), r, r);
-}
-__device__ __forceinline__ float rr_rcp(float x) { return __frcp_rn(x); }
-
-// atan2(y, x) for y >= 0, (x, y) != (0, 0): the angle in [0, pi].  Octant reduction
-// t = min/max of (|x|, y), then a turn by pi/4 when t > tan(pi/8) so that |t| <= tan(pi/8); one
-// division (hardware seed, Newton step, residual correction: correctly rounded to ~1 ulp);
-// atan t = t + t u Q(u), u = t^2, Q = degree-10 interpolant at the Chebyshev nodes of
-// [0, tan^2(pi/8)] (max error 6e-17 against 60-digit arithmetic, profiles/ note r01b).
-__constant__ double RR_ATAN_D[11] = {
-    -3.33333333333331205e-01, 1.99999999999408928e-01,  -1.42857142792502445e-01,
-    1.11111107449196583e-01,  -9.09089680906402658e-02, 7.69204533090222520e-02,
-    -6.66295181362919070e-02, 5.84687829733087222e-02,  -5.03510245660155203e-02,
-    3.79652574538659332e-02,  -1.78053972054194459e-02};
-__device__ __forceinline__ double rr_atan2_pos(double y, double x) {
-  const double ax = fabs(x);
-  const bool swap = y > ax;
-  const double mx = swap ? y : ax, mn = swap ? ax : y;
-  const bool red = mn > 0.41421356237309503 * mx;
-  const double num = red ? mn - mx : mn;
-  const double den = red ? mn + mx : mx;
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
-  r = fma(fma(-den, r, 1.0), r, r);
-  double t = num * r;
-  t = fma(fma(-den, t, num), r, t);
-  const double u = t * t;
-  // Q(u) = Qe(u^2) + u Qo(u^2): two half-length Horner chains in flight
-  const double u2 = u * u;
-  double qe = RR_ATAN_D[10], qo = RR_ATAN_D[9];
-#pragma unroll
-  for (int i = 8; i >= 2; i -= 2) {
-    qe = fma(qe, u2, RR_ATAN_D[i]);
-    qo = fma(qo, u2, RR_ATAN_D[i - 1]);
-  }
-  qe = fma(qe, u2, RR_ATAN_D[0]);
-  const double q = fma(qo, u, qe);
-  const double base = fma(t * u, q, t) + (red ? 0.78539816339744831 : 0.0);
-  const bool neg = x < 0.0;
-  const double off = swap ? 1.5707963267948966 : (neg ? 3.1415926535897932 : 0.0);
-  return fma((swap != neg) ? -1.0 : 1.0, base, off);
-}
-
-// Nearest integer of |x| < 2^51 as a double (two adds, no conversion instruction).
-__device__ __forceinline__ double rr_round(double x) {
-  const double M = 6755399441055744.0;   // 2^52 + 2^51
-  return __dadd_rn(__dadd_rn(x, M), -M);
-}
-
-// sin x and cos x - 1 on |x| <= RR_TRIG_SMALL.
-__device__ __forceinline__ void rr_sincosm1_small(double x, double &s, double &cm1) {
-  const double x2 = x * x;
-  double ps = RR_SIN_D[5], pc = RR_COS_D[6];
-  pc = fma(pc, x2, RR_COS_D[5]);
-#pragma unroll
-  for (int i = 4; i >= 0; --i) {
-    ps = fma(ps, x2, RR_SIN_D[i]);
-    pc = fma(pc, x2, RR_COS_D[i]);
-  }
-  s = fma(x * x2, ps, x);
-  cm1 = x2 * pc;
-}
-__device__ __forceinline__ void rr_sincosm1_small(float x, float &s, float &cm1) {
-  const float x2 = x * x;
-  float ps = RR_SIN_F[2], pc = RR_COS_F[3];
-  pc = fmaf(pc, x2, RR_COS_F[2]);
-#pragma unroll
-  for (int i = 1; i >= 0; --i) {
-    ps = fmaf(ps, x2, RR_SIN_F[i]);
-    pc = fmaf(pc, x2, RR_COS_F[i]);
-  }
-  s = fmaf(x * x2, ps, x);
-  cm1 = x2 * pc;
 }
 
 // ---- per-(tile, pv) constants, staged in shared memory in the working precision -----------------------

@@ -7,6 +7,7 @@
 //             c = g (1+k).  Reading R5: the g = 1 node (a = 0) takes the limit, all weight in the
 //             outermost annulus.
 #include "rr_common.cuh"
+#include "rr_math.cuh"
 
 // Area common to two discs of radii r1, r2 with centres d apart (textbook lens; PAPER.md:57, :69
 // "cheap to calculate analytically").  Partial overlap = two circular sectors minus the kite;
@@ -72,6 +73,17 @@ __global__ void rr_weights_kernel(int nk, double k0, double k1, int ng, int nz,
   W[idx] = w;
 }
 
+// The same area for the direct-model rows (evaluate-time path): the hot path's own sqrt and atan2.
+__device__ __forceinline__ double rr_lens_area_fast(double r1, double r2, double d) {
+  if (d >= r1 + r2) return 0.0;
+  const double rmin = fmin(r1, r2);
+  if (d <= fabs(r1 - r2)) return RR_PI * rmin * rmin;
+  const double kite = rr_sqrt((r1 + r2 - d) * (d + r1 - r2) * (d - r1 + r2) * (d + r1 + r2));
+  const double th1 = rr_atan2_pos(kite, fma(d - r2, d + r2, r1 * r1));
+  const double th2 = rr_atan2_pos(kite, fma(d - r1, d + r1, r2 * r2));
+  return fma(r1 * r1, th1, fma(r2 * r2, th2, -0.5 * kite));
+}
+
 // ---- direct model on the device -------------------------------
 // The paper's default setting: no k grid.  For every (pv, passband) row the weights are computed at
 // the pv's OWN k, `dg, w = calculate_weights(k, ze, ng)`, and contracted at once with the profile,
@@ -106,11 +118,25 @@ rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
       out = (double)pr[nz - 1];                  // reading R5: all weight in the outermost annulus
     } else {
       const double c = ((double)ig / (double)(ng - 1)) * (1.0 + k);
+      // edges are sorted: ze[e] <= c-k have A = 0; ze[e] >= c+k have A = pi k^2 and their D_e
+      // telescope to ldp[e_hi - 1]; only the edges in between need a lens area
+      int nlo = 0, nhi = 0;
+      for (int e = 1 + lane; e <= nz; e += 32) {
+        nlo += zes[e] <= c - k;
+        nhi += zes[e] < c + k;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        nlo += __shfl_xor_sync(0xffffffffu, nlo, o);
+        nhi += __shfl_xor_sync(0xffffffffu, nhi, o);
+      }
+      const int e_lo = 1 + nlo, e_hi = 1 + nhi;          // partial edges: e_lo <= e < e_hi
       double s = 0.0;
-      for (int e = 1 + lane; e <= nz; e += 32) s = fma(rr_lens_area(zes[e], k, c), D[e], s);
+      for (int e = e_lo + lane; e < e_hi; e += 32) s = fma(rr_lens_area_fast(zes[e], k, c), D[e], s);
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-      out = s / rr_lens_area(1.0, k, c);
+      if (e_hi <= nz) s = fma(RR_PI * k * k, (double)pr[e_hi - 1], s);
+      out = s / rr_lens_area_fast(1.0, k, c);
     }
     if (lane == 0) rows[row * ng + ig] = (TR)out;
   }
