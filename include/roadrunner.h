@@ -135,6 +135,11 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
                       void *stream);
 /* RR_TABLE_*; takes effect at the next rr_build_ld_table.  RR_TABLE_DIRECT needs nz <= 2000.     */
 int rr_set_table_mode(rr_ctx *ctx, int32_t mode);
+/* Transmission-spectroscopy shortcut (meaningful with nkpb = npb): on != 0 takes
+ * the LD weights of every passband at the MEAN of the pv's radius ratios (one weight array per pv);
+ * each passband keeps its own k for g = z/(1+k) and for the intersection area (reading R13).
+ * Takes effect at the next rr_evaluate.                                                          */
+int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on);
 /* Diagnostics: device pointers to the full table (built on demand in lazy mode; synchronous) and
  * Istar of the last rr_build_ld_table (ctx precision), or NULL.                                 */
 const void *rr_table_ptr(rr_ctx *ctx);

@@ -61,13 +61,18 @@ def load():
                                     C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32,
                                     _D, _I, _D, C.c_int32]
     lib.oracle_evaluate.restype = None
+    lib.oracle_evaluate_mk.argtypes = [_D, _I, C.c_int64, _I, _I, _D, C.c_int32,
+                                       _D, C.c_int32, C.c_int64, _D, _D,
+                                       C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32,
+                                       C.c_int32, _D, _I, _D, C.c_int32]
+    lib.oracle_evaluate_mk.restype = None
     lib.oracle_direct_rows.argtypes = [_D, C.c_int, C.c_int, _D, _D, C.c_int64, _D]
     lib.oracle_direct_rows.restype = None
     lib.oracle_flux_from_row.argtypes = [C.c_double, C.c_double, _D, C.c_int, C.c_double]
     lib.oracle_flux_from_row.restype = C.c_double
     lib.oracle_evaluate_direct.argtypes = [_D, _I, C.c_int64, _I, _I, _D, _D, C.c_int32,
-                                           C.c_int64, _D, _D, C.c_int32, C.c_int32, _D, _I,
-                                           C.c_int32]
+                                           C.c_int64, _D, _D, C.c_int32, C.c_int32, C.c_int32,
+                                           _D, _I, C.c_int32]
     lib.oracle_evaluate_direct.restype = None
     _lib = lib
     return lib
@@ -165,7 +170,7 @@ class OracleModel:
         return self.T, self.istar
 
     def evaluate(self, times, lc_index, passband_index, supersampling, exposure_time, pv,
-                 nthreads=1, want_z=False):
+                 nthreads=1, want_z=False, mean_k_weights=False):
         times, pv = _f64(times), _f64(pv)
         pv = pv.reshape(-1, self.nkpb + 6)
         lc_index, passband_index = _i32(lc_index), _i32(passband_index)
@@ -180,11 +185,13 @@ class OracleModel:
         if want_z:
             nsub = int(supersampling.astype(np.int64)[lc_index].sum())
             z = np.empty((npv, nsub))
-        load().oracle_evaluate(_dp(times), _ip(lc_index), npt, _ip(passband_index),
-                               _ip(supersampling), _dp(exposure_time), passband_index.size,
-                               _dp(pv), self.nkpb, npv, _dp(self.T), _dp(self.istar),
-                               self.npb, self.nk, self.k0, self.k1, self.ng,
-                               _dp(flux), _ip(status), _dp(z) if want_z else None, int(nthreads))
+        load().oracle_evaluate_mk(_dp(times), _ip(lc_index), npt, _ip(passband_index),
+                                  _ip(supersampling), _dp(exposure_time), passband_index.size,
+                                  _dp(pv), self.nkpb, npv, _dp(self.T), _dp(self.istar),
+                                  self.npb, self.nk, self.k0, self.k1, self.ng,
+                                  int(bool(mean_k_weights)),
+                                  _dp(flux), _ip(status), _dp(z) if want_z else None,
+                                  int(nthreads))
         return (flux, status, z) if want_z else (flux, status)
 
 
@@ -202,34 +209,39 @@ class OracleDirectModel:
     def from_config(cls, m):
         return cls(m.nzin, m.nzlimb, m.zcut, m.ng, m.npb, m.nkpb)
 
-    def rows(self, ldp, pv):
-        """ldw[npv][npb][ng] and Istar[npv][npb] for the k of every (pv, passband)."""
+    def rows(self, ldp, pv, mean_k_weights=False):
+        """ldw[npv][npb][ng] and Istar[npv][npb] for the k of every (pv, passband); with
+        mean_k_weights the weights of every passband are taken at the pv's mean k (PAPER.md:188-190;
+        the selection of which k to pass is the only thing done here)."""
         ldp = _f64(ldp).reshape(-1, self.npb, self.nz)
         pv = _f64(pv).reshape(-1, self.nkpb + 6)
         npv = ldp.shape[0]
         kcol = [0] * self.npb if self.nkpb == 1 else list(range(self.npb))
         k = _f64(pv[:, kcol])                                   # [npv][npb]
+        if mean_k_weights:
+            k = _f64(np.repeat(pv[:, :self.nkpb].mean(axis=1)[:, None], self.npb, axis=1))
         out = np.empty((npv, self.npb, self.ng))
         load().oracle_direct_rows(_dp(self.ze), self.nz, self.ng, _dp(k), _dp(ldp),
                                   npv * self.npb, _dp(out))
         return out, istar(self.ze, ldp)
 
     def evaluate(self, times, lc_index, passband_index, supersampling, exposure_time, pv, ldp,
-                 nthreads=1):
+                 nthreads=1, mean_k_weights=False):
         times, pv = _f64(times), _f64(pv).reshape(-1, self.nkpb + 6)
         lc_index, passband_index = _i32(lc_index), _i32(passband_index)
         supersampling, exposure_time = _i32(supersampling), _f64(exposure_time)
         ok = np.all(np.isfinite(pv[:, :self.nkpb]) & (pv[:, :self.nkpb] > 0), axis=1)
         safe = pv.copy()
         safe[~ok, :self.nkpb] = 0.1                              # rows of invalid pvs are not used
-        rows, ist = self.rows(ldp, safe)
+        rows, ist = self.rows(ldp, safe, mean_k_weights)
         npv, npt = pv.shape[0], times.size
         flux = np.empty((npv, npt))
         status = np.empty(npv, np.int32)
         load().oracle_evaluate_direct(_dp(times), _ip(lc_index), npt, _ip(passband_index),
                                       _ip(supersampling), _dp(exposure_time), _dp(pv), self.nkpb,
-                                      npv, _dp(rows), _dp(ist), self.npb, self.ng, _dp(flux),
-                                      _ip(status), int(nthreads))
+                                      npv, _dp(rows), _dp(ist), self.npb, self.ng,
+                                      int(bool(mean_k_weights)), _dp(flux), _ip(status),
+                                      int(nthreads))
         return flux, status
 
 

@@ -201,17 +201,22 @@ double oracle_separation(double t, double t0, double p, double a, double inc, do
 }
 
 /* ---- step 9: one sub-sample's flux from the table (reading R10) ---- */
-double oracle_flux_from_table(double z, double k, const double *T /*[nk][ng]*/, int nk, double k0,
-                              double k1, int ng, double istar)
+/* kw = the radius ratio the limb-darkening weights are taken at: k itself, or the mean of the pv's
+ * radius ratios over the passbands (transmission-spectroscopy shortcut, reading
+ * R13: the weight array - its g axis included - is that of a planet of radius kw; the passband's
+ * own k sets the transit's extent and the intersection area). */
+double oracle_flux_from_table_kw(double z, double k, double kw, const double *T /*[nk][ng]*/,
+                                 int nk, double k0, double k1, int ng, double istar)
 {
     if (z >= 1.0 + k) return 1.0;
     double dk = (k1 - k0) / (double)(nk - 1), dg = 1.0 / (double)(ng - 1);
-    double x = (k - k0) / dk;
+    double x = (kw - k0) / dk;
     int ik = (int)floor(x);
     if (ik > nk - 2) ik = nk - 2;
     if (ik < 0) ik = 0;
     double ak = x - ik;
-    double y = (z / (1.0 + k)) / dg;
+    double y = (z / (1.0 + kw)) / dg;      /* the weights belong to a planet of radius kw at z */
+    if (y > (double)(ng - 1)) y = (double)(ng - 1);   /* 1+kw <= z < 1+k: limb node (R5, R13) */
     int ig = (int)floor(y);
     if (ig > ng - 2) ig = ng - 2;
     double ag = y - ig;
@@ -220,6 +225,12 @@ double oracle_flux_from_table(double z, double k, const double *T /*[nk][ng]*/, 
               + ak * ((1.0 - ag) * T1[ig] + ag * T1[ig + 1]);
     double ap = oracle_lens_area(1.0, k, z);
     return (istar - ip * ap) / istar;
+}
+
+double oracle_flux_from_table(double z, double k, const double *T /*[nk][ng]*/, int nk, double k0,
+                              double k1, int ng, double istar)
+{
+    return oracle_flux_from_table_kw(z, k, k, T, nk, k0, k1, ng, istar);
 }
 
 /* Per-pv validity (reading R12): bit 0 k outside [k0,k1]; bit 1 e outside [0,1); bit 2 a <= 0;
@@ -237,6 +248,15 @@ int oracle_pv_status(const double *pv, int nkpb, double k0, double k1)
     return st;
 }
 
+void oracle_evaluate_mk(const double *times, const int32_t *lc_index, int64_t npt,
+                        const int32_t *passband_index, const int32_t *supersampling,
+                        const double *exposure_time, int32_t nlc,
+                        const double *pv, int32_t nkpb, int64_t npv,
+                        const double *T, const double *istar,
+                        int32_t npb, int32_t nk, double k0, double k1, int32_t ng,
+                        int32_t mean_k_weights,
+                        double *flux, int32_t *status, double *z_out, int32_t nthreads);
+
 /* ---- steps 7-10: the whole L2 evaluation ---------------------------------------------------------
  * flux[npv][npt]; z_out (optional) [npv][nsub], nsub = sum over exposures of their ns, sub-samples
  * of exposure i stored contiguously in exposure order; behind-the-star sub-samples store -z.
@@ -248,6 +268,20 @@ void oracle_evaluate(const double *times, const int32_t *lc_index, int64_t npt,
                      const double *T /*[npv][npb][nk][ng]*/, const double *istar /*[npv][npb]*/,
                      int32_t npb, int32_t nk, double k0, double k1, int32_t ng,
                      double *flux, int32_t *status, double *z_out, int32_t nthreads)
+{
+    oracle_evaluate_mk(times, lc_index, npt, passband_index, supersampling, exposure_time, nlc, pv,
+                       nkpb, npv, T, istar, npb, nk, k0, k1, ng, 0, flux, status, z_out, nthreads);
+}
+
+/* mean_k_weights != 0: PAPER.md:188-190, LD weights at the mean of the pv's radius ratios. */
+void oracle_evaluate_mk(const double *times, const int32_t *lc_index, int64_t npt,
+                        const int32_t *passband_index, const int32_t *supersampling,
+                        const double *exposure_time, int32_t nlc,
+                        const double *pv, int32_t nkpb, int64_t npv,
+                        const double *T, const double *istar,
+                        int32_t npb, int32_t nk, double k0, double k1, int32_t ng,
+                        int32_t mean_k_weights,
+                        double *flux, int32_t *status, double *z_out, int32_t nthreads)
 {
     (void)nlc;
     int64_t nsub = 0;
@@ -276,6 +310,12 @@ void oracle_evaluate(const double *times, const int32_t *lc_index, int64_t npt,
             int ns = supersampling[l];
             double tau = exposure_time[l];
             double k = row[nkpb == 1 ? 0 : pb];
+            double kw = k;
+            if (mean_k_weights) {
+                kw = 0.0;
+                for (int q = 0; q < nkpb; ++q) kw += row[q];
+                kw /= (double)nkpb;
+            }
             const double *Tvp = T + ((size_t)v * npb + pb) * (size_t)(nk * ng);
             double is = istar[v * npb + pb];
             double sum = 0.0;
@@ -284,7 +324,7 @@ void oracle_evaluate(const double *times, const int32_t *lc_index, int64_t npt,
                 int front;
                 double z = oracle_separation(t, t0, p, a, inc, e, w, &front);
                 if (z_out) z_out[v * nsub + q++] = front ? z : -z;
-                sum += front ? oracle_flux_from_table(z, k, Tvp, nk, k0, k1, ng, is) : 1.0;
+                sum += front ? oracle_flux_from_table_kw(z, k, kw, Tvp, nk, k0, k1, ng, is) : 1.0;
             }
             flux[v * npt + i] = sum / (double)ns;        /* mean over sub-samples */
         }
@@ -313,11 +353,13 @@ void oracle_direct_rows(const double *ze, int nz, int ng, const double *k /*[nro
 }
 
 /* One sub-sample's flux from a direct-model row (reading R10 for the last cell). */
-double oracle_flux_from_row(double z, double k, const double *ldw /*[ng]*/, int ng, double istar)
+double oracle_flux_from_row_kw(double z, double k, double kw, const double *ldw /*[ng]*/, int ng,
+                               double istar)
 {
     if (z >= 1.0 + k) return 1.0;
     double dg = 1.0 / (double)(ng - 1);
-    double y = (z / (1.0 + k)) / dg;
+    double y = (z / (1.0 + kw)) / dg;
+    if (y > (double)(ng - 1)) y = (double)(ng - 1);
     int ig = (int)floor(y);
     if (ig > ng - 2) ig = ng - 2;
     double ag = y - ig;
@@ -326,13 +368,20 @@ double oracle_flux_from_row(double z, double k, const double *ldw /*[ng]*/, int 
     return (istar - ip * ap) / istar;
 }
 
+double oracle_flux_from_row(double z, double k, const double *ldw /*[ng]*/, int ng, double istar)
+{
+    return oracle_flux_from_row_kw(z, k, k, ldw, ng, istar);
+}
+
 /* The whole direct-model evaluation: as oracle_evaluate, with rows[npv][npb][ng] from
- * oracle_direct_rows in place of the table, and k > 0 the only limit on k (status bit 0). */
+ * oracle_direct_rows in place of the table, and k > 0 the only limit on k (status bit 0).
+ * mean_k_weights: the rows were built at the pv's mean k (reading R13). */
 void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_t npt,
                             const int32_t *passband_index, const int32_t *supersampling,
                             const double *exposure_time, const double *pv, int32_t nkpb,
                             int64_t npv, const double *rows, const double *istar, int32_t npb,
-                            int32_t ng, double *flux, int32_t *status, int32_t nthreads)
+                            int32_t ng, int32_t mean_k_weights, double *flux, int32_t *status,
+                            int32_t nthreads)
 {
 #ifdef _OPENMP
     if (nthreads > 0) omp_set_num_threads(nthreads);
@@ -356,6 +405,12 @@ void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_
             int ns = supersampling[l];
             double tau = exposure_time[l];
             double k = row[nkpb == 1 ? 0 : pb];
+            double kw = k;
+            if (mean_k_weights) {
+                kw = 0.0;
+                for (int q = 0; q < nkpb; ++q) kw += row[q];
+                kw /= (double)nkpb;
+            }
             const double *ldw = rows + ((size_t)v * npb + pb) * (size_t)ng;
             double is = istar[v * npb + pb];
             double sum = 0.0;
@@ -363,7 +418,7 @@ void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_
                 double t = times[i] + tau * ((s + 0.5) / (double)ns - 0.5);
                 int front;
                 double z = oracle_separation(t, t0, p, a, inc, e, w, &front);
-                sum += front ? oracle_flux_from_row(z, k, ldw, ng, is) : 1.0;
+                sum += front ? oracle_flux_from_row_kw(z, k, kw, ldw, ng, is) : 1.0;
             }
             flux[v * npt + i] = sum / (double)ns;
         }

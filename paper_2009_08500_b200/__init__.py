@@ -33,7 +33,7 @@ SYMBOLS = (
     "rr_evaluate_flat", "rr_orbit_z", "rr_num_subsamples", "rr_num_tiles", "rr_get_tiles",
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
-    "rr_get_kernel_times", "rr_get_rows",
+    "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
 )
 
 
@@ -94,6 +94,7 @@ def load() -> C.CDLL:
         "rr_measure_fma_peak": (C.c_int, [_I32, C.POINTER(_DBL), _VP]),
         "rr_set_table_mode": (C.c_int, [_VP, _I32]),
         "rr_get_rows": (C.c_int, [_VP, _VP]),
+        "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
         "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
         "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
@@ -244,6 +245,10 @@ def rr_set_reduction(ctx: int, mode: int):
 
 def rr_set_table_mode(ctx: int, mode: int):
     _check(load().rr_set_table_mode(ctx, mode), "rr_set_table_mode")
+
+
+def rr_set_mean_k_weights(ctx: int, on: bool):
+    _check(load().rr_set_mean_k_weights(ctx, int(bool(on))), "rr_set_mean_k_weights")
 
 
 def rr_enable_kernel_timing(ctx: int, on: bool):

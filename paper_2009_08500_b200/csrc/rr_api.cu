@@ -222,6 +222,12 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
   return rr_ld_table_launch(ctx, &ctx->work[0], d_ldp, d_istar, npv, (cudaStream_t)stream);
 }
 
+int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on) {
+  if (!ctx) return RR_ENULL;
+  ctx->mean_k = on ? 1 : 0;
+  return RR_OK;
+}
+
 int rr_set_table_mode(rr_ctx *ctx, int32_t mode) {
   if (!ctx) return RR_ENULL;
   if (mode != RR_TABLE_LAZY && mode != RR_TABLE_FULL && mode != RR_TABLE_DIRECT) return RR_ECONFIG;

@@ -58,7 +58,9 @@ struct RRPvBand {
   double k2;           // k^2
   double gscale;       // (ng-1)/(1+k): y = z*gscale is the g coordinate in table cells
   double ak;           // weight of table row ik+1
-  int32_t ik;          // lower k row, clamped to nk-2 (reading R10)
+  double kw;           // radius ratio the LD weights are taken at: k, or the mean of the pv's k over
+                       // the passbands (transmission-spectroscopy shortcut)
+  int32_t ik;          // lower k row of kw, clamped to nk-2 (reading R10)
   int32_t pad;
 };
 
@@ -107,7 +109,8 @@ struct rr_ctx {
   int64_t scratch_cap;
   int32_t reduction;
   int32_t any_shuffle;
-  int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL
+  int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL | RR_TABLE_DIRECT
+  int32_t mean_k;       // 1: LD weights at the mean k of the passbands
   // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
   RRWork work[3];
   // counters / accounting

@@ -37,7 +37,7 @@ constexpr int FT = 256;   // threads per flux block
 // ---- per-pv prep ---------------------------------------------------------------------------------
 __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, int nkpb, int nk,
                                   double k0, double k1, double kmin, double kmax_ok, int ng,
-                                  int fp32,
+                                  int fp32, int mean_k, int row_pad,
                                   RRPvOrbit *__restrict__ pvo, RRPvBand *__restrict__ pvb,
                                   int32_t *__restrict__ status_out) {
   int64_t v = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -56,12 +56,14 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     if (a <= 0.0) st |= RR_PV_A_RANGE;
     if (p <= 0.0) st |= RR_PV_P_RANGE;
   }
-  if (status_out) status_out[v] = st;
+  int st_k = 0;
   RRPvOrbit po;
-  po.status = st;
   po.circular = (e == 0.0);
   double kmax = 0.0;
   const double dk = (k1 - k0) / (double)(nk - 1);
+  double kmean = 0.0;
+  for (int q = 0; q < nkpb; ++q) kmean += row[q];
+  kmean /= (double)nkpb;
   for (int q = 0; q < nkpb; ++q) {
     double k = row[q];
     RRPvBand b;
@@ -71,8 +73,12 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     double rmin = fmin(1.0, k);
     b.afull = RR_PI * rmin * rmin;
     b.k2 = k * k;
-    b.gscale = (double)(ng - 1) / (1.0 + k);
-    double x = (k - k0) / dk;
+    const double kw = mean_k ? kmean : k;
+    b.kw = kw;
+    b.gscale = (double)(ng - 1) / (1.0 + kw);   // the g axis of the weights is that of radius kw
+    // mean-k weights: y = z gscale reaches (ng-1)(1+k)/(1+kw); the staged row is padded up to there
+    if (!(b.gscale * (1.0 + k) < (double)(ng + row_pad) - 1.5)) st_k = 1;
+    double x = (kw - k0) / dk;
     int ik = (int)floor(x);
     ik = min(max(ik, 0), nk - 2);
     b.ik = ik;
@@ -81,6 +87,9 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     pvb[v * nkpb + q] = b;
     kmax = fmax(kmax, k);
   }
+  if (st_k && !st) st = RR_PV_K_RANGE;
+  if (status_out) status_out[v] = st;
+  po.status = st;
   po.t0 = t0;
   po.inv_p = 1.0 / p;
   double ci = cos(inc);
@@ -380,6 +389,8 @@ struct FluxParams {
   int64_t npt, npv, ntiles;
   int npb, nkpb, nk, ng;
   int shuffle_min_ns;   // light curves with ns >= this use the lanes-over-sub-samples layout
+  int ldw_len;          // staged row length: ng + 1, or more with mean-k weights, where g of a
+                        // passband with k > kw passes the last node (reading R13): limb value
   unsigned nchunks;     // blocks per parameter vector
   unsigned chunk_len;   // dispatch tiles per block
 };
@@ -586,13 +597,13 @@ rr_flux_kernel(const FluxParams P) {
         __syncthreads();
         if (P.rows) {                                  // lazy mode: the row was collapsed for this k
           const R *rw = reinterpret_cast<const R *>(P.rows) + trow * (int64_t)P.ng;
-          for (int ig = threadIdx.x; ig <= P.ng; ig += FT) ldw[ig] = rw[min(ig, P.ng - 1)];
+          for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) ldw[ig] = rw[min(ig, P.ng - 1)];
         } else {
           const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
           const R *T1 = T0 + P.ng;
           const R ak = (R)pb.ak;
-          for (int ig = threadIdx.x; ig <= P.ng; ig += FT) {
-            const int jg = min(ig, P.ng - 1);          // ldw[ng] = ldw[ng-1]: see rr_cell
+          for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) {
+            const int jg = min(ig, P.ng - 1);          // ldw[ng..] = ldw[ng-1]: see rr_cell
             ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
           }
         }
@@ -716,6 +727,15 @@ int fma_peak_typed(double *h_fma_per_s, cudaStream_t st) {
 
 }  // namespace
 
+// Extra nodes of the staged table row beyond ng - 1 (all equal to the limb node): 1 normally; with
+// mean-k weights and chromatic k, g = z/(1+kw) of a passband with k > kw runs up to (1+k)/(1+kw).
+static int rr_row_pad(const rr_ctx *ctx) {
+  const rr_config &c = ctx->cfg;
+  if (!(ctx->mean_k && c.nkpb > 1)) return 1;
+  if (ctx->table_mode == RR_TABLE_DIRECT) return c.ng + 2;    // no k limits: up to k = 1 + 2 kw
+  return (int)ceil((c.ng - 1) * (c.k1 - c.k0) / (1.0 + c.k0)) + 3;
+}
+
 // ---- host launchers -------------------------------------------------------------------------------
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
                       int32_t *d_status, cudaStream_t st) {
@@ -737,7 +757,7 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
   const bool direct = wk->lazy == 2;
   rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
       d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, direct ? 1e-300 : c.k0, direct ? 1e300 : c.k1, c.ng,
-      c.precision == RR_FP32, wk->pvo, wk->pvb, d_status);
+      c.precision == RR_FP32, ctx->mean_k, rr_row_pad(ctx), wk->pvo, wk->pvb, d_status);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
@@ -771,6 +791,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   // shuffle; lanes-over-sub-samples multiplies the parallelism by ns, which only pays when
   // npv x npt alone cannot fill the GPU.
   const int64_t resident = (int64_t)ctx->sm_count * 2048;
+  P.ldw_len = c.ng + rr_row_pad(ctx);
   if (ctx->reduction == RR_REDUCE_THREAD) P.shuffle_min_ns = 0x7fffffff;
   else if (ctx->reduction == RR_REDUCE_SHUFFLE) P.shuffle_min_ns = 2;
   else P.shuffle_min_ns = (npv * ctx->npt < 2 * resident) ? 4 : 0x7fffffff;
@@ -787,7 +808,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + c.ng + 1) * (c.precision == RR_FP32 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + P.ldw_len) * (c.precision == RR_FP32 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
     if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);

@@ -104,7 +104,7 @@ rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
   const int64_t row = blockIdx.x;
   const int64_t v = row / npb;
   const int pb = (int)(row - v * npb);
-  const double k = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].k;
+  const double k = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].kw;   // the k the weights are taken at
   const TR *pr = ldp + row * nz;
   for (int e = threadIdx.x; e <= nz; e += 256) {
     zes[e] = ze[e];

@@ -220,6 +220,40 @@ def test_direct_model_has_no_k_limits(rr):
     assert want[0].min() < 0.85
 
 
+@pytest.mark.parametrize("mode", [0, 1, 2])
+def test_mean_k_weights_shortcut(rr, mode):
+    """Transmission-spectroscopy shortcut (reading R13) with chromatic k, in the
+    lazy, full-table and direct modes, against the oracle's statement of it."""
+    mc = workloads.ModelConfig(npb=3, nkpb=3)
+    rng = np.random.default_rng(8)
+    base = workloads.make_workload(1, npv=9, npt=10).pv
+    kk = np.clip(base[:, :1] * (1 + 0.05 * rng.uniform(-1, 1, (9, 3))), 0.021, 0.199)
+    pv = np.concatenate([kk, base[:, 1:]], axis=1)
+    times = np.tile(np.linspace(-0.15, 0.15, 700), 3)
+    lc = np.repeat(np.arange(3, dtype=np.int32), 700)
+    coeffs = rng.uniform(0.1, 0.4, (9, 3, 2))
+    pbs, nss, ets = [0, 1, 2], [1, 1, 3], [0.0, 0.0, 0.01]
+    if mode == 2:
+        om = oracle.OracleDirectModel.from_config(mc)
+        want, _ = om.evaluate(times, lc, pbs, nss, ets, pv,
+                              workloads.sample_profile("quadratic", coeffs, om.mu),
+                              mean_k_weights=True)
+    else:
+        om = oracle.OracleModel.from_config(mc)
+        om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+        want, _ = om.evaluate(times, lc, pbs, nss, ets, pv, mean_k_weights=True)
+        exact, _ = om.evaluate(times, lc, pbs, nss, ets, pv)
+        assert np.max(np.abs(want - exact)) > 1e-7            # the shortcut is visible ...
+    gm = rr.RoadRunner.from_config(mc)
+    rr.rr_set_table_mode(gm.ctx, mode)
+    rr.rr_set_mean_k_weights(gm.ctx, True)
+    gm.set_data(times, lc, pbs, nss, ets)
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy()
+    assert np.max(np.abs(got - want)) <= TOL64                 # ... and the GPU takes the same one
+    gm.close()
+
+
 def test_kernel_timing_counts_calls(rr):
     wl = small_workload(1)
     gm = gpu_model(rr, wl)

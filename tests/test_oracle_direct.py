@@ -88,3 +88,41 @@ def test_direct_evaluate_equals_table_model_on_a_k_node_and_allows_any_k():
                           wl.exposure_time, pv, wl.ldp(md.mu))
     assert list(st) == [0, 1, 0, 0] and np.all(np.isnan(got[1])) and np.all(np.isfinite(got[0]))
     assert got[0].min() < 0.9          # a k = 0.45 transit is deep
+
+
+# ---- transmission-spectroscopy shortcut (reading R13) ------------------------------
+def _chromatic_case(spread):
+    mc = workloads.ModelConfig(npb=3, nkpb=3)
+    rng = np.random.default_rng(8)
+    base = workloads.make_workload(1, npv=5, npt=10).pv
+    kk = np.clip(base[:, :1] * (1 + spread * rng.uniform(-1, 1, (5, 3))), 0.021, 0.199)
+    pv = np.concatenate([kk, base[:, 1:]], axis=1)
+    times = np.tile(np.linspace(-0.15, 0.15, 400), 3)
+    lc = np.repeat(np.arange(3, dtype=np.int32), 400)
+    coeffs = rng.uniform(0.1, 0.4, (5, 3, 2))
+    return mc, pv, times, lc, coeffs
+
+
+def test_mean_k_weights_equal_k_is_identity_and_small_otherwise():
+    """All passbands at the same k: the shortcut changes nothing (exact).  With +-3 % of chromatic
+    variation (large for transmission spectroscopy) it moves the flux by < 1e-4, most in
+    ingress/egress and for grazing transits, where a planet of radius kbar and one of radius k sample
+    different parts of the steep limb: the 'insignificant effect' of PAPER.md:190.  Not zero."""
+    for spread, lo, hi in ((0.0, -1.0, 0.0), (0.03, 1e-12, 1e-4)):
+        mc, pv, times, lc, coeffs = _chromatic_case(spread)
+        for model in ("table", "direct"):
+            if model == "table":
+                om = oracle.OracleModel.from_config(mc)
+                om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+                a, _ = om.evaluate(times, lc, [0, 1, 2], [1, 1, 2], [0.0, 0.0, 0.01], pv)
+                b, _ = om.evaluate(times, lc, [0, 1, 2], [1, 1, 2], [0.0, 0.0, 0.01], pv,
+                                   mean_k_weights=True)
+            else:
+                om = oracle.OracleDirectModel.from_config(mc)
+                ldp = workloads.sample_profile("quadratic", coeffs, om.mu)
+                a, _ = om.evaluate(times, lc, [0, 1, 2], [1, 1, 2], [0.0, 0.0, 0.01], pv, ldp)
+                b, _ = om.evaluate(times, lc, [0, 1, 2], [1, 1, 2], [0.0, 0.0, 0.01], pv, ldp,
+                                   mean_k_weights=True)
+            d = float(np.max(np.abs(a - b)))
+            assert lo < d <= hi, (spread, model, d)
+            assert (a < 1).sum() > 100
