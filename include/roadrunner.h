@@ -140,6 +140,12 @@ int rr_set_table_mode(rr_ctx *ctx, int32_t mode);
  * each passband keeps its own k for g = z/(1+k) and for the intersection area (reading R13).
  * Takes effect at the next rr_evaluate.                                                          */
 int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on);
+/* Small-planet approximation (reading R14): for rows whose weight radius is
+ * <= k_threshold the mean occulted brightness is replaced by the profile's value at the planet's
+ * centre (linear interpolation of ldp over the bin means zm, constant beyond the first and last
+ * node).  k_threshold = 0 (default) switches it off.  Needs RR_TABLE_LAZY or RR_TABLE_DIRECT
+ * (rr_evaluate returns RR_ESTATE on a full table).  Takes effect at the next rr_evaluate.        */
+int rr_set_small_planet(rr_ctx *ctx, double k_threshold);
 /* Diagnostics: device pointers to the full table (built on demand in lazy mode; synchronous) and
  * Istar of the last rr_build_ld_table (ctx precision), or NULL.                                 */
 const void *rr_table_ptr(rr_ctx *ctx);

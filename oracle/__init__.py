@@ -68,6 +68,10 @@ def load():
     lib.oracle_evaluate_mk.restype = None
     lib.oracle_direct_rows.argtypes = [_D, C.c_int, C.c_int, _D, _D, C.c_int64, _D]
     lib.oracle_direct_rows.restype = None
+    lib.oracle_direct_rows_sp.argtypes = [_D, _D, C.c_int, C.c_int, _D, _D, C.c_int64, C.c_double, _D]
+    lib.oracle_direct_rows_sp.restype = None
+    lib.oracle_profile_at.argtypes = [C.c_double, _D, _D, C.c_int]
+    lib.oracle_profile_at.restype = C.c_double
     lib.oracle_flux_from_row.argtypes = [C.c_double, C.c_double, _D, C.c_int, C.c_double]
     lib.oracle_flux_from_row.restype = C.c_double
     lib.oracle_evaluate_direct.argtypes = [_D, _I, C.c_int64, _I, _I, _D, _D, C.c_int32,
@@ -209,7 +213,7 @@ class OracleDirectModel:
     def from_config(cls, m):
         return cls(m.nzin, m.nzlimb, m.zcut, m.ng, m.npb, m.nkpb)
 
-    def rows(self, ldp, pv, mean_k_weights=False):
+    def rows(self, ldp, pv, mean_k_weights=False, small_planet_k=0.0):
         """ldw[npv][npb][ng] and Istar[npv][npb] for the k of every (pv, passband); with
         mean_k_weights the weights of every passband are taken at the pv's mean k (PAPER.md:188-190;
         the selection of which k to pass is the only thing done here)."""
@@ -221,19 +225,19 @@ class OracleDirectModel:
         if mean_k_weights:
             k = _f64(np.repeat(pv[:, :self.nkpb].mean(axis=1)[:, None], self.npb, axis=1))
         out = np.empty((npv, self.npb, self.ng))
-        load().oracle_direct_rows(_dp(self.ze), self.nz, self.ng, _dp(k), _dp(ldp),
-                                  npv * self.npb, _dp(out))
+        load().oracle_direct_rows_sp(_dp(self.ze), _dp(self.zm), self.nz, self.ng, _dp(k), _dp(ldp),
+                                     npv * self.npb, float(small_planet_k), _dp(out))
         return out, istar(self.ze, ldp)
 
     def evaluate(self, times, lc_index, passband_index, supersampling, exposure_time, pv, ldp,
-                 nthreads=1, mean_k_weights=False):
+                 nthreads=1, mean_k_weights=False, small_planet_k=0.0):
         times, pv = _f64(times), _f64(pv).reshape(-1, self.nkpb + 6)
         lc_index, passband_index = _i32(lc_index), _i32(passband_index)
         supersampling, exposure_time = _i32(supersampling), _f64(exposure_time)
         ok = np.all(np.isfinite(pv[:, :self.nkpb]) & (pv[:, :self.nkpb] > 0), axis=1)
         safe = pv.copy()
         safe[~ok, :self.nkpb] = 0.1                              # rows of invalid pvs are not used
-        rows, ist = self.rows(ldp, safe, mean_k_weights)
+        rows, ist = self.rows(ldp, safe, mean_k_weights, small_planet_k)
         npv, npt = pv.shape[0], times.size
         flux = np.empty((npv, npt))
         status = np.empty(npv, np.int32)
@@ -243,6 +247,11 @@ class OracleDirectModel:
                                       int(bool(mean_k_weights)), _dp(flux), _ip(status),
                                       int(nthreads))
         return flux, status
+
+
+def profile_at(z, zm, ldp):
+    zm, ldp = _f64(zm), _f64(ldp)
+    return load().oracle_profile_at(float(z), _dp(zm), _dp(ldp), zm.size)
 
 
 def flux_from_row(z, k, ldw, istar_value):

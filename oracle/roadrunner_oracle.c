@@ -424,3 +424,37 @@ void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_
         }
     }
 }
+
+/* ==== small-planet approximation (reading R14) ====================
+ * "If the planet is small enough, the weighted average can be replaced with the limb darkening
+ * value evaluated at the centre of the planet."  The profile is known at the bin means zm (R1):
+ * its value at z is the linear interpolant over zm, held constant before the first and after the
+ * last node (a centre beyond the limb sees the limb sample, consistent with R5).  In the row
+ * formalism of PAPER.md:97-105 the node g_ig holds the profile at z = g_ig (1+k). */
+double oracle_profile_at(double z, const double *zm, const double *ldp, int nz)
+{
+    if (z <= zm[0]) return ldp[0];
+    if (z >= zm[nz - 1]) return ldp[nz - 1];
+    int j = 0;
+    while (zm[j + 1] <= z) ++j;                        /* zm[j] <= z < zm[j+1] */
+    double a = (z - zm[j]) / (zm[j + 1] - zm[j]);
+    return (1.0 - a) * ldp[j] + a * ldp[j + 1];
+}
+
+/* Direct-model rows with the small-planet approximation for rows whose k <= k_small
+ * (k_small <= 0: never). */
+void oracle_direct_rows_sp(const double *ze, const double *zm, int nz, int ng, const double *k,
+                           const double *ldp, int64_t nrows, double k_small, double *rows)
+{
+    double dg = 1.0 / (double)(ng - 1);
+    for (int64_t r = 0; r < nrows; ++r) {
+        if (k_small > 0.0 && k[r] <= k_small) {
+            for (int ig = 0; ig < ng; ++ig) {
+                double g = (ig == ng - 1) ? 1.0 : ig * dg;
+                rows[r * ng + ig] = oracle_profile_at(g * (1.0 + k[r]), zm, ldp + r * nz, nz);
+            }
+        } else {
+            oracle_direct_rows(ze, nz, ng, k + r, ldp + r * nz, 1, rows + r * ng);
+        }
+    }
+}

@@ -34,6 +34,7 @@ SYMBOLS = (
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
+    "rr_set_small_planet",
 )
 
 
@@ -95,6 +96,7 @@ def load() -> C.CDLL:
         "rr_set_table_mode": (C.c_int, [_VP, _I32]),
         "rr_get_rows": (C.c_int, [_VP, _VP]),
         "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
+        "rr_set_small_planet": (C.c_int, [_VP, _DBL]),
         "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
         "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
@@ -245,6 +247,10 @@ def rr_set_reduction(ctx: int, mode: int):
 
 def rr_set_table_mode(ctx: int, mode: int):
     _check(load().rr_set_table_mode(ctx, mode), "rr_set_table_mode")
+
+
+def rr_set_small_planet(ctx: int, k_threshold: float):
+    _check(load().rr_set_small_planet(ctx, float(k_threshold)), "rr_set_small_planet")
 
 
 def rr_set_mean_k_weights(ctx: int, on: bool):

@@ -222,6 +222,13 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
   return rr_ld_table_launch(ctx, &ctx->work[0], d_ldp, d_istar, npv, (cudaStream_t)stream);
 }
 
+int rr_set_small_planet(rr_ctx *ctx, double k_threshold) {
+  if (!ctx) return RR_ENULL;
+  if (!(k_threshold >= 0.0) || !isfinite(k_threshold)) return RR_ECONFIG;
+  ctx->k_small = k_threshold;
+  return RR_OK;
+}
+
 int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on) {
   if (!ctx) return RR_ENULL;
   ctx->mean_k = on ? 1 : 0;
@@ -279,6 +286,7 @@ int rr_evaluate(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, void
   if (!ctx || !d_pv || !d_flux) return RR_ENULL;
   if (npv <= 0 || npar != ctx->cfg.nkpb + 6) return RR_ESIZE;
   if (ctx->ntiles < 0 || ctx->work[0].table_npv != npv) return RR_ESTATE;
+  if (ctx->k_small > 0.0 && !ctx->work[0].lazy) return RR_ESTATE;   // needs the row builders
   cudaStream_t st = (cudaStream_t)stream;
   int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, d_status, st);
   if (rc != RR_OK) return rc;
@@ -290,6 +298,9 @@ int rr_evaluate(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, void
     RR_CUDA(cudaEventRecord(ev[0], st));
   }
   if (ctx->work[0].lazy && (rc = rr_ld_rows_launch(ctx, &ctx->work[0], npv, st)) != RR_OK) return rc;
+  if (ctx->work[0].lazy && ctx->k_small > 0.0 &&
+      (rc = rr_ld_rows_small_launch(ctx, &ctx->work[0], npv, st)) != RR_OK)
+    return rc;
   if (timed) RR_CUDA(cudaEventRecord(ev[1], st));
   rc = rr_flux_launch(ctx, &ctx->work[0], npv, d_flux, st);
   if (timed) RR_CUDA(cudaEventRecord(ev[2], st));
@@ -383,6 +394,8 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
     }
     if ((rc = rr_pv_prep_launch(ctx, wk, d_pv, nv, d_status, st)) != RR_OK) break;
     if (wk->lazy && (rc = rr_ld_rows_launch(ctx, wk, nv, st)) != RR_OK) break;
+    if (wk->lazy && ctx->k_small > 0.0 && (rc = rr_ld_rows_small_launch(ctx, wk, nv, st)) != RR_OK)
+      break;
     if ((rc = rr_flux_launch(ctx, wk, nv, d_flux, st)) != RR_OK) break;
     RR_CUDA(cudaMemcpyAsync((char *)h_flux + v0 * flux_row, d_flux, nv * flux_row,
                             cudaMemcpyDeviceToHost, st));

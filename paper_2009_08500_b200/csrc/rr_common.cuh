@@ -111,6 +111,7 @@ struct rr_ctx {
   int32_t any_shuffle;
   int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL | RR_TABLE_DIRECT
   int32_t mean_k;       // 1: LD weights at the mean k of the passbands
+  double k_small;       // small-planet approximation for kw <= k_small; 0: off
   // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
   RRWork work[3];
   // counters / accounting
@@ -151,6 +152,7 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
 int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_ld_table.cu
 int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st);         // rr_ld_table.cu
 int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_geometry.cu
+int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);   // rr_geometry.cu
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
                       int32_t *d_status, cudaStream_t st);                     // rr_flux.cu

@@ -159,6 +159,60 @@ int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t 
   return RR_OK;
 }
 
+// ---- small-planet approximation (reading R14) ---------------------
+// Rows whose weight radius kw is <= the threshold take, at node g_ig, the profile's value at the
+// planet's centre z = g_ig (1+kw): linear interpolation of ldp over the bin means zm, constant
+// before the first and after the last node.  Runs after the row builder of the current mode and
+// overwrites those rows (one warp per row, lanes over g nodes, binary search in zm).
+template <typename TR>
+__global__ void __launch_bounds__(256)
+rr_ld_rows_small_kernel(const TR *__restrict__ ldp, const double *__restrict__ zm,
+                        const RRPvBand *__restrict__ pvb, TR *__restrict__ rows, double k_small,
+                        int64_t M, int npb, int nkpb, int ng, int nz) {
+  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  const int64_t v = row / npb;
+  const int pb = (int)(row - v * npb);
+  const double k = pvb[v * nkpb + (nkpb == 1 ? 0 : pb)].kw;
+  if (!(k <= k_small)) return;
+  const TR *pr = ldp + row * nz;
+  for (int ig = lane; ig < ng; ig += 32) {
+    const double z = (ig == ng - 1) ? 1.0 + k : ((double)ig / (double)(ng - 1)) * (1.0 + k);
+    double out;
+    if (z <= zm[0]) {
+      out = (double)pr[0];
+    } else if (z >= zm[nz - 1]) {
+      out = (double)pr[nz - 1];
+    } else {
+      int lo = 0, hi = nz - 1;                     // zm[lo] <= z < zm[hi]
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (zm[mid] <= z) lo = mid; else hi = mid;
+      }
+      const double a = (z - zm[lo]) / (zm[lo + 1] - zm[lo]);
+      out = (1.0 - a) * (double)pr[lo] + a * (double)pr[lo + 1];
+    }
+    rows[row * ng + ig] = (TR)out;
+  }
+}
+
+int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t M = npv * c.npb;
+  const unsigned grid = (unsigned)((M * 32 + 255) / 256);
+  if (c.precision == RR_FP32)
+    rr_ld_rows_small_kernel<float><<<grid, 256, 0, st>>>(
+        (const float *)wk->ldp_src, ctx->d_zm, wk->pvb, (float *)wk->rows, ctx->k_small, M, c.npb,
+        c.nkpb, c.ng, ctx->nz);
+  else
+    rr_ld_rows_small_kernel<double><<<grid, 256, 0, st>>>(
+        (const double *)wk->ldp_src, ctx->d_zm, wk->pvb, (double *)wk->rows, ctx->k_small, M, c.npb,
+        c.nkpb, c.ng, ctx->nz);
+  RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
 int rr_geometry_build(rr_ctx *ctx) {
   const rr_config &c = ctx->cfg;
   int nz = ctx->nz;

@@ -254,6 +254,39 @@ def test_mean_k_weights_shortcut(rr, mode):
     gm.close()
 
 
+@pytest.mark.parametrize("mode,precision", [(2, 0), (0, 0), (2, 1)])
+def test_small_planet_approximation(rr, mode, precision):
+    """PAPER.md:184-186 (reading R14): pvs with k <= threshold take the profile at the planet's
+    centre; the others are untouched.  Direct mode: every pv against the direct oracle with the
+    same threshold.  Lazy mode: small pvs against that oracle, the rest against the table oracle."""
+    wl = workloads.make_workload(4, npv=60, npt=3000)
+    thr = 0.08
+    small = wl.pv[:, 0] <= thr
+    assert 5 < small.sum() < 55
+    od = oracle.OracleDirectModel.from_config(wl.model)
+    want_d, _ = od.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                            wl.exposure_time, wl.pv, wl.ldp(od.mu), nthreads=0, small_planet_k=thr)
+    want_t, _ = oracle_flux(wl)
+    gm = rr.RoadRunner.from_config(wl.model, precision)
+    rr.rr_set_table_mode(gm.ctx, mode)
+    rr.rr_set_small_planet(gm.ctx, thr)
+    gm.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    got = gm.evaluate(wl.pv).cpu().numpy().astype(np.float64)
+    tol = TOL32 if precision else TOL64
+    assert np.max(np.abs(got[small] - want_d[small])) <= tol
+    ref = want_d if mode == 2 else want_t
+    assert np.max(np.abs(got[~small] - ref[~small])) <= tol
+    assert np.max(np.abs(want_d[small] - want_t[small])) > 1e-7     # the approximation is visible
+    if mode == 0:                                                   # a full table cannot do it
+        rr.rr_set_table_mode(gm.ctx, rr.RR_TABLE_FULL)
+        gm.build_ld_table(wl.ldp(gm.mu))
+        with pytest.raises(rr.RoadRunnerError) as e:
+            gm.evaluate(wl.pv)
+        assert e.value.code == -5
+    gm.close()
+
+
 def test_kernel_timing_counts_calls(rr):
     wl = small_workload(1)
     gm = gpu_model(rr, wl)

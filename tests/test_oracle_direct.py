@@ -126,3 +126,45 @@ def test_mean_k_weights_equal_k_is_identity_and_small_otherwise():
             d = float(np.max(np.abs(a - b)))
             assert lo < d <= hi, (spread, model, d)
             assert (a < 1).sum() > 100
+
+
+# ---- small-planet approximation (reading R14) ---------------------------------------
+def test_profile_at_is_the_library_interpolant():
+    """oracle_profile_at = numpy.interp over the bin means (linear, constant beyond the end nodes)."""
+    m = oracle.OracleDirectModel()
+    rng = np.random.default_rng(4)
+    ld = np.sort(rng.uniform(0.1, 1.0, m.nz))[::-1].copy()
+    for z in np.concatenate([rng.uniform(0, 1.3, 300), m.zm[[0, 1, 50, -2, -1]], [0.0, 1.0]]):
+        assert abs(oracle.profile_at(z, m.zm, ld) - float(np.interp(z, m.zm, ld))) < 1e-15
+
+
+def test_small_planet_rows_and_threshold():
+    """Rows with k <= threshold hold the profile at the planet's centre z = g (1+k); rows above the
+    threshold are the direct-model rows, bit for bit."""
+    m = oracle.OracleDirectModel()
+    ld = truth.power2(0.6, 0.7)(m.mu)
+    pv = np.array([[0.01, 0, 3, 8, 1.5, 0, 0], [0.05, 0, 3, 8, 1.5, 0, 0]])
+    ldp = np.stack([ld, ld])[:, None, :]
+    plain, _ = m.rows(ldp, pv)
+    sp, _ = m.rows(ldp, pv, small_planet_k=0.02)
+    assert np.array_equal(sp[1], plain[1])
+    g = np.arange(m.ng) / (m.ng - 1)
+    g[-1] = 1.0
+    assert np.max(np.abs(sp[0, 0] - np.interp(g * 1.01, m.zm, ld))) < 1e-15
+    assert sp[0, 0, -1] == ld[-1]                                  # centre beyond the limb: R5
+
+
+def test_small_planet_is_close_to_the_direct_model_inside_the_disc():
+    """'If the planet is small enough': k = 0.01, centre at z <= 0.8: the flux moves by < 5e-8
+    (depth 1e-4); at the limb the approximation is poor, which is why it has a threshold."""
+    m = oracle.OracleDirectModel()
+    ld = truth.quadratic(0.4, 0.2)(m.mu)
+    k = 0.01
+    pv = np.array([[k, 0, 3, 8, 1.5, 0, 0]])
+    a, ist = m.rows(ld, pv)
+    b, _ = m.rows(ld, pv, small_planet_k=0.02)
+    inner = max(abs(oracle.flux_from_row(z, k, a[0, 0], ist[0, 0])
+                    - oracle.flux_from_row(z, k, b[0, 0], ist[0, 0])) for z in np.linspace(0, 0.8, 81))
+    limb = max(abs(oracle.flux_from_row(z, k, a[0, 0], ist[0, 0])
+                   - oracle.flux_from_row(z, k, b[0, 0], ist[0, 0])) for z in np.linspace(0.97, 1.009, 40))
+    assert 0 < inner < 5e-8 and limb > inner
