@@ -323,7 +323,11 @@ def run_ours(args):
     alg_bytes = (wl.npv * wl.npt * es + wl.npt * 12 + nrows * (2 * wl.model.ng + 1) * es
                  + wl.npv * 184)
     t_flux = ms_flux * 1e-3
-    ops = ALG_OPS[args.precision]
+    ops = dict(ALG_OPS[args.precision])
+    if args.precision == "fp64":
+        # circular orbits: per exposure phase 5 + sin/cos polynomials 15, per sub-sample one plane
+        # rotation 4 + z^2 2
+        ops["circular"] = 6.0 + 20.0 * wl.npt / wl.evaluations_per_pv
     alg_fma = (counts["skipped"] * ops["skipped"] + counts["circular"] * ops["circular"]
                + counts["eccentric"] * ops["eccentric_fixed"]
                + counts["solver_iters"] * ops["solver_iter"]

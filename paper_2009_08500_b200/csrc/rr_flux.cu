@@ -170,6 +170,7 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
 // lets 4 blocks of 256 threads share an SM.
 enum {
   K_ZC0, K_ZC1,           // circular (pair)
+  K_CD, K_SD,             // circular: cos, sin of the phase step between sub-samples (pair)
   K_C4, K_C3,             // starter (pair)
   K_C2, K_KY,             // (pair)
   K_B, K_C,               // (pair)
@@ -188,7 +189,7 @@ enum {
   K_TOTAL,
   K_SMEM = (K_TOTAL + 3) & ~3   // 16-byte multiple in both precisions
 };
-static_assert(K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
+static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
 template <typename R> struct Cst {
   const volatile R *p;
   __device__ __forceinline__ R operator[](int i) const { return p[i]; }
@@ -204,10 +205,12 @@ template <typename R> struct Cst {
 };
 
 template <typename R>
-__device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, const RRPvBand &b) {
+__device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, const RRPvBand &b,
+                                                   double du) {
   const int t = threadIdx.x;
   double v = 0.0;
   switch (t) {
+    case K_CD: v = cospi(2.0 * du); break;   case K_SD: v = sinpi(2.0 * du); break;
     case K_ZC0: v = o.zc0; break;       case K_ZC1: v = o.zc1; break;
     case K_E: v = o.e; break;           case K_SE: v = o.sE; break;
     case K_CE: v = o.cE; break;         case K_A: v = o.A; break;
@@ -472,9 +475,44 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
         f = rr_nan<R>();
       } else {
         R acc = (R)0;
-        double w = wr + off0;
-        for (int s = 0; s < ns; ++s, w += du)
-          acc += rr_subsample<R, COUNT, CIRC>(w, u_mid, hwid, k, ldw, ng, cnt);
+        if (CIRC && sizeof(R) == 8) {
+          // circular orbit, fp64: sin and cos of the first sub-sample's phase, then one plane
+          // rotation per sub-sample (constant phase step); no per-sub-sample window test is
+          // needed, outside the window z >= 1+k by construction.  (fp32 keeps the polynomial per
+          // sub-sample: a rotation's ABSOLUTE rounding error times a is too much for z there.)
+          const double ur0 = (wr + off0) + u_mid;
+          R sn, cs;
+          if (fabs(ur0) <= 0.0795) {
+            R cm1;
+            rr_sincosm1_small((R)(RR_TWOPI * ur0), sn, cm1);
+            cs = (R)1 + cm1;
+          } else {
+            double s_, c_;
+            sincospi(2.0 * ur0, &s_, &c_);
+            sn = (R)s_;
+            cs = (R)c_;
+          }
+          R zc0, zc1, cd, sd;
+          k.pair(K_ZC0, zc0, zc1);
+          k.pair(K_CD, cd, sd);
+          const R opk2 = k[K_OPK2];
+          for (int s = 0; s < ns; ++s) {
+            const R z2 = fma(sn * sn, zc1, zc0);
+            if (cs > (R)0 && z2 < opk2) {
+              int ing = 0;
+              acc += rr_deficit<R>(z2, k, ldw, ng, ing);
+              if (COUNT) { cnt[3]++; cnt[4] += ing; }
+            }
+            const R s1 = fma(sn, cd, cs * sd);
+            cs = fma(cs, cd, -sn * sd);
+            sn = s1;
+          }
+          if (COUNT) cnt[1] += ns;
+        } else {
+          double w = wr + off0;
+          for (int s = 0; s < ns; ++s, w += du)
+            acc += rr_subsample<R, COUNT, CIRC>(w, u_mid, hwid, k, ldw, ng, cnt);
+        }
         f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
       out[i] = f;
@@ -607,7 +645,7 @@ rr_flux_kernel(const FluxParams P) {
             ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
           }
         }
-        rr_stage_constants<R>(cst, po, pb);
+        rr_stage_constants<R>(cst, po, pb, 2.0 * hw / lc.ns);
         if (threadIdx.x == K_COUNT)
           cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
         __syncthreads();
@@ -662,7 +700,7 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
     }
     RRPvBand nob = {};
     __syncthreads();
-    rr_stage_constants<R>(cst, po, nob);
+    rr_stage_constants<R>(cst, po, nob, 0.0);
     __syncthreads();
     const double hw = 0.5 * lc.exptime * po.inv_p;
     const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0);
