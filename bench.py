@@ -353,6 +353,7 @@ def run_ours(args):
         "ld_table_parts_ms": {"rr_build_ld_table": ms_table, "rows_in_rr_evaluate": ms_rows},
         "rr_evaluate_ms": ms_eval, "table_mode": args.table_mode,
         "algorithmic_bytes": int(alg_bytes), "algorithmic_fma": int(alg_fma),
+        "algorithmic_ops_per_unit": ops,
         "hbm_frac": hbm_achieved / hbm_peak, "alu_frac": alu_achieved / alu_peak_tflops,
         "fma_peak_measured_live_tflops": 2.0 * fma_live / 1e12,
         "class_counts": counts,
