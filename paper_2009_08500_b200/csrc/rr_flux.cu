@@ -428,11 +428,12 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 
 // Occulted light of the sub-sample at phase w (turns, measured from the window centre).
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
-template <typename R, bool COUNT, bool CIRC>
+template <typename R, bool COUNT, bool CIRC, bool NOWRAP>
 __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
                                           const Cst<R> k, const R *__restrict__ ldw, int ng,
                                           unsigned long long *cnt) {
-  const double wr = w - rr_round(w);
+  // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
+  const double wr = NOWRAP ? w : w - rr_round(w);
   R def = (R)0;
   if (fabs(wr) <= hwid) {
     bool front;
@@ -450,7 +451,7 @@ __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
 }
 
 // The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
-template <typename R, bool COUNT, bool CIRC>
+template <typename R, bool COUNT, bool CIRC, bool NOWRAP>
 __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__restrict__ out,
                                         int count, int ns, int shuffle, double t0, double inv_p,
                                         double u_mid, double hwid, double hw, R scale,
@@ -511,7 +512,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC>(w, u_mid, hwid, k, ldw, ng, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP>(w, u_mid, hwid, k, ldw, ng, cnt);
         }
         f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
@@ -534,7 +535,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
         if (fabs(wr) <= hskip) {
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
-            acc += rr_subsample<R, COUNT, CIRC>(fma(du, (double)s, w0), u_mid, hwid, k, ldw, ng,
+            acc += rr_subsample<R, COUNT, CIRC, false>(fma(du, (double)s, w0), u_mid, hwid, k, ldw, ng,
                                                 cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
@@ -653,12 +654,16 @@ rr_flux_kernel(const FluxParams P) {
         staged_lc = tlc;
       }
       const int shuffle = lc.ns >= P.shuffle_min_ns;
+      const bool nowrap = hwid + 2.0 * hw < 0.499;
       if (circular)
-        rr_tile<R, COUNT, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0, inv_p,
-                                u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+        rr_tile<R, COUNT, true, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                       inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+      else if (nowrap)
+        rr_tile<R, COUNT, false, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                       inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
       else
-        rr_tile<R, COUNT, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0, inv_p,
-                                 u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+        rr_tile<R, COUNT, false, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                        inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
     }
   }
   if (f0 >= 0) rr_fill<R>(row + f0, f1 - f0, (R)1);
