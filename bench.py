@@ -40,7 +40,7 @@ FP64_LANES_PER_SM, FP32_LANES_PER_SM, SM_COUNT = 64, 128, 148
 # merged out-of-window fill runs cost no arithmetic.
 ALG_OPS = {
     "fp64": dict(skipped=2, circular=16, eccentric_fixed=26, solver_iter=31, occulting=18,
-                 ingress=68),
+                 ingress=64),
     "fp32": dict(skipped=4, circular=19, eccentric_fixed=32, solver_iter=24, occulting=11,
                  ingress=61),
 }

@@ -370,7 +370,12 @@ __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restric
     R opk, k2;
     k.pair(K_OPK, opk, k2);
     R kite = rr_sqrt((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk));
-    R th1 = rr_atan2_pos(kite, fma(z - kk, z + kk, (R)1));
+    // half-angle at the star's centre: at most asin k, so for k <= sin(pi/8) (block-uniform) its
+    // tangent needs no octant reduction
+    const R x1 = fma(z - kk, z + kk, (R)1);
+    R th1;
+    if (k2 <= (R)0.1464) th1 = rr_atan_small(kite, x1);
+    else th1 = rr_atan2_pos(kite, x1);
     R th2 = rr_atan2_pos(kite, fma(z - (R)1, z + (R)1, k2));
     ap = th1 + k2 * th2 - (R)0.5 * kite;
     ++ningress;
