@@ -470,6 +470,38 @@ def test_grazing_wide_window_and_secondary_eclipse(rr):
         gm.close()
 
 
+@pytest.mark.parametrize("precision", [0, 1])
+def test_long_exposures_many_subsamples_and_distant_epochs(rr, precision):
+    """Degenerate corners of the supersampling path: an exposure longer than half the period (the
+    phase of its sub-samples wraps), ns = 1000 sub-samples in one exposure (both reduction layouts
+    through RR_REDUCE_AUTO), and epochs hundreds of periods away from t0."""
+    mc = workloads.ModelConfig()
+    pv = np.array([
+        [0.1, 0.0, 1.0, 6.0, np.deg2rad(88.0), 0.0, 0.0],
+        [0.15, 0.05, 1.3, 5.0, np.deg2rad(86.0), 0.4, 2.0],
+        [0.05, -0.1, 2.7, 9.0, np.deg2rad(89.0), 0.2, 5.0],
+        [0.2, 0.2, 0.8, 3.0, np.deg2rad(80.0), 0.6, 0.3],
+    ])
+    coeffs = np.tile(np.array([[[0.4, 0.25]]]), (pv.shape[0], 1, 1))
+    t_a = np.linspace(-0.6, 0.6, 300)                     # lc 0: exposure 0.7 d > p/2 for pv 0, 3
+    t_b = np.linspace(-0.05, 0.05, 7)                     # lc 1: ns = 1000
+    t_c = 300.0 * 1.3 + np.linspace(-0.1, 0.1, 400)       # lc 2: 300 periods of pv 1 later
+    times = np.concatenate([t_a, t_b, t_c])
+    lc = np.concatenate([np.zeros(300), np.ones(7), np.full(400, 2)]).astype(np.int32)
+    pbs, nss, ets = [0, 0, 0], [9, 1000, 2], [0.7, 0.02, 0.001]
+    om = oracle.OracleModel.from_config(mc)
+    om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+    want, _ = om.evaluate(times, lc, pbs, nss, ets, pv, nthreads=0)
+    gm = rr.RoadRunner.from_config(mc, precision)
+    gm.set_data(times, lc, pbs, nss, ets)
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy().astype(np.float64)
+    # 300 periods away the phase itself carries 300 * eps of rounding: ~1e-13 in z, no more
+    assert np.max(np.abs(got - want)) <= (TOL32 if precision else TOL64)
+    assert (want[:, :300] < 1).sum() > 200 and (want[:, 307:] < 1).sum() > 50
+    gm.close()
+
+
 def test_uniform_disk_closed_form(rr):
     """ldp = 1: flux = 1 - a(z,k)/pi straight from the CUDA path."""
     wl = workloads.make_workload(1, npv=8, npt=2000)
