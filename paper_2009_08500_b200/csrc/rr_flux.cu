@@ -191,16 +191,41 @@ enum {
 };
 static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
 template <typename R> struct Cst {
-  const volatile R *p;
-  __device__ __forceinline__ R operator[](int i) const { return p[i]; }
+  unsigned base;   // 32-bit shared-window address of cst[0]
+  __device__ __forceinline__ explicit Cst(const R *cst) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(cst);
+    // fp32 has a register to spare: an opaque move keeps the address instead of rematerialising it
+    // at every load; in fp64 (64-register budget) holding it costs more than recomputing (measured)
+    if constexpr (sizeof(R) == 4) asm volatile("mov.u32 %0, %1;" : "=r"(base) : "r"(a));
+    else base = a;
+  }
+  __device__ __forceinline__ R operator[](int i) const {
+    R v;
+    if constexpr (sizeof(R) == 8)
+      asm volatile("ld.volatile.shared.f64 %0, [%1];" : "=d"(v) : "r"(base + 8u * i));
+    else
+      asm volatile("ld.volatile.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + 4u * i));
+    return v;
+  }
+  // the two table nodes ldw[ig], ldw[ig+1] of the row staged K_SMEM elements after the constants
+  __device__ __forceinline__ void nodes(int ig, R &l0, R &l1) const {
+    const unsigned a = base + (unsigned)sizeof(R) * (unsigned)(K_SMEM + ig);
+    if constexpr (sizeof(R) == 8) {
+      asm volatile("ld.shared.f64 %0, [%1];" : "=d"(l0) : "r"(a));
+      asm volatile("ld.shared.f64 %0, [%1+8];" : "=d"(l1) : "r"(a));
+    } else {
+      asm volatile("ld.shared.f32 %0, [%1];" : "=f"(l0) : "r"(a));
+      asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(l1) : "r"(a));
+    }
+  }
   // two neighbouring constants (i even) with one 16-/8-byte shared load
   __device__ __forceinline__ void pair(int i, double &a, double &b) const {
-    unsigned addr = (unsigned)__cvta_generic_to_shared(const_cast<const R *>(p) + i);
-    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "r"(addr));
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];"
+                 : "=d"(a), "=d"(b) : "r"(base + 8u * i));
   }
   __device__ __forceinline__ void pair(int i, float &a, float &b) const {
-    unsigned addr = (unsigned)__cvta_generic_to_shared(const_cast<const R *>(p) + i);
-    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(a), "=f"(b) : "r"(addr));
+    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];"
+                 : "=f"(a), "=f"(b) : "r"(base + 4u * i));
   }
 };
 
@@ -357,7 +382,8 @@ __device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restric
   R gscale, kk;
   k.pair(K_GSCALE, gscale, kk);
   rr_cell(z * gscale, ig, ag);
-  R l0 = ldw[ig], l1 = ldw[ig + 1];
+  R l0, l1;
+  k.nodes(ig, l0, l1);              // = ldw[ig], ldw[ig + 1]
   R ip = fma(ag, l1 - l0, l0);              // mean occulted brightness
   R ap;
   R omk2, afull;
@@ -563,7 +589,7 @@ rr_flux_kernel(const FluxParams P) {
   extern __shared__ __align__(16) unsigned char rr_smem[];
   R *cst = reinterpret_cast<R *>(rr_smem);             // fixed offsets: immediates in the loads
   R *ldw = cst + K_SMEM;
-  const Cst<R> k{cst};
+  const Cst<R> k(cst);
   __shared__ unsigned tflags[FT / 32];
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
@@ -693,7 +719,7 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
                 const RRLc *__restrict__ lcs, const RRPvOrbit *__restrict__ pvo, int64_t ntiles,
                 int64_t npv, int64_t nsub, double *__restrict__ zout) {
   __shared__ __align__(16) R cst[K_TOTAL];
-  const Cst<R> k{cst};
+  const Cst<R> k(cst);
   const int64_t total = ntiles * npv;
   for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
     const int64_t v = w / ntiles;
