@@ -66,6 +66,18 @@ extern "C" {
                                 rr_evaluate the weights are computed at each pv's own k and contracted
                                 with its profile (g interpolation only); any k > 0 is valid        */
 
+/* named limb-darkening laws (rr_build_ld_table_law); x = 1 - mu */
+#define RR_LD_UNIFORM       0  /* I = 1                                                nldc 0  */
+#define RR_LD_LINEAR        1  /* 1 - u x                                                   1  */
+#define RR_LD_QUADRATIC     2  /* 1 - u1 x - u2 x^2                                         2  */
+#define RR_LD_QUADRATIC_TRI 3  /* quadratic with u1 = 2 sqrt(q1) q2, u2 = sqrt(q1)(1 - 2 q2) 2  */
+#define RR_LD_GENERAL       4  /* 1 - sum_{n=1..N} c_n (1 - mu^n)                        N<=64  */
+#define RR_LD_NONLINEAR     5  /* 1 - sum_{n=1..4} c_n (1 - mu^(n/2))                       4  */
+#define RR_LD_LOGARITHMIC   6  /* 1 - u1 x - u2 mu ln mu                                    2  */
+#define RR_LD_EXPONENTIAL   7  /* 1 - u1 x - u2 / (1 - e^mu)   (Istar by reading R6)        2  */
+#define RR_LD_POWER2        8  /* 1 - c (1 - mu^alpha)                                      2  */
+#define RR_LD_POWER2_PM     9  /* power-2 with c = 1 - h1 + h2, alpha = log2(c / h2)        2  */
+
 /* supersample reduction layout of the fused flux kernel (rr_set_reduction) */
 #define RR_REDUCE_AUTO    0  /* library picks per light curve from ns and the amount of work    */
 #define RR_REDUCE_THREAD  1  /* one thread per exposure, in-thread loop over its sub-samples    */
@@ -133,6 +145,14 @@ int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, i
  * Both give the same flux to rounding (tested).  Buffers are owned by ctx and grown as needed.   */
 int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64_t npv,
                       void *stream);
+/* Named laws on the device: evaluates the law RR_LD_* with the
+ * coefficients d_ldc[npv][npb][nldc] (fp64, device) at mu[nz] into a profile buffer owned by ctx,
+ * takes Istar = 2 pi int_0^1 mu I dmu in closed form ("integrated analytically", PAPER.md:156;
+ * RR_LD_EXPONENTIAL has none: reading R6), and then behaves as rr_build_ld_table in the current
+ * table mode.  The paper names the laws without printing them: the forms above are the textbook
+ * ones of its footnote 4.  RR_ESIZE if nldc does not fit the law.  Synchronous on `stream`.      */
+int rr_build_ld_table_law(rr_ctx *ctx, int32_t law, const double *d_ldc, int32_t nldc, int64_t npv,
+                          void *stream);
 /* RR_TABLE_*; takes effect at the next rr_build_ld_table.  RR_TABLE_DIRECT needs nz <= 2000.     */
 int rr_set_table_mode(rr_ctx *ctx, int32_t mode);
 /* Transmission-spectroscopy shortcut (meaningful with nkpb = npb): on != 0 takes

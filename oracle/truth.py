@@ -45,6 +45,47 @@ def istar_poly(coeffs):
     return np.pi * (1 + sum(2 * cn / ((n + 2) * (n + 3)) for n, cn in enumerate(coeffs)))
 
 
+# The named laws of PAPER.md:143-156 (the paper lists the names and cites their sources; forms are
+# the textbook ones) as callables of mu and their closed-form disc integrals, pinned against
+# mpmath quadrature in tests/test_oracle_direct.py.  name -> (callable factory, Istar or None).
+def law(name, c):
+    c = [float(x) for x in c]
+    if name == "uniform":
+        return (lambda mu: 1 + 0 * mu), np.pi
+    if name == "linear":
+        return (lambda mu: 1 - c[0] * (1 - mu)), np.pi * (1 - c[0] / 3)
+    if name == "quadratic":
+        return quadratic(*c), istar_quadratic(*c)
+    if name == "quadratic-tri":                       # Kipping (2013)
+        u1, u2 = 2 * c[0] ** 0.5 * c[1], c[0] ** 0.5 * (1 - 2 * c[1])
+        return quadratic(u1, u2), istar_quadratic(u1, u2)
+    if name == "general":                             # 1 - sum_n c_n (1 - mu^n), n = 1..N
+        return (lambda mu: 1 - sum(cn * (1 - mu ** (n + 1)) for n, cn in enumerate(c)),
+                np.pi * (1 - sum(cn * (n + 1) / (n + 3) for n, cn in enumerate(c))))
+    if name == "nonlinear":                           # Claret (2000), four coefficients
+        return (lambda mu: 1 - sum(cn * (1 - mu ** ((n + 1) / 2)) for n, cn in enumerate(c)),
+                np.pi * (1 - sum(cn * (n + 1) / (n + 5) for n, cn in enumerate(c))))
+    if name == "logarithmic":
+        def f(mu):
+            if isinstance(mu, np.ndarray):
+                safe = np.where(mu > 0, mu, 1.0)
+                return 1 - c[0] * (1 - mu) - c[1] * np.where(mu > 0, mu * np.log(safe), 0.0)
+            return 1 - c[0] * (1 - mu) - c[1] * (mu * mp.log(mu) if mu > 0 else 0)
+        return f, np.pi * (1 - c[0] / 3 + 2 * c[1] / 9)
+    if name == "exponential":
+        def f(mu):
+            e = np.exp(mu) if isinstance(mu, np.ndarray) else mp.exp(mu)
+            return 1 - c[0] * (1 - mu) - c[1] / (1 - e)
+        return f, None
+    if name == "power-2":
+        return power2(*c), istar_power2(*c)
+    if name == "power-2-pm":                          # Maxted (2018)
+        cc = 1 - c[0] + c[1]
+        al = float(np.log2(cc / c[1]))
+        return power2(cc, al), istar_power2(cc, al)
+    raise ValueError(name)
+
+
 def istar_mp(ld, dps=30):
     with mp.workdps(dps):
         return 2 * mp.pi * mp.quad(lambda mu: mu * ld(mu), [0, 1])

@@ -23,6 +23,8 @@ from . import build as _build
 RR_FP64, RR_FP32 = 0, 1
 RR_REDUCE_AUTO, RR_REDUCE_THREAD, RR_REDUCE_SHUFFLE = 0, 1, 2
 RR_TABLE_LAZY, RR_TABLE_FULL, RR_TABLE_DIRECT = 0, 1, 2
+LD_LAWS = {"uniform": 0, "linear": 1, "quadratic": 2, "quadratic-tri": 3, "general": 4,
+           "nonlinear": 5, "logarithmic": 6, "exponential": 7, "power-2": 8, "power-2-pm": 9}
 RR_PV_K_RANGE, RR_PV_E_RANGE, RR_PV_A_RANGE, RR_PV_P_RANGE, RR_PV_NONFINITE = 1, 2, 4, 8, 16
 
 # every symbol include/roadrunner.h declares (tests check the library exports each of them)
@@ -34,7 +36,7 @@ SYMBOLS = (
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
-    "rr_set_small_planet",
+    "rr_set_small_planet", "rr_build_ld_table_law",
 )
 
 
@@ -97,6 +99,7 @@ def load() -> C.CDLL:
         "rr_get_rows": (C.c_int, [_VP, _VP]),
         "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
         "rr_set_small_planet": (C.c_int, [_VP, _DBL]),
+        "rr_build_ld_table_law": (C.c_int, [_VP, _I32, _VP, _I32, _I64, _VP]),
         "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
         "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
@@ -187,6 +190,17 @@ def rr_build_ld_table(ctx: int, ldp, npv: int, istar=None, stream=None):
     _check(load().rr_build_ld_table(ctx, _dev(ldp, ldp.dtype, "ldp"),
                                     None if istar is None else _dev(istar, ldp.dtype, "istar"),
                                     npv, _stream(stream)), "rr_build_ld_table")
+
+
+def rr_build_ld_table_law(ctx: int, law, ldc, npv: int, stream=None):
+    """law: RR_LD_* code or a name of LD_LAWS; ldc f64 CUDA tensor [npv][npb][nldc] (or None for
+    the uniform law)."""
+    import torch
+    code = LD_LAWS[law] if isinstance(law, str) else int(law)
+    nldc = 0 if ldc is None else int(ldc.shape[-1])
+    _check(load().rr_build_ld_table_law(ctx, code,
+                                        None if ldc is None else _dev(ldc, torch.float64, "ldc"),
+                                        nldc, npv, _stream(stream)), "rr_build_ld_table_law")
 
 
 def rr_evaluate(ctx: int, pv, flux, status=None, stream=None):
@@ -359,6 +373,23 @@ class RoadRunner:
             istar = torch.as_tensor(np.ascontiguousarray(istar)).to(self.dtype).cuda()
         self.npv = ldp.shape[0]
         rr_build_ld_table(self.ctx, ldp, self.npv, istar)
+
+    def build_ld_table_law(self, law, ldc):
+        """Named law on the device: ldc array or CUDA tensor [npv][npb][nldc] (fp64)."""
+        import torch
+        if ldc is not None and not isinstance(ldc, torch.Tensor):
+            ldc = torch.as_tensor(np.ascontiguousarray(ldc, np.float64)).cuda()
+        if ldc is not None:
+            ldc = ldc.reshape(-1, self.npb, ldc.shape[-1]).contiguous()
+        self.npv = int(ldc.shape[0]) if ldc is not None else self.npv
+        rr_build_ld_table_law(self.ctx, law, ldc, self.npv)
+
+    def profile_and_istar(self):
+        """Diagnostics: Istar[npv][npb] of the last table build (numpy)."""
+        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        I = np.empty((self.npv, self.npb), npdt)
+        _check(load().rr_get_table(self.ctx, None, I.ctypes.data), "rr_get_table")
+        return I
 
     def table(self):
         """Copy of T[npv][npb][nk][ng] and Istar[npv][npb] as numpy arrays (diagnostics)."""

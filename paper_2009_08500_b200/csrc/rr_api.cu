@@ -226,6 +226,16 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
   return rr_ld_table_launch(ctx, &ctx->work[0], d_ldp, d_istar, npv, (cudaStream_t)stream);
 }
 
+int rr_build_ld_table_law(rr_ctx *ctx, int32_t law, const double *d_ldc, int32_t nldc, int64_t npv,
+                          void *stream) {
+  if (!ctx || (!d_ldc && law != RR_LD_UNIFORM)) return RR_ENULL;
+  if (npv <= 0) return RR_ESIZE;
+  static const int need[] = {0, 1, 2, 2, -1, 4, 2, 2, 2, 2};
+  if (law < RR_LD_UNIFORM || law > RR_LD_POWER2_PM) return RR_ECONFIG;
+  if (need[law] >= 0 ? nldc != need[law] : (nldc < 1 || nldc > 64)) return RR_ESIZE;
+  return rr_ld_law_launch(ctx, &ctx->work[0], law, d_ldc, nldc, npv, (cudaStream_t)stream);
+}
+
 int rr_set_small_planet(rr_ctx *ctx, double k_threshold) {
   if (!ctx) return RR_ENULL;
   if (!(k_threshold >= 0.0) || !isfinite(k_threshold)) return RR_ECONFIG;

@@ -151,6 +151,8 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
                          int64_t npv, int copy, cudaStream_t st);              // rr_ld_table.cu
 int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_ld_table.cu
 int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st);         // rr_ld_table.cu
+int rr_ld_law_launch(rr_ctx *ctx, RRWork *wk, int law, const double *d_ldc, int nc, int64_t npv,
+                     cudaStream_t st);                                         // rr_ld_table.cu
 int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);  // rr_geometry.cu
 int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);   // rr_geometry.cu
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu

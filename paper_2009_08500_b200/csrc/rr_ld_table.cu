@@ -124,6 +124,85 @@ __global__ void rr_istar_kernel(const TA *__restrict__ A, const double *__restri
   if (lane == 0) out[row] = (TC)s;
 }
 
+// ---- named limb-darkening laws on the device --------------------
+// ldp[row][j] = I(mu_j; ldc[row]) and the analytic disc integral Istar = 2 pi int_0^1 mu I dmu
+// ("all integrated analytically over the stellar disk").  The paper names the laws
+// and cites their sources without printing them; the forms are the textbook ones, stated in
+// include/roadrunner.h.  One thread per (row, j); fp64 arithmetic, stored in the ctx precision.
+__device__ double rr_law_value(int law, const double *c, int nc, double mu) {
+  const double x = 1.0 - mu;
+  switch (law) {
+    case RR_LD_UNIFORM: return 1.0;
+    case RR_LD_LINEAR: return 1.0 - c[0] * x;
+    case RR_LD_QUADRATIC: return 1.0 - c[0] * x - c[1] * x * x;
+    case RR_LD_QUADRATIC_TRI: {
+      const double sq = sqrt(c[0]), u1 = 2.0 * sq * c[1], u2 = sq * (1.0 - 2.0 * c[1]);
+      return 1.0 - u1 * x - u2 * x * x;
+    }
+    case RR_LD_GENERAL: {
+      double s = 1.0, p = 1.0;
+      for (int n = 0; n < nc; ++n) { p *= mu; s -= c[n] * (1.0 - p); }       // 1 - mu^(n+1)
+      return s;
+    }
+    case RR_LD_NONLINEAR: {
+      const double r = sqrt(mu);
+      return 1.0 - c[0] * (1.0 - r) - c[1] * (1.0 - mu) - c[2] * (1.0 - mu * r) - c[3] * (1.0 - mu * mu);
+    }
+    case RR_LD_LOGARITHMIC: return 1.0 - c[0] * x - c[1] * (mu > 0.0 ? mu * log(mu) : 0.0);
+    case RR_LD_EXPONENTIAL: return 1.0 - c[0] * x - c[1] / (1.0 - exp(mu));
+    case RR_LD_POWER2: return 1.0 - c[0] * (1.0 - pow(mu, c[1]));
+    case RR_LD_POWER2_PM: {
+      const double cc = 1.0 - c[0] + c[1], al = log2(cc / c[1]);
+      return 1.0 - cc * (1.0 - pow(mu, al));
+    }
+    default: return 1.0;
+  }
+}
+
+// Istar / pi in closed form; < 0: none (the caller falls back to the discretised integral, R6).
+__device__ double rr_law_istar_over_pi(int law, const double *c, int nc) {
+  switch (law) {
+    case RR_LD_UNIFORM: return 1.0;
+    case RR_LD_LINEAR: return 1.0 - c[0] / 3.0;
+    case RR_LD_QUADRATIC: return 1.0 - c[0] / 3.0 - c[1] / 6.0;
+    case RR_LD_QUADRATIC_TRI: {
+      const double sq = sqrt(c[0]), u1 = 2.0 * sq * c[1], u2 = sq * (1.0 - 2.0 * c[1]);
+      return 1.0 - u1 / 3.0 - u2 / 6.0;
+    }
+    case RR_LD_GENERAL: {
+      double s = 1.0;
+      for (int n = 0; n < nc; ++n) s -= c[n] * (double)(n + 1) / (double)(n + 3);
+      return s;
+    }
+    case RR_LD_NONLINEAR:
+      return 1.0 - c[0] / 5.0 - c[1] / 3.0 - 3.0 * c[2] / 7.0 - c[3] / 2.0;
+    case RR_LD_LOGARITHMIC: return 1.0 - c[0] / 3.0 + 2.0 * c[1] / 9.0;
+    case RR_LD_POWER2: return 1.0 - c[0] * c[1] / (c[1] + 2.0);
+    case RR_LD_POWER2_PM: {
+      const double cc = 1.0 - c[0] + c[1], al = log2(cc / c[1]);
+      return 1.0 - cc * al / (al + 2.0);
+    }
+    default: return -1.0;
+  }
+}
+
+template <typename TR>
+__global__ void rr_ld_law_kernel(int law, const double *__restrict__ ldc, int nc,
+                                 const double *__restrict__ mu, int64_t M, int nz,
+                                 TR *__restrict__ ldp, TR *__restrict__ istar, int *no_closed_form) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= M * nz) return;
+  const int64_t row = idx / nz;
+  const int j = (int)(idx - row * nz);
+  const double *c = ldc + row * nc;
+  ldp[idx] = (TR)rr_law_value(law, c, nc, mu[j]);
+  if (j == 0) {
+    const double s = rr_law_istar_over_pi(law, c, nc);
+    if (s >= 0.0) istar[row] = (TR)(RR_PI * s);
+    else if (row == 0) *no_closed_form = 1;
+  }
+}
+
 // Lazy mode: the k-collapsed row of one (pv, passband),
 //   ldw[ig] = (1 - ak) sum_j W[ik][ig][j] ldp[j] + ak sum_j W[ik+1][ig][j] ldp[j]
 // for the pv's own k (ik, ak from the per-pv prep).  One block per (pv, passband); the profile sits
@@ -435,4 +514,43 @@ int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st) {
   RR_LAUNCH_CHECK(ctx);
   wk->have_full = 1;
   return RR_OK;
+}
+
+
+// Named law -> profile (into the ctx-owned copy) + analytic Istar, then as rr_build_ld_table.
+int rr_ld_law_launch(rr_ctx *ctx, RRWork *wk, int law, const double *d_ldc, int nc, int64_t npv,
+                     cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t M = npv * c.npb;
+  wk->table_npv = -1;
+  int rc = grow_buf(&wk->ldp, &wk->ldp_cap, M * ctx->nz * esz);
+  if (rc == RR_OK) rc = grow_buf(&wk->istar, &wk->istar_cap, M * esz);
+  void *given = nullptr;                           // analytic Istar, handed on as the override
+  int64_t given_cap = 0;
+  if (rc == RR_OK) rc = grow_buf(&given, &given_cap, M * esz + 16);
+  if (rc != RR_OK) return rc;
+  int *flag = (int *)((char *)given + M * esz);
+  RR_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+  const int64_t n = M * ctx->nz;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  if (c.precision == RR_FP32)
+    rr_ld_law_kernel<float><<<grid, 256, 0, st>>>(law, d_ldc, nc, ctx->d_mu, M, ctx->nz,
+                                                  (float *)wk->ldp, (float *)given, flag);
+  else
+    rr_ld_law_kernel<double><<<grid, 256, 0, st>>>(law, d_ldc, nc, ctx->d_mu, M, ctx->nz,
+                                                   (double *)wk->ldp, (double *)given, flag);
+  RR_LAUNCH_CHECK(ctx);
+  int h_flag = 0;
+  RR_CUDA(cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+  RR_CUDA(cudaStreamSynchronize(st));
+  const void *ist = h_flag ? nullptr : given;      // no closed form: discretised integral (R6)
+  if (ctx->table_mode != RR_TABLE_FULL && ctx->nz <= 2000)
+    rc = rr_ld_profile_launch(ctx, wk, wk->ldp, ist, npv, 0, st);
+  else
+    rc = rr_ld_table_launch(ctx, wk, wk->ldp, ist, npv, st);
+  if (rc == RR_OK && wk->lazy) wk->ldp_src = wk->ldp;
+  cudaStreamSynchronize(st);
+  cudaFree(given);
+  return rc;
 }

@@ -287,6 +287,64 @@ def test_small_planet_approximation(rr, mode, precision):
     gm.close()
 
 
+# ---- named laws on the device (NEXT-4) ------------------------------------------------------------------
+LAWS = [("uniform", None), ("linear", [(0.2, 0.8)]), ("quadratic", [(0.1, 0.6), (0.0, 0.3)]),
+        ("quadratic-tri", [(0.1, 0.8), (0.1, 0.5)]), ("general", [(0.1, 0.4), (0.0, 0.2), (-0.1, 0.1)]),
+        ("nonlinear", [(0.1, 0.5), (-0.2, 0.2), (0.1, 0.4), (-0.2, 0.1)]),
+        ("logarithmic", [(0.3, 0.7), (0.0, 0.3)]), ("exponential", [(0.3, 0.6), (0.0, 0.02)]),
+        ("power-2", [(0.3, 0.9), (0.3, 1.2)]), ("power-2-pm", [(0.6, 0.8), (0.35, 0.55)])]
+
+
+@pytest.mark.parametrize("name,ranges", LAWS)
+@pytest.mark.parametrize("precision", [0, 1])
+def test_named_laws_on_device(rr, name, ranges, precision):
+    """rr_build_ld_table_law: the law evaluated on the device at the library's mu grid with its
+    closed-form Istar, against the test harness's statement of the same law
+    (oracle/truth.py, disc integrals pinned to quadrature) fed through the table oracle."""
+    from oracle import truth
+    mc = workloads.ModelConfig(npb=2)
+    base = workloads.make_workload(1, npv=7, npt=10)
+    rng = np.random.default_rng(12)
+    ldc = None if ranges is None else np.stack(
+        [rng.uniform(lo, hi, (7, 2)) for lo, hi in ranges], axis=-1)
+    times = np.tile(np.linspace(-0.2, 0.2, 800), 2)
+    lc = np.repeat(np.arange(2, dtype=np.int32), 800)
+    om = oracle.OracleModel.from_config(mc)
+    ldp = np.empty((7, 2, om.nz))
+    ist = np.empty((7, 2))
+    for v in range(7):
+        for b in range(2):
+            f, i0 = truth.law(name, [] if ldc is None else ldc[v, b])
+            ldp[v, b] = f(om.mu)
+            ist[v, b] = np.nan if i0 is None else i0
+    closed = not np.isnan(ist).any()
+    om.build_ld_table(ldp, istar_override=ist if closed else None)
+    want, _ = om.evaluate(times, lc, [0, 1], [1, 2], [0.0, 0.01], base.pv)
+    gm = rr.RoadRunner.from_config(mc, precision)
+    gm.set_data(times, lc, [0, 1], [1, 2], [0.0, 0.01])
+    gm.npv = 7
+    gm.build_ld_table_law(name, ldc)
+    got = gm.evaluate(base.pv).cpu().numpy().astype(np.float64)
+    I_g = gm.profile_and_istar().astype(np.float64)
+    assert np.max(np.abs(I_g / om.istar - 1.0)) <= (3e-7 if precision else 1e-13)
+    assert np.max(np.abs(got - want)) <= (TOL32 if precision else TOL64)
+    assert (want < 1).sum() > 200
+    gm.close()
+
+
+def test_named_law_argument_errors(rr):
+    import torch
+    gm = rr.RoadRunner()
+    ldc = torch.zeros((3, 1, 3), dtype=torch.float64, device="cuda")
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_build_ld_table_law(gm.ctx, "quadratic", ldc, 3)      # needs 2 coefficients
+    assert e.value.code == -3
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_build_ld_table_law(gm.ctx, 17, ldc, 3)
+    assert e.value.code == -2
+    gm.close()
+
+
 def test_kernel_timing_counts_calls(rr):
     wl = small_workload(1)
     gm = gpu_model(rr, wl)
