@@ -53,7 +53,8 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
-    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"])
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
+                    help="mixed = fp32 z and Ip*Ap, fp64 averaging / subtraction / flux (PAPER.md:293)")
     ap.add_argument("--npv", type=int, default=None, help="shrink the population (debugging)")
     ap.add_argument("--npt", type=int, default=None, help="shrink the time axis (debugging)")
     ap.add_argument("--table-mode", default="lazy", choices=["lazy", "full", "direct"],
@@ -207,8 +208,8 @@ def run_ours(args):
         shard.init_process_group("nccl")
     rr.load()
 
-    precision = rr.RR_FP32 if args.precision == "fp32" else rr.RR_FP64
-    npdt = np.float32 if precision == rr.RR_FP32 else np.float64
+    precision = {"fp64": rr.RR_FP64, "fp32": rr.RR_FP32, "mixed": rr.RR_MIXED}[args.precision]
+    npdt = np.float32 if precision != rr.RR_FP64 else np.float64
     wl = workloads.make_workload(args.config, npv=args.npv, npt=args.npt)
     if rank:   # weak scaling: every rank gets a full population, rotated so that data differ
         sh = (rank * 97) % wl.npv
@@ -222,7 +223,7 @@ def run_ours(args):
     ldp_h = np.ascontiguousarray(wl.ldp(model.mu), dtype=npdt)
     ldp = torch.as_tensor(ldp_h).to(dev)
     pv = torch.as_tensor(wl.pv).to(dev)
-    flux = torch.empty((wl.npv, wl.npt), dtype=model.dtype, device=dev)
+    flux = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype, device=dev)
     status = torch.empty(wl.npv, dtype=torch.int32, device=dev)
     ctx = model.ctx
     npv = wl.npv
@@ -274,12 +275,12 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         try:
-            flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.dtype, pin_memory=True)
+            flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype, pin_memory=True)
             ldp_h_t = torch.as_tensor(ldp_h).pin_memory()
             pv_h_t = torch.as_tensor(wl.pv).pin_memory()
             pinned = True
         except RuntimeError:
-            flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.dtype)
+            flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype)
             ldp_h_t, pv_h_t = torch.as_tensor(ldp_h), torch.as_tensor(wl.pv)
             pinned = False
         status_h = np.empty(wl.npv, np.int32)
@@ -316,14 +317,14 @@ def run_ours(args):
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else \
         "6650 GB/s (of fallback)"
-    es = 4 if precision == rr.RR_FP32 else 8
+    es = 4 if precision == rr.RR_FP32 else 8            # flux element
     nrows = wl.npv * wl.model.npb
     # algorithmic bytes per launch: flux written once, times read once, two table rows + Istar +
     # the per-pv constants read once per (pv, passband)
     alg_bytes = (wl.npv * wl.npt * es + wl.npt * 12 + nrows * (2 * wl.model.ng + 1) * es
                  + wl.npv * 184)
     t_flux = ms_flux * 1e-3
-    ops = dict(ALG_OPS[args.precision])
+    ops = dict(ALG_OPS["fp64" if args.precision == "fp64" else "fp32"])
     if args.precision == "fp64":
         # circular orbits: per exposure phase 5 + sin/cos polynomials 15, per sub-sample one plane
         # rotation 4 + z^2 2
@@ -332,7 +333,7 @@ def run_ours(args):
                + counts["eccentric"] * ops["eccentric_fixed"]
                + counts["solver_iters"] * ops["solver_iter"]
                + counts["occulting"] * ops["occulting"] + counts["ingress"] * ops["ingress"])
-    lanes = FP32_LANES_PER_SM if precision == rr.RR_FP32 else FP64_LANES_PER_SM
+    lanes = FP32_LANES_PER_SM if precision != rr.RR_FP64 else FP64_LANES_PER_SM
     sm_max = (clocks or {}).get("sm_max_mhz") or float(peaks.get("sm_max_mhz", 1965.0))
     alu_peak_tflops = 2.0 * lanes * SM_COUNT * sm_max * 1e6 / 1e12
     fma_live = rr.rr_measure_fma_peak(precision)
@@ -374,7 +375,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": warm, "ms_per_step": ms_total / steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if precision == rr.RR_FP32 else "f64", "data": "synthetic",
+        "dtype": {"fp64": "f64", "fp32": "f32", "mixed": "f32 (sum and flux f64)"}[args.precision],
+        "data": "synthetic",
         "config": workload_config(wl, args.precision, {
             "parallelism": f"pv-sharded x{world}, no collective",
             "l2": "working set per step (flux + LD table) is far larger than the 126 MB L2; "

@@ -41,6 +41,9 @@ extern "C" {
 /* ---- codes ------------------------------------------------------------------------------- */
 #define RR_FP64 0
 #define RR_FP32 1
+#define RR_MIXED 2           /* the paper's proposed scheme: z and Ip*Ap in fp32; their
+                                average over the sub-samples, 1 - avg/Istar and the stored flux in
+                                fp64.  ldp, istar, table: fp32; flux: fp64                        */
 
 #define RR_OK            0
 #define RR_ENULL        -1   /* a required pointer is NULL                                     */
@@ -96,7 +99,7 @@ typedef struct {
   double  k0, k1;    /* 0 < k0 < k1                                                              */
   int32_t npb;       /* passbands                                                (>= 1)          */
   int32_t nkpb;      /* 1 = one k per parameter vector; npb = one k per passband  */
-  int32_t precision; /* RR_FP64 or RR_FP32: type of ldp, istar, the table and flux               */
+  int32_t precision; /* RR_FP64, RR_FP32 (type of ldp, istar, the table and flux) or RR_MIXED    */
 } rr_config;
 
 /* ---- life cycle ------------------------------------------------------------------------------

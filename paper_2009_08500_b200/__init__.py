@@ -20,7 +20,7 @@ import numpy as np
 
 from . import build as _build
 
-RR_FP64, RR_FP32 = 0, 1
+RR_FP64, RR_FP32, RR_MIXED = 0, 1, 2
 RR_REDUCE_AUTO, RR_REDUCE_THREAD, RR_REDUCE_SHUFFLE = 0, 1, 2
 RR_TABLE_LAZY, RR_TABLE_FULL, RR_TABLE_DIRECT = 0, 1, 2
 LD_LAWS = {"uniform": 0, "linear": 1, "quadratic": 2, "quadratic-tri": 3, "general": 4,
@@ -288,8 +288,9 @@ def rr_evaluate_host(ctx: int, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray
     """Whole step from HOST arrays (numpy, or the .numpy() view of a pinned torch tensor)."""
     if not (ldp.flags.c_contiguous and pv.flags.c_contiguous and flux.flags.c_contiguous):
         raise TypeError("host arrays must be C-contiguous")
-    if pv.dtype != np.float64 or ldp.dtype != flux.dtype:
-        raise TypeError("pv must be float64; ldp and flux must share the ctx precision")
+    if pv.dtype != np.float64 or ldp.dtype not in (np.float32, np.float64) \
+            or flux.dtype not in (np.float32, np.float64):
+        raise TypeError("pv must be float64; ldp and flux float32/float64 as the ctx precision asks")
     npv, npar = pv.shape
     _check(load().rr_evaluate_host(ctx, ldp.ctypes.data, pv.ctypes.data, npar, npv,
                                    flux.ctypes.data,
@@ -331,7 +332,8 @@ class RoadRunner:
         import torch
         self.nz, self.ng, self.nk, self.npb, self.nkpb = nzin + nzlimb, ng, nk, npb, nkpb
         self.precision = precision
-        self.dtype = torch.float32 if precision == RR_FP32 else torch.float64
+        self.dtype = torch.float32 if precision != RR_FP64 else torch.float64     # ldp, istar, table
+        self.flux_dtype = torch.float32 if precision == RR_FP32 else torch.float64
         self.ctx = rr_create(nzin, nzlimb, zcut, ng, nk, k0, k1, npb, nkpb, precision)
         self.mu = rr_get_mu(self.ctx, self.nz)
         self.ze = rr_get_ze(self.ctx, self.nz)
@@ -386,14 +388,14 @@ class RoadRunner:
 
     def profile_and_istar(self):
         """Diagnostics: Istar[npv][npb] of the last table build (numpy)."""
-        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        npdt = np.float32 if self.precision != RR_FP64 else np.float64
         I = np.empty((self.npv, self.npb), npdt)
         _check(load().rr_get_table(self.ctx, None, I.ctypes.data), "rr_get_table")
         return I
 
     def table(self):
         """Copy of T[npv][npb][nk][ng] and Istar[npv][npb] as numpy arrays (diagnostics)."""
-        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        npdt = np.float32 if self.precision != RR_FP64 else np.float64
         T = np.empty((self.npv, self.npb, self.nk, self.ng), npdt)
         I = np.empty((self.npv, self.npb), npdt)
         _check(load().rr_get_table(self.ctx, T.ctypes.data, I.ctypes.data), "rr_get_table")
@@ -401,7 +403,7 @@ class RoadRunner:
 
     def rows(self):
         """Copy of the collapsed rows ldw[npv][npb][ng] of the last evaluate (lazy / direct mode)."""
-        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        npdt = np.float32 if self.precision != RR_FP64 else np.float64
         out = np.empty((self.npv, self.npb, self.ng), npdt)
         _check(load().rr_get_rows(self.ctx, out.ctypes.data), "rr_get_rows")
         return out
@@ -412,7 +414,7 @@ class RoadRunner:
         if not isinstance(pv, torch.Tensor):
             pv = torch.as_tensor(np.ascontiguousarray(pv, np.float64)).cuda()
         pv = pv.reshape(-1, self.nkpb + 6).contiguous()
-        flux = torch.empty((pv.shape[0], self.npt), dtype=self.dtype, device="cuda")
+        flux = torch.empty((pv.shape[0], self.npt), dtype=self.flux_dtype, device="cuda")
         status = torch.empty(pv.shape[0], dtype=torch.int32, device="cuda")
         rr_evaluate(self.ctx, pv, flux, status)
         return (flux, status) if want_status else flux
@@ -429,10 +431,11 @@ class RoadRunner:
 
     def evaluate_host(self, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray | None = None,
                       status: np.ndarray | None = None):
-        npdt = np.float32 if self.precision == RR_FP32 else np.float64
+        npdt = np.float32 if self.precision != RR_FP64 else np.float64
         ldp = np.ascontiguousarray(ldp, npdt).reshape(-1, self.npb, self.nz)
         pv = np.ascontiguousarray(pv, np.float64).reshape(-1, self.nkpb + 6)
         if flux is None:
-            flux = np.empty((pv.shape[0], self.npt), npdt)
+            flux = np.empty((pv.shape[0], self.npt),
+                            np.float32 if self.precision == RR_FP32 else np.float64)
         rr_evaluate_host(self.ctx, ldp, pv, flux, status)
         return flux

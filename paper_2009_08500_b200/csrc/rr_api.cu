@@ -15,7 +15,9 @@
 
 namespace {
 
-int esize(const rr_ctx *ctx) { return ctx->cfg.precision == RR_FP32 ? 4 : 8; }
+// element size of ldp, T, Istar, rows (fp32 in RR_FP32 and RR_MIXED) and of flux (fp32 in RR_FP32)
+int esize(const rr_ctx *ctx) { return ctx->cfg.precision != RR_FP64 ? 4 : 8; }
+int esize_flux(const rr_ctx *ctx) { return ctx->cfg.precision == RR_FP32 ? 4 : 8; }
 
 void free_work(RRWork *w) {
   if (w->T) cudaFree(w->T);
@@ -91,7 +93,7 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   if (cfg->nzin < 1 || cfg->nzlimb < 1 || !(cfg->zcut > 0.0 && cfg->zcut < 1.0) || cfg->ng < 2 ||
       cfg->nk < 2 || !(cfg->k0 > 0.0) || !(cfg->k1 > cfg->k0) || !isfinite(cfg->k1) ||
       cfg->npb < 1 || (cfg->nkpb != 1 && cfg->nkpb != cfg->npb) ||
-      (cfg->precision != RR_FP64 && cfg->precision != RR_FP32) ||
+      (cfg->precision != RR_FP64 && cfg->precision != RR_FP32 && cfg->precision != RR_MIXED) ||
       (int64_t)cfg->nzin + cfg->nzlimb > 100000 || cfg->ng > 5600 ||
       (int64_t)cfg->nk * cfg->ng > 0x7fffffffLL / 2)
     return RR_ECONFIG;
@@ -369,17 +371,17 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
   if (npv <= 0 || npar != ctx->cfg.nkpb + 6) return RR_ESIZE;
   if (ctx->ntiles < 0) return RR_ESTATE;
   const rr_config &c = ctx->cfg;
-  const int64_t es = esize(ctx);
+  const int64_t es = esize(ctx), esf = esize_flux(ctx);
   for (int s = 0; s < 2; ++s) {
     if (!ctx->hs[s]) RR_CUDA(cudaStreamCreateWithFlags(&ctx->hs[s], cudaStreamNonBlocking));
     if (!ctx->hev[s]) RR_CUDA(cudaEventCreateWithFlags(&ctx->hev[s], cudaEventDisableTiming));
   }
   // chunk: about 256 MB of flux, at least 1 pv
-  int64_t chunk = (256LL << 20) / (ctx->npt * es);
+  int64_t chunk = (256LL << 20) / (ctx->npt * esf);
   chunk = std::max<int64_t>(1, std::min(chunk, npv));
   if (chunk > 64) chunk = (chunk / 64) * 64;
   const int64_t ldp_row = (int64_t)c.npb * ctx->nz * es, pv_row = (int64_t)npar * 8,
-                flux_row = ctx->npt * es;
+                flux_row = ctx->npt * esf;
   int rc = RR_OK;
   int64_t n_chunks = (npv + chunk - 1) / chunk;
   for (int64_t ci = 0; ci < n_chunks && rc == RR_OK; ++ci) {
@@ -470,7 +472,7 @@ int rr_get_kernel_times(rr_ctx *ctx, double *h_ms, int64_t *h_calls) {
 
 int rr_measure_fma_peak(int32_t precision, double *h_fma_per_s, void *stream) {
   if (!h_fma_per_s) return RR_ENULL;
-  if (precision != RR_FP64 && precision != RR_FP32) return RR_ECONFIG;
+  if (precision != RR_FP64 && precision != RR_FP32 && precision != RR_MIXED) return RR_ECONFIG;
   return rr_fma_peak_launch(precision, h_fma_per_s, (cudaStream_t)stream);
 }
 

@@ -488,10 +488,12 @@ __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
 }
 
 // The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
-template <typename R, bool COUNT, bool CIRC, bool NOWRAP>
-__device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__restrict__ out,
+// R = arithmetic type of z and ip*ap; O = type of the sub-sample sum, the final 1 - sum/(Istar ns)
+// and the stored flux (O = double with R = float is RR_MIXED, the scheme of PAPER.md:293).
+template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP>
+__device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__restrict__ out,
                                         int count, int ns, int shuffle, double t0, double inv_p,
-                                        double u_mid, double hwid, double hw, R scale,
+                                        double u_mid, double hwid, double hw, O scale,
                                         const Cst<R> k, const R *__restrict__ ldw, int ng,
                                         unsigned long long *cnt) {
   const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
@@ -505,14 +507,14 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
       if (i + FT < count) tnext = times[i + FT];     // in flight while this exposure is evaluated
       const double wc = fma(tcur - t0, inv_p, -u_mid);
       const double wr = wc - rr_round(wc);           // exposure centre from the window centre
-      R f;
+      O f;
       if (fabs(wr) > hskip) {
-        f = (R)1;
+        f = (O)1;
         if (COUNT) cnt[0] += ns;
       } else if (!(wr == wr)) {
-        f = rr_nan<R>();
+        f = rr_nan<O>();
       } else {
-        R acc = (R)0;
+        O acc = (O)0;
         if (CIRC && sizeof(R) == 8) {
           // circular orbit, fp64: sin and cos of the first sub-sample's phase, then one plane
           // rotation per sub-sample (constant phase step); no per-sub-sample window test is
@@ -551,7 +553,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
           for (int s = 0; s < ns; ++s, w += du)
             acc += rr_subsample<R, COUNT, CIRC, NOWRAP>(w, u_mid, hwid, k, ldw, ng, cnt);
         }
-        f = fma(-acc, scale, (R)1);                  // mean of (Istar - ip ap)/Istar over ns
+        f = fma(-acc, scale, (O)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
       out[i] = f;
     }
@@ -564,7 +566,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
     for (int base = 0; base < count; base += per_pass) {
       const int i = base + (threadIdx.x / G);
       const bool live = i < count;
-      R acc = (R)0;
+      O acc = (O)0;
       double wr = 0.0;
       if (live) {
         const double wc = fma(times[i] - t0, inv_p, -u_mid);
@@ -579,7 +581,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
         }
       }
       for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if (live && sl == 0) out[i] = (wr == wr) ? fma(-acc, scale, (R)1) : rr_nan<R>();
+      if (live && sl == 0) out[i] = (wr == wr) ? fma(-acc, scale, (O)1) : rr_nan<O>();
     }
   }
 }
@@ -589,7 +591,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, R *__r
 // chunk meets; tiles outside the transit window are merged into contiguous runs and written as
 // flux = 1 with 16-byte stores, without touching the orbit.
 // Shared memory: cst[K_SMEM] (constants, working precision) | ldw[ng+1] (k-collapsed table row).
-template <typename R, bool COUNT>
+template <typename R, typename O, bool COUNT>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
   extern __shared__ __align__(16) unsigned char rr_smem[];
@@ -605,10 +607,10 @@ rr_flux_kernel(const FluxParams P) {
   const int64_t tl0 = (int64_t)chunk * P.chunk_len;
   const int64_t tl1 = min(tl0 + (int64_t)P.chunk_len, P.ntiles);
   const RRPvOrbit &po = P.pvo[v];
-  R *row = reinterpret_cast<R *>(P.flux) + (int64_t)v * P.npt;
+  O *row = reinterpret_cast<O *>(P.flux) + (int64_t)v * P.npt;
   if (po.status) {                                     // reading R12: NaN row
     const RRTile a = P.tiles[tl0], b = P.tiles[tl1 - 1];
-    rr_fill<R>(row + a.start, (int64_t)b.start + b.count - a.start, rr_nan<R>());
+    rr_fill<O>(row + a.start, (int64_t)b.start + b.count - a.start, rr_nan<O>());
     return;
   }
   const double t0 = po.t0, inv_p = po.inv_p, u_mid = po.u_mid, hwid = po.hwid;
@@ -616,7 +618,7 @@ rr_flux_kernel(const FluxParams P) {
   int desc_lc = -1, staged_lc = -1;                    // light curve of lc / of the staged table
   RRLc lc;
   double hw = 0.0;                                     // half an exposure, in turns
-  R scale = (R)0;
+  O scale = (O)0;
   int64_t f0 = -1, f1 = 0;                             // pending run of exposures with flux 1
 
   for (int64_t base = tl0; base < tl1; base += FT) {
@@ -654,7 +656,7 @@ rr_flux_kernel(const FluxParams P) {
       if (q >= ngrp) break;
       pos = q + 1;
       if (f0 >= 0) {
-        rr_fill<R>(row + f0, f1 - f0, (R)1);
+        rr_fill<O>(row + f0, f1 - f0, (O)1);
         f0 = -1;
       }
       const RRTile *tp = P.tiles + base + q;
@@ -687,23 +689,23 @@ rr_flux_kernel(const FluxParams P) {
         if (threadIdx.x == K_COUNT)
           cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
         __syncthreads();
-        scale = k[K_SCALE];
+        scale = (O)k[K_SCALE];
         staged_lc = tlc;
       }
       const int shuffle = lc.ns >= P.shuffle_min_ns;
       const bool nowrap = hwid + 2.0 * hw < 0.499;
       if (circular)
-        rr_tile<R, COUNT, true, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, true, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                        inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
       else if (nowrap)
-        rr_tile<R, COUNT, false, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, false, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                        inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
       else
-        rr_tile<R, COUNT, false, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, false, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                         inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
     }
   }
-  if (f0 >= 0) rr_fill<R>(row + f0, f1 - f0, (R)1);
+  if (f0 >= 0) rr_fill<O>(row + f0, f1 - f0, (O)1);
   if (COUNT) {
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
@@ -837,7 +839,7 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
   const bool direct = wk->lazy == 2;
   rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
       d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, direct ? 1e-300 : c.k0, direct ? 1e300 : c.k1, c.ng,
-      c.precision == RR_FP32, ctx->mean_k, rr_row_pad(ctx), wk->pvo, wk->pvb, d_status);
+      c.precision != RR_FP64, ctx->mean_k, rr_row_pad(ctx), wk->pvo, wk->pvb, d_status);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
@@ -888,14 +890,16 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + P.ldw_len) * (c.precision == RR_FP32 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8);
   if (ctx->counters_on) {
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
-    if (c.precision == RR_FP32) rr_flux_kernel<float, true><<<grid, FT, smem, st>>>(P);
-    else rr_flux_kernel<double, true><<<grid, FT, smem, st>>>(P);
+    if (c.precision == RR_FP32) rr_flux_kernel<float, float, true><<<grid, FT, smem, st>>>(P);
+    else if (c.precision == RR_MIXED) rr_flux_kernel<float, double, true><<<grid, FT, smem, st>>>(P);
+    else rr_flux_kernel<double, double, true><<<grid, FT, smem, st>>>(P);
   } else {
-    if (c.precision == RR_FP32) rr_flux_kernel<float, false><<<grid, FT, smem, st>>>(P);
-    else rr_flux_kernel<double, false><<<grid, FT, smem, st>>>(P);
+    if (c.precision == RR_FP32) rr_flux_kernel<float, float, false><<<grid, FT, smem, st>>>(P);
+    else if (c.precision == RR_MIXED) rr_flux_kernel<float, double, false><<<grid, FT, smem, st>>>(P);
+    else rr_flux_kernel<double, double, false><<<grid, FT, smem, st>>>(P);
   }
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
@@ -917,6 +921,6 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
 }
 
 int rr_fma_peak_launch(int precision, double *h_fma_per_s, cudaStream_t st) {
-  if (precision == RR_FP32) return fma_peak_typed<float>(h_fma_per_s, st);
+  if (precision != RR_FP64) return fma_peak_typed<float>(h_fma_per_s, st);
   return fma_peak_typed<double>(h_fma_per_s, st);
 }

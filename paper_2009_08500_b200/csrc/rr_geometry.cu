@@ -147,7 +147,7 @@ int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t 
   const int64_t M = npv * c.npb;
   if (M > 0x7fffffffLL) return RR_ESIZE;
   const size_t smem = sizeof(double) * 2 * (ctx->nz + 1);
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_ld_rows_direct_kernel<float><<<(unsigned)M, 256, smem, st>>>(
         (const float *)wk->ldp_src, ctx->d_ze, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
         ctx->nz);
@@ -201,7 +201,7 @@ int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t s
   const rr_config &c = ctx->cfg;
   const int64_t M = npv * c.npb;
   const unsigned grid = (unsigned)((M * 32 + 255) / 256);
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_ld_rows_small_kernel<float><<<grid, 256, 0, st>>>(
         (const float *)wk->ldp_src, ctx->d_zm, wk->pvb, (float *)wk->rows, ctx->k_small, M, c.npb,
         c.nkpb, c.ng, ctx->nz);

@@ -366,7 +366,7 @@ int launch_typed(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar
 int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar,
                        int64_t npv, cudaStream_t st) {
   const rr_config &c = ctx->cfg;
-  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t needT = npv * c.npb * (int64_t)c.nk * c.ng * esz, needI = npv * c.npb * esz;
   if (needT > wk->T_cap) {
     if (wk->T) cudaFree(wk->T);
@@ -384,7 +384,7 @@ int rr_ld_table_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d
     if (cudaMalloc(&wk->istar, needI) != cudaSuccess) { cudaGetLastError(); return RR_EALLOC; }
     wk->istar_cap = needI;
   }
-  int rc = c.precision == RR_FP32 ? launch_typed<float>(ctx, wk, d_ldp, d_istar, npv, st)
+  int rc = c.precision != RR_FP64 ? launch_typed<float>(ctx, wk, d_ldp, d_istar, npv, st)
                                   : launch_typed<double>(ctx, wk, d_ldp, d_istar, npv, st);
   wk->table_npv = rc == RR_OK ? npv : -1;
   wk->lazy = 0;
@@ -408,7 +408,7 @@ static int grow_buf(void **p, int64_t *cap, int64_t need) {
 int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar,
                          int64_t npv, int copy, cudaStream_t st) {
   const rr_config &c = ctx->cfg;
-  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t M = npv * c.npb, needP = M * ctx->nz * esz, needI = M * esz;
   wk->table_npv = -1;
   int rc = grow_buf(&wk->istar, &wk->istar_cap, needI);
@@ -421,7 +421,7 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
     wk->ldp_src = d_ldp;
   }
   const int64_t threads = M * 32;
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_istar_kernel<float, float><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const float *)d_ldp, ctx->d_q, (const float *)d_istar, (float *)wk->istar, M, ctx->nz);
   else
@@ -437,7 +437,7 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
 // Lazy mode, at rr_evaluate (after the per-pv prep): the rows the flux kernel stages.
 int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
   const rr_config &c = ctx->cfg;
-  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t M = npv * c.npb;
   if (M > 0x7fffffffLL) return RR_ESIZE;
   int rc = grow_buf(&wk->rows, &wk->rows_cap, M * c.ng * esz);
@@ -462,7 +462,7 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
     rr_rows_scatter<<<gb, 256, 0, st>>>(wk->pvb, M, c.npb, c.nkpb, offs, cursor, list);
     RR_LAUNCH_CHECK(ctx);
     const unsigned tiles_max = (unsigned)((M + RB - 1) / RB + nb);
-    if (c.precision == RR_FP32) {
+    if (c.precision != RR_FP64) {
       if (smem_b > 48 * 1024)
         RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<float>,
                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
@@ -481,7 +481,7 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
     return RR_OK;
   }
   const size_t smem = sizeof(double) * ctx->nz;
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_ld_rows_kernel<float><<<(unsigned)M, RT, smem, st>>>(
         (const float *)wk->ldp_src, ctx->d_W, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
         ctx->nz);
@@ -498,14 +498,14 @@ int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st) {
   if (wk->have_full) return RR_OK;
   if (wk->table_npv <= 0 || wk->ldp_src != wk->ldp || !wk->ldp) return RR_ESTATE;
   const rr_config &c = ctx->cfg;
-  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t npv = wk->table_npv;
   int rc = grow_buf(&wk->T, &wk->T_cap, npv * c.npb * (int64_t)c.nk * c.ng * esz);
   if (rc != RR_OK) return rc;
   const int64_t M = npv * c.npb;
   const int N = c.nk * c.ng, K = ctx->nz;
   dim3 grid((N + BN - 1) / BN, (unsigned)((M + BM - 1) / BM));
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_ld_table_kernel<float, float><<<grid, NT, 0, st>>>((const float *)wk->ldp, ctx->d_W,
                                                           (float *)wk->T, M, N, K);
   else
@@ -521,7 +521,7 @@ int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st) {
 int rr_ld_law_launch(rr_ctx *ctx, RRWork *wk, int law, const double *d_ldc, int nc, int64_t npv,
                      cudaStream_t st) {
   const rr_config &c = ctx->cfg;
-  const int64_t esz = c.precision == RR_FP32 ? 4 : 8;
+  const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t M = npv * c.npb;
   wk->table_npv = -1;
   int rc = grow_buf(&wk->ldp, &wk->ldp_cap, M * ctx->nz * esz);
@@ -534,7 +534,7 @@ int rr_ld_law_launch(rr_ctx *ctx, RRWork *wk, int law, const double *d_ldc, int 
   RR_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
   const int64_t n = M * ctx->nz;
   const unsigned grid = (unsigned)((n + 255) / 256);
-  if (c.precision == RR_FP32)
+  if (c.precision != RR_FP64)
     rr_ld_law_kernel<float><<<grid, 256, 0, st>>>(law, d_ldc, nc, ctx->d_mu, M, ctx->nz,
                                                   (float *)wk->ldp, (float *)given, flag);
   else

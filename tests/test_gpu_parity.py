@@ -287,6 +287,30 @@ def test_small_planet_approximation(rr, mode, precision):
     gm.close()
 
 
+# ---- mixed precision (NEXT-4) ------------------------------------------------------------
+@pytest.mark.parametrize("config", [2, 3, 4])
+def test_mixed_precision_scheme(rr, config):
+    """RR_MIXED: z and Ip*Ap in fp32, their average over the sub-samples and 1 - avg/Istar in fp64,
+    fp64 flux out (the scheme PAPER.md:293 proposes).  Error against the fp64 oracle: measured, and
+    clearly below the fp32 mode's (whose stored flux alone is rounded to 6e-8 near 1)."""
+    wl = small_workload(config)
+    want, st_o = oracle_flux(wl)
+    got32 = gpu_flux(rr, wl, precision=1)
+    gm = gpu_model(rr, wl, precision=rr.RR_MIXED)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    flux, status = gm.evaluate(wl.pv, want_status=True)
+    assert flux.dtype == __import__("torch").float64
+    gotm = flux.cpu().numpy()
+    assert np.array_equal(status.cpu().numpy(), st_o)
+    em, e32 = np.max(np.abs(gotm - want)), np.max(np.abs(got32 - want))
+    assert em <= 2e-8 and em < 0.6 * e32, (config, em, e32)
+    assert np.array_equal(gotm == 1.0, want == 1.0)
+    status_h = np.empty(wl.npv, np.int32)
+    host = gm.evaluate_host(wl.ldp(gm.mu), wl.pv, status=status_h)
+    assert host.dtype == np.float64 and np.array_equal(host, gotm)
+    gm.close()
+
+
 # ---- named laws on the device (NEXT-4) ------------------------------------------------------------------
 LAWS = [("uniform", None), ("linear", [(0.2, 0.8)]), ("quadratic", [(0.1, 0.6), (0.0, 0.3)]),
         ("quadratic-tri", [(0.1, 0.8), (0.1, 0.5)]), ("general", [(0.1, 0.4), (0.0, 0.2), (-0.1, 0.1)]),
