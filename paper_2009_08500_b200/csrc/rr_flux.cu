@@ -2,9 +2,11 @@
 //   per-pv prep      validity (reading R12), k-interpolation index, orbit
 //                    constants at inferior conjunction, and the transit window in orbital phase
 //   rr_orbit_kernel  kernel 2 alone: z for every sub-sample (tests / diagnostics)
-//   rr_flux_kernel   kernels 2+3 fused over (dispatch tile, parameter vector) pairs:
-//                    PAPER.md:101-107 (g interpolation, area, flux), :131 (k collapse of the two
-//                    bracketing table rows), :214 (supersampling), :220 (orbit parameters)
+//   rr_flux_kernel   kernels 2+3 fused, one block per (parameter vector, chunk of dispatch tiles):
+//                    PAPER.md:101-107 (g interpolation, area, flux), :131 (k-collapsed table
+//                    row), :214 (supersampling), :220 (orbit parameters); template <R, O>:
+//                    R = arithmetic of z and ip*ap, O = sub-sample sum and stored flux
+//                    (double/double, float/float, float/double = RR_MIXED)
 // Orbit formulation (kernel 2).  Time enters as the phase u = (t - t0)/p in turns,
 // reduced in fp64.  z < 1+k in front of the star is only possible in a window around conjunction
 // computed per pv; everything outside it has flux 1 exactly and costs a compare.  Inside, Kepler's
@@ -15,10 +17,12 @@
 // a*eps(E) ~ 4e-6 in z), and it removes atan2 and the true anomaly from the path: the sky position
 // is linear in (cos d - 1, sin d) with per-pv coefficients.
 // Solver: a 4th-order series-reversion starter (exact derivatives of G at d = 0 are per-pv
-// constants) and ONE Halley step, accepted when the step is below a per-pv tolerance that bounds
-// the remaining error by ~2.5e-13 (fp64); anything else (large |d|, e near 1 at periastron) goes to a
-// bracketed Halley/bisection loop.  sin d, cos d - 1 on |d| <= 0.8 are Taylor polynomials with their
-// coefficients in constant memory (operands of the FMAs, no register traffic).
+// constants) and Halley steps, the first accepted for ~91 % of sub-samples: a step below a per-pv
+// tolerance bounds the remaining error by ~2e-15 (fp64) and is applied by a second-order rotation of
+// (sin d, cos d - 1), so one sincos suffices; anything else (|d| > 0.5, e near 1 at periastron) goes
+// to a bracketed Halley/bisection loop.  sin d, cos d - 1 on |d| <= 0.5 are Taylor polynomials with
+// their coefficients in constant memory (rr_math.cuh).  Circular orbits in fp64: sin/cos once per
+// exposure, one plane rotation per further sub-sample.
 #include <algorithm>
 
 #include "rr_common.cuh"
