@@ -28,6 +28,9 @@
 #include "rr_common.cuh"
 #include "rr_math.cuh"
 
+// flux is written once and never re-read: streaming stores keep W, times and the rows in L2
+#define RR_STORE(p, v) __stcs((p), (v))
+
 namespace {
 
 #ifndef RR_FLUX_THREADS
@@ -456,12 +459,12 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
     double2 v = make_double2((double)val, (double)val);
     double2 *o = reinterpret_cast<double2 *>(out + head);
 #pragma unroll 4
-    for (int64_t i = threadIdx.x; i < nvec; i += FT) o[i] = v;
+    for (int64_t i = threadIdx.x; i < nvec; i += FT) RR_STORE(o + i, v);
   } else {
     float4 v = make_float4((float)val, (float)val, (float)val, (float)val);
     float4 *o = reinterpret_cast<float4 *>(out + head);
 #pragma unroll 4
-    for (int64_t i = threadIdx.x; i < nvec; i += FT) o[i] = v;
+    for (int64_t i = threadIdx.x; i < nvec; i += FT) RR_STORE(o + i, v);
   }
   const int64_t done = head + nvec * VN;
   if ((int64_t)threadIdx.x < count - done) out[done + threadIdx.x] = val;
@@ -559,7 +562,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         }
         f = fma(-acc, scale, (O)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
-      out[i] = f;
+      RR_STORE(out + i, f);
     }
   } else {
     // ---- sub-samples across lanes, warp-shuffle sum ----
