@@ -365,7 +365,7 @@ def run_ours(args):
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        rate, dt, n = oracle_rate(wl, 12.0)
+        rate, dt, n = oracle_rate(wl, 24.0)
         cpu_baseline = {"value": rate, "unit": UNIT, "cores": os.cpu_count() or 1,
                         "kind": "oracle", "seconds": dt,
                         "sample": f"first {n} of {wl.npv} parameter vectors x all {wl.npt} "
