@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(256)
 rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ ze,
                          const RRPvBand *__restrict__ pvb, TR *__restrict__ rows, int npb, int nkpb,
                          int ng, int nz) {
-  extern __shared__ double sh[];                 // D[nz+1] (index = edge) | ze[nz+1]
-  double *D = sh, *zes = sh + nz + 1;
+  extern __shared__ double sh[];                 // D[nz+1] (index = edge) | ze[nz+1] | a[ng]
+  double *D = sh, *zes = sh + nz + 1, *area = sh + 2 * (nz + 1);
   const int64_t row = blockIdx.x;
   const int64_t v = row / npb;
   const int pb = (int)(row - v * npb);
@@ -110,6 +110,9 @@ rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
     zes[e] = ze[e];
     D[e] = (e == 0) ? 0.0 : (e < nz ? (double)pr[e - 1] - (double)pr[e] : (double)pr[nz - 1]);
   }
+  // the whole occulted area a(c_ig, k) of every node: one thread per node, not one warp per node
+  for (int ig = threadIdx.x; ig < ng - 1; ig += 256)
+    area[ig] = rr_lens_area_fast(1.0, k, ((double)ig / (double)(ng - 1)) * (1.0 + k));
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int ig = warp; ig < ng; ig += 8) {
@@ -136,7 +139,7 @@ rr_ld_rows_direct_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
       if (e_hi <= nz) s = fma(RR_PI * k * k, (double)pr[e_hi - 1], s);
-      out = s / rr_lens_area_fast(1.0, k, c);
+      out = s / area[ig];
     }
     if (lane == 0) rows[row * ng + ig] = (TR)out;
   }
@@ -146,7 +149,13 @@ int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t 
   const rr_config &c = ctx->cfg;
   const int64_t M = npv * c.npb;
   if (M > 0x7fffffffLL) return RR_ESIZE;
-  const size_t smem = sizeof(double) * 2 * (ctx->nz + 1);
+  const size_t smem = sizeof(double) * (2 * (ctx->nz + 1) + c.ng);   // <= 77 kB (nz <= 2000, ng <= 5600)
+  if (smem > 48 * 1024) {
+    RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_direct_kernel<float>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_direct_kernel<double>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  }
   if (c.precision != RR_FP64)
     rr_ld_rows_direct_kernel<float><<<(unsigned)M, 256, smem, st>>>(
         (const float *)wk->ldp_src, ctx->d_ze, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
