@@ -898,16 +898,18 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
   const size_t smem = (size_t)(K_SMEM + P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8);
-  if (ctx->counters_on) {
+  if (ctx->counters_on)
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
-    if (c.precision == RR_FP32) rr_flux_kernel<float, float, true><<<grid, FT, smem, st>>>(P);
-    else if (c.precision == RR_MIXED) rr_flux_kernel<float, double, true><<<grid, FT, smem, st>>>(P);
-    else rr_flux_kernel<double, double, true><<<grid, FT, smem, st>>>(P);
-  } else {
-    if (c.precision == RR_FP32) rr_flux_kernel<float, float, false><<<grid, FT, smem, st>>>(P);
-    else if (c.precision == RR_MIXED) rr_flux_kernel<float, double, false><<<grid, FT, smem, st>>>(P);
-    else rr_flux_kernel<double, double, false><<<grid, FT, smem, st>>>(P);
-  }
+  using Kernel = void (*)(const FluxParams);
+  const int pi = c.precision == RR_FP32 ? 1 : (c.precision == RR_MIXED ? 2 : 0);
+  static const Kernel kernels[3][2] = {
+      {rr_flux_kernel<double, double, false>, rr_flux_kernel<double, double, true>},
+      {rr_flux_kernel<float, float, false>, rr_flux_kernel<float, float, true>},
+      {rr_flux_kernel<float, double, false>, rr_flux_kernel<float, double, true>}};
+  const Kernel kern = kernels[pi][ctx->counters_on ? 1 : 0];
+  if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory
+    RR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  kern<<<grid, FT, smem, st>>>(P);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }

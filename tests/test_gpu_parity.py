@@ -333,6 +333,31 @@ def test_random_setups_match_oracle(rr, seed):
             gm.close()
 
 
+def test_maximum_resolutions(rr):
+    """ng and nz near the library's limits: the flux and direct-row kernels opt in to > 48 kB of
+    dynamic shared memory (ng = 5000 staged nodes; direct rows with nz = 1500 edges)."""
+    mc = workloads.ModelConfig(nzin=700, nzlimb=800, ng=5000, nk=3, k0=0.05, k1=0.15)
+    wl = workloads.make_workload(1, npv=3, npt=900)
+    wl.pv[:, 0] = [0.06, 0.1, 0.149]
+    coeffs = wl.ld_coeffs
+    om = oracle.OracleModel.from_config(mc)
+    om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+    want_t, _ = om.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                            wl.exposure_time, wl.pv)
+    od = oracle.OracleDirectModel.from_config(mc)
+    want_d, _ = od.evaluate(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                            wl.exposure_time, wl.pv, workloads.sample_profile("quadratic", coeffs, od.mu))
+    for mode, want in ((0, want_t), (2, want_d)):
+        gm = rr.RoadRunner.from_config(mc)
+        rr.rr_set_table_mode(gm.ctx, mode)
+        gm.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
+        gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+        got = gm.evaluate(wl.pv).cpu().numpy()
+        assert np.max(np.abs(got - want)) <= TOL64
+        gm.close()
+    assert (want_t < 1).sum() > 100
+
+
 # ---- mixed precision (NEXT-4, PAPER.md:293) ------------------------------------------------------------
 @pytest.mark.parametrize("config", [2, 3, 4])
 def test_mixed_precision_scheme(rr, config):
