@@ -144,33 +144,53 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   po.Y0 = (1.0 - e) * (1.0 + e) / den;           // r(t0)/a
   po.Y1 = bcw * sE + sw * cE;
   po.Y2 = bcw * cE - sw * sE;
-  // transit window: z >= |x_sky| = r |cos(w+f)| >= a(1-e) |cos(w+f)|, so z < 1+k needs
-  // |cos(w+f)| < q = (1+k)/(a(1-e)), i.e. w+f within asin(q) of pi/2 (in front of the star).
+  // Transit window.  z^2 = r^2 (c2 sin^2 i + cos^2 i), c2 = cos^2(w+f), so z < 1+k needs
+  //   c2 < q2 = ((1+k)^2 / r^2 - cos^2 i) / sin^2 i   with any lower bound r_lo of r on the window,
+  // i.e. w+f within h = asin(sqrt(q2)) of pi/2 (in front of the star); q2 <= 0: no transit at
+  // all.  r_lo starts at a(1-e) and is raised to the minimum of r over the window found so far
+  // (the in-transit set stays inside every window of the sequence, by induction), which matters
+  // for eccentric orbits that transit far from periastron: up to (1+e)/(1-e) narrower.
   double u_lo = -0.5, u_hi = 0.5;
-  double q = (1.0 + kmax) / (a * (1.0 - e));
-  if (!st && q < 0.999999) {
-    double h = asin(q);
-    if (po.circular) {
-      u_hi = h / RR_TWOPI;
-      u_lo = -u_hi;
-    } else {
-      double ftr = 0.5 * RR_PI - w;
-      double sq1 = sqrt(1.0 - e), sq2 = sqrt(1.0 + e);
-      double Etr = 2.0 * atan2(sq1 * sin(0.5 * ftr), sq2 * cos(0.5 * ftr));
-      double fh = ftr + h, fl = ftr - h;
-      double Eh = 2.0 * atan2(sq1 * sin(0.5 * fh), sq2 * cos(0.5 * fh));
-      double El = 2.0 * atan2(sq1 * sin(0.5 * fl), sq2 * cos(0.5 * fl));
-      double dEh = Eh - Etr, dEl = El - Etr;
-      dEh -= RR_TWOPI * floor(dEh / RR_TWOPI);   // [0, 2pi)
-      dEl -= RR_TWOPI * ceil(dEl / RR_TWOPI);    // (-2pi, 0]
-      double dMh = dEh - e * (sin(Etr + dEh) - sin(Etr));
-      double dMl = dEl - e * (sin(Etr + dEl) - sin(Etr));
-      u_hi = dMh / RR_TWOPI;
-      u_lo = dMl / RR_TWOPI;
+  if (!st) {
+    const double ci2 = ci * ci, om = 1.0 - ci2;
+    const double ftr = 0.5 * RR_PI - w;            // true anomaly at inferior conjunction
+    double r_lo = a * (1.0 - e), h = 0.0;
+    bool full = false;
+    for (int it = 0; it < 4; ++it) {
+      const double Q = (1.0 + kmax) / r_lo, Q2 = Q * Q;
+      const double q2 = om > 1e-12 ? (Q2 - ci2) / om : (Q2 > ci2 ? 2.0 : -1.0);
+      if (q2 >= 0.999998) { full = true; break; }
+      h = q2 > 0.0 ? asin(sqrt(q2)) : 0.0;
+      if (po.circular) break;
+      const double fa = ftr - h, fb = ftr + h;     // r is smallest where cos f is largest
+      double cosmax = fmax(cos(fa), cos(fb));
+      if (ceil(fa / RR_TWOPI) <= floor(fb / RR_TWOPI)) cosmax = 1.0;   // periastron inside
+      const double rn = a * (1.0 - e) * (1.0 + e) / (1.0 + e * cosmax);
+      if (!(rn > r_lo * (1.0 + 1e-9))) break;
+      r_lo = rn;
     }
-    u_hi = u_hi * (1.0 + 1e-9) + 1e-9;
-    u_lo = u_lo * (1.0 + 1e-9) - 1e-9;
-    if (!(u_hi - u_lo < 0.999) || !(u_hi > 0.0) || !(u_lo < 0.0)) { u_lo = -0.5; u_hi = 0.5; }
+    if (!full) {
+      if (po.circular) {
+        u_hi = h / RR_TWOPI;
+        u_lo = -u_hi;
+      } else {
+        double sq1 = sqrt(1.0 - e), sq2 = sqrt(1.0 + e);
+        double Etr = 2.0 * atan2(sq1 * sin(0.5 * ftr), sq2 * cos(0.5 * ftr));
+        double fh = ftr + h, fl = ftr - h;
+        double Eh = 2.0 * atan2(sq1 * sin(0.5 * fh), sq2 * cos(0.5 * fh));
+        double El = 2.0 * atan2(sq1 * sin(0.5 * fl), sq2 * cos(0.5 * fl));
+        double dEh = Eh - Etr, dEl = El - Etr;
+        dEh -= RR_TWOPI * floor(dEh / RR_TWOPI);   // [0, 2pi)
+        dEl -= RR_TWOPI * ceil(dEl / RR_TWOPI);    // (-2pi, 0]
+        double dMh = dEh - e * (sin(Etr + dEh) - sin(Etr));
+        double dMl = dEl - e * (sin(Etr + dEl) - sin(Etr));
+        u_hi = dMh / RR_TWOPI;
+        u_lo = dMl / RR_TWOPI;
+      }
+      u_hi = u_hi * (1.0 + 1e-9) + 1e-9;
+      u_lo = u_lo * (1.0 + 1e-9) - 1e-9;
+      if (!(u_hi - u_lo < 0.999) || !(u_hi > 0.0) || !(u_lo < 0.0)) { u_lo = -0.5; u_hi = 0.5; }
+    }
   }
   po.u_mid = 0.5 * (u_lo + u_hi);
   po.hwid = 0.5 * (u_hi - u_lo);
