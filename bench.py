@@ -39,8 +39,8 @@ FP64_LANES_PER_SM, FP32_LANES_PER_SM, SM_COUNT = 64, 128, 148
 # fp64 phase instructions counted twice) per unit of each class of the flux kernel.  Sub-samples in
 # merged out-of-window fill runs cost no arithmetic.
 ALG_OPS = {
-    "fp64": dict(skipped=2, circular=16, eccentric_fixed=26, solver_iter=31, occulting=18,
-                 ingress=64),
+    "fp64": dict(skipped=1, circular=16, eccentric_fixed=24, solver_iter=31, occulting=13,
+                 ingress=62),
     "fp32": dict(skipped=4, circular=19, eccentric_fixed=32, solver_iter=24, occulting=11,
                  ingress=61),
 }
@@ -326,9 +326,9 @@ def run_ours(args):
     t_flux = ms_flux * 1e-3
     ops = dict(ALG_OPS["fp64" if args.precision == "fp64" else "fp32"])
     if args.precision == "fp64":
-        # circular orbits: per exposure phase 5 + sin/cos polynomials 15, per sub-sample one plane
+        # circular orbits: per exposure phase 4 + sin/cos polynomials 15, per sub-sample one plane
         # rotation 4 + z^2 2
-        ops["circular"] = 6.0 + 20.0 * wl.npt / wl.evaluations_per_pv
+        ops["circular"] = 6.0 + 19.0 * wl.npt / wl.evaluations_per_pv
     alg_fma = (counts["skipped"] * ops["skipped"] + counts["circular"] * ops["circular"]
                + counts["eccentric"] * ops["eccentric_fixed"]
                + counts["solver_iters"] * ops["solver_iter"]

@@ -393,13 +393,9 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
 // Table cell of y = g/dg in [0, ng-1]: lower node ig and weight ag = y - ig.  The staged row carries
 // one extra node ldw[ng] = ldw[ng-1], so that y = ng-1 (z = 1+k to rounding) needs no clamp: it
 // lands in cell ng-1 with ag = 0 (reading R10: the same value as cell ng-2 with ag = 1).
-// fp64: floor by adding 2^52+2^51 to y - 1/2 (the integer lands in the low word); a tie or a
-// rounding across a node picks the neighbouring cell with ag = 1 or 0, the same interpolant.
 __device__ __forceinline__ void rr_cell(double y, int &ig, double &ag) {
-  const double M = 6755399441055744.0;
-  const double t = __dadd_rn(y - 0.5, M);
-  ig = __double2loint(t);
-  ag = y - __dadd_rn(t, -M);
+  ig = __double2int_rd(y);                   // conversion unit, not the FP64 pipe
+  ag = y - __int2double_rn(ig);
 }
 __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
   ig = (int)y;
