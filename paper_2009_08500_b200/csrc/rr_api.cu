@@ -370,6 +370,7 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
   if (!ctx || !h_ldp || !h_pv || !h_flux) return RR_ENULL;
   if (npv <= 0 || npar != ctx->cfg.nkpb + 6) return RR_ESIZE;
   if (ctx->ntiles < 0) return RR_ESTATE;
+  if (ctx->k_small > 0.0 && !lazy_ok(ctx)) return RR_ESTATE;   // needs the row builders
   const rr_config &c = ctx->cfg;
   const int64_t es = esize(ctx), esf = esize_flux(ctx);
   for (int s = 0; s < 2; ++s) {
