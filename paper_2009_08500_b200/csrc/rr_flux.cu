@@ -364,7 +364,8 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
       const R g = (d - dM) - t;
       const R gp = A - fma(C, cm1, -B * s);        // 1 - e cos E
       const R gpp = B + t;                         // e sin E
-      const R dd = (R)-2 * g * gp * rr_rcp(fma((R)2 * gp, gp, -g * gpp));   // Halley
+      // Halley: -2 g g' / (2 g'^2 - g g'') = -(g g') / (g'^2 - g g''/2)
+      const R dd = -(g * gp) * rr_rcp(fma((R)-0.5 * g, gpp, gp * gp));
       iters += 1;
       if (fabs(dd) <= tol) {
         // (sin, cos - 1) of d + dd, second order in dd
