@@ -333,6 +333,38 @@ def test_random_setups_match_oracle(rr, seed):
             gm.close()
 
 
+def test_bucketed_row_builder_with_chromatic_k(rr):
+    """>= 2048 (pv, passband) rows with one k per passband: the ik-bucketed lazy builder must bucket
+    every row by ITS passband's k.  Rows against the direct statement (1-ak) T[ik] + ak T[ik+1] from
+    the oracle's table; flux against the oracle."""
+    mc = workloads.ModelConfig(npb=3, nkpb=3)
+    rng = np.random.default_rng(21)
+    npv = 700
+    base = workloads.make_workload(1, npv=npv, npt=10).pv
+    kk = rng.uniform(0.021, 0.199, (npv, 3))
+    pv = np.concatenate([kk, base[:, 1:]], axis=1)
+    times = np.tile(np.linspace(-0.2, 0.2, 60), 3)
+    lc = np.repeat(np.arange(3, dtype=np.int32), 60)
+    coeffs = rng.uniform(0.1, 0.4, (npv, 3, 2))
+    om = oracle.OracleModel.from_config(mc)
+    T, _ = om.build_ld_table(workloads.sample_profile("quadratic", coeffs, om.mu))
+    want, _ = om.evaluate(times, lc, [0, 1, 2], [1, 2, 1], [0.0, 0.01, 0.0], pv, nthreads=0)
+    gm = rr.RoadRunner.from_config(mc)
+    gm.set_data(times, lc, [0, 1, 2], [1, 2, 1], [0.0, 0.01, 0.0])
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy()
+    rows = gm.rows()
+    dk = (mc.k1 - mc.k0) / (mc.nk - 1)
+    x = (kk - mc.k0) / dk
+    ik = np.minimum(np.floor(x).astype(int), mc.nk - 2)
+    ak = x - ik
+    v, b = np.meshgrid(np.arange(npv), np.arange(3), indexing="ij")
+    rows_o = (1 - ak)[..., None] * T[v, b, ik] + ak[..., None] * T[v, b, ik + 1]
+    assert np.max(np.abs(rows - rows_o)) <= 1e-13
+    assert np.max(np.abs(got - want)) <= TOL64
+    gm.close()
+
+
 def test_maximum_resolutions(rr):
     """ng and nz near the library's limits: the flux and direct-row kernels opt in to > 48 kB of
     dynamic shared memory (ng = 5000 staged nodes; direct rows with nz = 1500 edges)."""
