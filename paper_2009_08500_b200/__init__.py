@@ -419,6 +419,25 @@ class RoadRunner:
         rr_evaluate(self.ctx, pv, flux, status)
         return (flux, status) if want_status else flux
 
+    def evaluate_ps(self, k, t0, p, a, i, e=0.0, w=0.0):
+        """The paper's call ``evaluate(k, ldc, t0, p, a, i, e, w)`` with the
+        profile already set by ``build_ld_table*``: scalars give flux of shape (npt,), arrays of
+        npv entries give (npv, npt); k may be (npv,) or (npv, nkpb).  Marshalling only."""
+        args = [np.atleast_1d(np.asarray(x, np.float64)) for x in (t0, p, a, i, e, w)]
+        k = np.asarray(k, np.float64)
+        scalar = k.ndim == 0 and all(x.size == 1 for x in args)
+        k = k.reshape(1, -1) if k.ndim <= 1 and self.nkpb > 1 and k.size == self.nkpb else \
+            k.reshape(-1, self.nkpb) if k.ndim == 2 else k.reshape(-1, 1)
+        npv = max([k.shape[0]] + [x.size for x in args])
+        if k.shape[1] == 1 and self.nkpb > 1:
+            k = np.repeat(k, self.nkpb, axis=1)
+        pv = np.empty((npv, self.nkpb + 6))
+        pv[:, :self.nkpb] = np.broadcast_to(k, (npv, self.nkpb))
+        for col, x in enumerate(args):
+            pv[:, self.nkpb + col] = np.broadcast_to(x, (npv,))
+        flux = self.evaluate(pv)
+        return flux[0] if scalar else flux
+
     def orbit_z(self, pv, fp32_math=False):
         import torch
         if not isinstance(pv, torch.Tensor):

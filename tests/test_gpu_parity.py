@@ -724,6 +724,24 @@ def test_chromatic_k(rr):
     gm.close()
 
 
+def test_paper_call_shapes(rr):
+    """scalar parameters -> flux (npt,); arrays of npv -> (npv, npt); same values
+    as the pv-matrix call."""
+    wl = workloads.make_workload(3, npv=5, npt=6 * 40)
+    gm = gpu_model(rr, wl)
+    gm.build_ld_table(np.repeat(wl.ldp(gm.mu)[:1], 5, axis=0))
+    pv = wl.pv
+    ref = gm.evaluate(pv).cpu().numpy()
+    many = gm.evaluate_ps(pv[:, 0], pv[:, 1], pv[:, 2], pv[:, 3], pv[:, 4], pv[:, 5], pv[:, 6])
+    assert tuple(many.shape) == (5, wl.npt) and np.array_equal(many.cpu().numpy(), ref)
+    gm.build_ld_table(wl.ldp(gm.mu)[:1])
+    one = gm.evaluate_ps(*[float(x) for x in pv[0]])
+    assert tuple(one.shape) == (wl.npt,) and np.array_equal(one.cpu().numpy(), ref[0])
+    circ = gm.evaluate_ps(0.1, 0.0, 3.0, 8.0, 1.53)               # e, w default to 0 (PAPER.md:265)
+    assert tuple(circ.shape) == (wl.npt,) and float(circ.min()) < 1.0
+    gm.close()
+
+
 def test_argument_errors(rr):
     import torch
     gm = rr.RoadRunner()
