@@ -4,7 +4,7 @@
  *
  * The method is H. Parviainen, "RoadRunner: a fast and flexible exoplanet transit model"
  * (arXiv:2009.08500).  Citations below are PAPER.md line numbers (section / equation); readings
- * of the paper where it is silent are numbered R1..R12 in DESIGN.md section 3.
+ * of the paper where it is silent are numbered R1..R14 in DESIGN.md section 3.
  *
  * The two calls of the problem statement are
  *     build_ld_table(ldp[npv x npb x nz])                                   -> rr_build_ld_table
@@ -24,7 +24,8 @@
  *     rr_error_string() names any code.  No exception crosses the ABI.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with a CUDA error.
  *
- * Per-parameter-vector validity (reading R12): a parameter vector whose k is outside [k0,k1], whose
+ * Per-parameter-vector validity (reading R12): a parameter vector whose k is outside [k0,k1] (in
+ * RR_TABLE_DIRECT mode: k <= 0), whose
  * e is outside [0,1), whose a <= 0 or p <= 0, or that holds a non-finite value gets an all-NaN
  * flux row and a non-zero status word (bits below); the call itself still returns 0, so that a
  * sampler does not lose its other walkers.
@@ -126,7 +127,7 @@ int rr_get_weights(const rr_ctx *ctx, double *h_W /*[nk][ng][nz]*/);
  *                       t + tau*((s+1/2)/n - 1/2)                               (reading R7)
  * The library copies all five and runs the heterogeneous-dispatch kernels (DESIGN.md section 6,
  * kernel 4), which cut the exposure axis into tiles of one light curve each (uniform ns, tau,
- * passband) with their time range.  Synchronous on `stream` (it reads back the tile count).
+ * passband; 512 R exposures, R = clamp((8 + ns/2)/ns, 1, 8)) with their time range.  Synchronous on `stream` (it reads back the tile count).
  * RR_EINDEX if any index is out of range (nothing is kept then).                                */
 int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, int64_t npt,
                 const int32_t *h_passband_index, const int32_t *h_supersampling,
@@ -221,8 +222,10 @@ int rr_set_reduction(rr_ctx *ctx, int32_t mode);
  * h_ldp[npv][npb][nz], h_pv[npv][npar] -> h_flux[npv][npt], h_status[npv] (optional).  Runs
  * rr_build_ld_table + rr_evaluate over chunks of parameter vectors on two internal streams so
  * that the host<->device copies of one chunk overlap the kernels of the next.  Host buffers may be
- * pageable or pinned (pinned ones copy faster).  Needs rr_set_data.  Synchronous.  Afterwards the
- * ctx table holds the LAST chunk only.                                                           */
+ * pageable or pinned (pinned ones copy faster).  h_ldp in the ctx input precision (fp32 in RR_FP32
+ * and RR_MIXED), h_flux in the flux precision (fp32 only in RR_FP32).  Honours the table mode, the
+ * mean-k and the small-planet settings.  Needs rr_set_data.  Synchronous.  Afterwards the host-path
+ * buffers hold the LAST chunks only (rr_get_table / rr_get_rows refer to the device-pointer API).   */
 int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t npar, int64_t npv,
                      void *h_flux, int32_t *h_status);
 
