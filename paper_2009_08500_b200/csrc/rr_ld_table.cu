@@ -330,16 +330,29 @@ rr_ld_rows_bucket_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
   const double *pr = prof + lane * stride;
   const double ak = akr[lane];
   const int64_t orow = (int64_t)rid[lane] * ng;
-  for (int ig = warp; ig < ng; ig += 8) {
-    const double *w0 = W0 + (int64_t)ig * nz, *w1 = W1 + (int64_t)ig * nz;
-    double s0 = 0.0, s1 = 0.0;
-#pragma unroll 4
-    for (int j = 0; j < nz; ++j) {
-      const double p = pr[j];
-      s0 = fma(__ldg(w0 + j), p, s0);
-      s1 = fma(__ldg(w1 + j), p, s1);
+  // The weight rows of 8 g nodes at a time go through shared memory: all 256 threads load them
+  // coalesced (deep memory-level parallelism; read straight from L2 one element per FMA they left
+  // the FMA chains waiting on 300-cycle loads), then every warp takes one node, lane = row.
+  double *wb0 = prof + RB * stride, *wb1 = wb0 + 8 * nz;
+  for (int c0 = 0; c0 < ng; c0 += 8) {
+    const int nrow = min(8, ng - c0);
+    __syncthreads();                               // the previous chunk is consumed
+    for (int idx = threadIdx.x; idx < nrow * nz; idx += 256) {
+      wb0[idx] = __ldg(W0 + (int64_t)c0 * nz + idx);
+      wb1[idx] = __ldg(W1 + (int64_t)c0 * nz + idx);
     }
-    if (lane < nr) rows[orow + ig] = (TR)fma(ak, s1 - s0, s0);
+    __syncthreads();
+    if (warp < nrow) {
+      const double *w0 = wb0 + warp * nz, *w1 = wb1 + warp * nz;
+      double s0 = 0.0, s1 = 0.0;
+#pragma unroll 4
+      for (int j = 0; j < nz; ++j) {
+        const double p = pr[j];
+        s0 = fma(w0[j], p, s0);                    // warp-uniform shared loads: broadcasts
+        s1 = fma(w1[j], p, s1);
+      }
+      if (lane < nr) rows[orow + c0 + warp] = (TR)fma(ak, s1 - s0, s0);
+    }
   }
 }
 
@@ -445,7 +458,7 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
   if (wk->lazy == 2) return rr_ld_rows_direct_launch(ctx, wk, npv, st);
   const int nb = c.nk - 1;                         // buckets: lower k row ik in [0, nk-2]
   const int stride = ctx->nz | 1;
-  const size_t smem_b = sizeof(double) * RB * stride;
+  const size_t smem_b = sizeof(double) * (RB * stride + 16 * ctx->nz);   // profiles + 2 x 8 weight rows
   if (M >= 2048 && nb <= 4096 && smem_b <= 96 * 1024) {
     // bucketed builder
     const int64_t need = sizeof(int32_t) * (4 * (int64_t)nb + 4 + M);
