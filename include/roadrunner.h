@@ -4,7 +4,7 @@
  *
  * The method is H. Parviainen, "RoadRunner: a fast and flexible exoplanet transit model"
  * (arXiv:2009.08500).  Citations below are PAPER.md line numbers (section / equation); readings
- * of the paper where it is silent are numbered R1..R14 in DESIGN.md section 3.
+ * of the paper where it is silent are numbered R1..R15 in DESIGN.md section 3.
  *
  * The two calls of the problem statement are
  *     build_ld_table(ldp[npv x npb x nz])                                   -> rr_build_ld_table
@@ -118,7 +118,8 @@ int rr_get_ze(const rr_ctx *ctx, double *h_ze /*[nz+1]*/);
 int rr_get_weights(const rr_ctx *ctx, double *h_W /*[nk][ng][nz]*/);
 
 /* ---- data: paper's tm.set_data(times, lcids, pbids, nsamples, exptimes), PAPER.md:230-236 -----
- * d_times[npt]          mid-exposure times (days), fp64, any order
+ * d_times[npt]          mid-exposure times (days), fp64, any order; a NaN or infinite time gives
+ *                       NaN flux for that exposure (reading R15)
  * d_lc_index[npt]       light-curve index of each exposure, 0 <= . < nlc
  * h_passband_index[nlc] passband of each light curve, 0 <= . < npb     (reading R11: per light
  *                       curve, as in the paper; per-point passband = passband_index[lc_index[i]])

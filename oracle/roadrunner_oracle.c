@@ -327,6 +327,7 @@ void oracle_evaluate_mk(const double *times, const int32_t *lc_index, int64_t np
                 sum += front ? oracle_flux_from_table_kw(z, k, kw, Tvp, nk, k0, k1, ng, is) : 1.0;
             }
             flux[v * npt + i] = sum / (double)ns;        /* mean over sub-samples */
+            if (!isfinite(times[i])) flux[v * npt + i] = NAN;   /* reading R15: no time, no flux */
         }
     }
 }
@@ -421,6 +422,7 @@ void oracle_evaluate_direct(const double *times, const int32_t *lc_index, int64_
                 sum += front ? oracle_flux_from_row_kw(z, k, kw, ldw, ng, is) : 1.0;
             }
             flux[v * npt + i] = sum / (double)ns;
+            if (!isfinite(times[i])) flux[v * npt + i] = NAN;   /* reading R15 */
         }
     }
 }

@@ -687,6 +687,22 @@ def test_long_exposures_many_subsamples_and_distant_epochs(rr, precision):
     gm.close()
 
 
+@pytest.mark.parametrize("precision", [0, 1, 2])
+def test_non_finite_times(rr, precision):
+    """Reading R15: NaN / infinite times give NaN flux for those exposures in every layout
+    (thread per exposure, lanes over sub-samples); everything else matches the oracle."""
+    wl = workloads.make_workload(3, npv=5, npt=6 * 300)
+    rng = np.random.default_rng(9)
+    bad = rng.choice(wl.npt, 25, replace=False)
+    wl.times[bad] = rng.choice([np.nan, np.inf, -np.inf], 25)
+    want, _ = oracle_flux(wl)
+    for reduction in (1, 2):
+        got = gpu_flux(rr, wl, precision=precision, reduction=reduction)
+        assert np.array_equal(np.isnan(got), np.isnan(want)) and np.isnan(want).sum() == 25 * 5
+        ok = ~np.isnan(want)
+        assert np.max(np.abs(got[ok] - want[ok])) <= {0: TOL64, 1: TOL32, 2: 2e-8}[precision]
+
+
 def test_uniform_disk_closed_form(rr):
     """ldp = 1: flux = 1 - a(z,k)/pi straight from the CUDA path."""
     wl = workloads.make_workload(1, npv=8, npt=2000)

@@ -258,3 +258,16 @@ def test_config0_worked_example():
     dt = wl.times[1] - wl.times[0]
     assert abs(n_in - t14 / dt) <= 1.0
     assert abs(flux[0].min() - (1 - k * k * 1.18)) < 2e-3     # depth ~ k^2 x limb-darkening boost
+
+
+def test_non_finite_times_give_nan_flux():
+    """Reading R15: a NaN / infinite exposure time -> NaN flux for that exposure, every pv; the other
+    exposures are untouched."""
+    wl = make_workload(3, npv=3, npt=6 * 20)
+    ref, _ = oracle.evaluate_workload(wl)
+    bad = [5, 40, 77]
+    wl.times[bad] = [np.nan, np.inf, -np.inf]
+    got, _ = oracle.evaluate_workload(wl)
+    assert np.all(np.isnan(got[:, bad]))
+    ok = np.setdiff1d(np.arange(wl.npt), bad)
+    assert np.array_equal(got[:, ok], ref[:, ok])
