@@ -31,6 +31,10 @@
 // flux is written once and never re-read: streaming stores keep W, times and the rows in L2
 #define RR_STORE(p, v) __stcs((p), (v))
 
+// Dynamic shared memory of rr_flux_kernel and rr_orbit_kernel.  Global scope: the PTX symbol is
+// "rr_dyn", which the inline loads of Cst<> name directly.
+extern __shared__ __align__(16) unsigned char rr_dyn[];
+
 namespace {
 
 #ifndef RR_FLUX_THREADS
@@ -200,7 +204,11 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
 // ---- per-(tile, pv) constants, staged in shared memory in the working precision -----------------------
 // Read with volatile loads at the point of use: they are warp-uniform broadcasts that ride in the
 // issue slots the half-rate FP64 pipe leaves free, and keeping ~25 of them out of registers is what
-// lets 4 blocks of 256 threads share an SM.
+// lets 8 blocks of 128 threads share an SM.  The loads name the dynamic shared array by its PTX
+// symbol (rr_dyn, declared at global scope so that the name is not mangled) with an immediate
+// offset: ptxas then addresses them off the shared-window base it keeps in a UNIFORM register
+// (LDS [UR+imm]); round 1 passed the address in a vector register, which ptxas rematerialised
+// with S2R/LEA at every use (5 instructions per sub-sample).
 enum {
   K_ZC0, K_ZC1,           // circular (pair)
   K_CD, K_SD,             // circular: cos, sin of the phase step between sub-samples (pair)
@@ -211,60 +219,54 @@ enum {
   K_X1, K_X2,             // (pair)
   K_Y1, K_Y2,             // (pair)
   K_Y0, K_ACI2,           // (pair)
-  K_E, K_SE, K_CE,        // robust solver path
-  K_OPK2,                 // radius ratio
-  K_OMK2, K_AFULL,        // (pair)
-  K_GSCALE, K_K,          // (pair)
-  K_OPK, K_K2,            // (pair)
-  K_OMK,
-  K_COUNT,
-  K_SCALE = K_COUNT,      // 1 / (Istar ns)
+  K_E, K_SE,              // robust solver path (pair)
+  K_CE, K_OPK2,           // (1+k)^2
+  K_OMK2, K_AFULL,        // (1-k)^2, pi min(1,k)^2 (pair)
+  K_GSCALE, K_OPK,        // (ng-1)/(1+kw), 1+k (pair)
+  K_OMKS, K_K2,           // 1-k (signed), k^2 (pair)
+  K_2K2, K_SCALE,         // 2 k^2, 1/(Istar ns) (pair)
   K_TOTAL,
+  K_COUNT = K_SCALE,      // entries rr_stage_constants writes
   K_SMEM = (K_TOTAL + 3) & ~3   // 16-byte multiple in both precisions
 };
-static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_OMK2 % 2 == 0 && K_GSCALE % 2 == 0 && K_OPK % 2 == 0, "pairs");
+static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_E % 2 == 0 && K_OMK2 % 2 == 0 &&
+              K_GSCALE % 2 == 0 && K_OMKS % 2 == 0 && K_2K2 % 2 == 0, "pairs");
+template <typename T> struct Vec2T;
+template <> struct Vec2T<double> { using type = double2; };
+template <> struct Vec2T<float> { using type = float2; };
+
+// Shared memory of the flux and orbit kernels: cst[K_SMEM] | ldw2[ldw_len] (node, slope) pairs.
 template <typename R> struct Cst {
-  unsigned base;   // 32-bit shared-window address of cst[0]
-  __device__ __forceinline__ explicit Cst(const R *cst) {
-    const unsigned a = (unsigned)__cvta_generic_to_shared(cst);
-    // fp32 has a register to spare: an opaque move keeps the address instead of rematerialising it
-    // at every load; in fp64 (64-register budget) holding it costs more than recomputing (measured)
-    if constexpr (sizeof(R) == 4) asm volatile("mov.u32 %0, %1;" : "=r"(base) : "r"(a));
-    else base = a;
-  }
-  __device__ __forceinline__ R operator[](int i) const {
+  static __device__ __forceinline__ R *base() { return reinterpret_cast<R *>(rr_dyn); }
+  template <int I> static __device__ __forceinline__ R get() {
     R v;
     if constexpr (sizeof(R) == 8)
-      asm volatile("ld.volatile.shared.f64 %0, [%1];" : "=d"(v) : "r"(base + 8u * i));
+      asm volatile("ld.volatile.shared.f64 %0, [rr_dyn+%1];" : "=d"(v) : "n"(8 * I));
     else
-      asm volatile("ld.volatile.shared.f32 %0, [%1];" : "=f"(v) : "r"(base + 4u * i));
+      asm volatile("ld.volatile.shared.f32 %0, [rr_dyn+%1];" : "=f"(v) : "n"(4 * I));
     return v;
   }
-  // the two table nodes ldw[ig], ldw[ig+1] of the row staged K_SMEM elements after the constants
-  __device__ __forceinline__ void nodes(int ig, R &l0, R &l1) const {
-    const unsigned a = base + (unsigned)sizeof(R) * (unsigned)(K_SMEM + ig);
-    if constexpr (sizeof(R) == 8) {
-      asm volatile("ld.shared.f64 %0, [%1];" : "=d"(l0) : "r"(a));
-      asm volatile("ld.shared.f64 %0, [%1+8];" : "=d"(l1) : "r"(a));
-    } else {
-      asm volatile("ld.shared.f32 %0, [%1];" : "=f"(l0) : "r"(a));
-      asm volatile("ld.shared.f32 %0, [%1+4];" : "=f"(l1) : "r"(a));
-    }
+  // two neighbouring constants (I even) with one 16-/8-byte shared load
+  template <int I> static __device__ __forceinline__ void pair(double &a, double &b) {
+    static_assert(I % 2 == 0, "pair");
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [rr_dyn+%2];" : "=d"(a), "=d"(b) : "n"(8 * I));
   }
-  // two neighbouring constants (i even) with one 16-/8-byte shared load
-  __device__ __forceinline__ void pair(int i, double &a, double &b) const {
-    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];"
-                 : "=d"(a), "=d"(b) : "r"(base + 8u * i));
+  template <int I> static __device__ __forceinline__ void pair(float &a, float &b) {
+    static_assert(I % 2 == 0, "pair");
+    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [rr_dyn+%2];" : "=f"(a), "=f"(b) : "n"(4 * I));
   }
-  __device__ __forceinline__ void pair(int i, float &a, float &b) const {
-    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];"
-                 : "=f"(a), "=f"(b) : "r"(base + 4u * i));
+  // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
+  using R2 = typename Vec2T<R>::type;
+  static __device__ __forceinline__ R2 *row() { return reinterpret_cast<R2 *>(rr_dyn) + K_SMEM / 2; }
+  static __device__ __forceinline__ void cell(int ig, R &l0, R &sl) {
+    const R2 v = row()[ig];
+    l0 = v.x;
+    sl = v.y;
   }
 };
 
 template <typename R>
-__device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, const RRPvBand &b,
-                                                   double du) {
+__device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRPvBand &b, double du) {
   const int t = threadIdx.x;
   double v = 0.0;
   switch (t) {
@@ -279,14 +281,14 @@ __device__ __forceinline__ void rr_stage_constants(R *cst, const RRPvOrbit &o, c
     case K_X1: v = o.X1; break;         case K_X2: v = o.X2; break;
     case K_Y0: v = o.Y0; break;         case K_Y1: v = o.Y1; break;
     case K_Y2: v = o.Y2; break;         case K_ACI2: v = o.aci2; break;
-    case K_K: v = b.k; break;           case K_OPK: v = b.opk; break;
-    case K_OPK2: v = b.opk * b.opk; break;
-    case K_OMK: v = b.omk; break;       case K_AFULL: v = b.afull; break;
+    case K_OPK: v = b.opk; break;       case K_OPK2: v = b.opk * b.opk; break;
+    case K_OMKS: v = 1.0 - b.k; break;  case K_AFULL: v = b.afull; break;
     case K_K2: v = b.k2; break;         case K_GSCALE: v = b.gscale; break;
     case K_OMK2: v = b.omk * b.omk; break;
+    case K_2K2: v = 2.0 * b.k2; break;
     default: break;
   }
-  if (t < K_COUNT) cst[t] = (R)v;
+  if (t < K_COUNT) Cst<R>::base()[t] = (R)v;
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
@@ -328,32 +330,36 @@ __device__ RR_ROBUST_INLINE int rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out
 // ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
 // Returns z^2; front = planet between observer and star.  iters counts sincos evaluations.
 template <typename R, bool CIRC>
-__device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &front, int &iters) {
+__device__ __forceinline__ R rr_separation2(double ur, bool &front, int &iters) {
+  using K = Cst<R>;
   if (CIRC) {
     // e = 0: z^2 = a^2 (sin^2 phi + cos^2 phi cos^2 i) = a^2 cos^2 i + a^2 sin^2 i sin^2 phi
     R s;
-    if (fabs(ur) <= 0.0795) {
+    if (fabs(ur) <= 0.07949995994567871) {             // 0x3FB45A1C'00000000: 2 pi u <= 0.4995
       R cm1;
-      rr_sincosm1_small((R)(RR_TWOPI * ur), s, cm1);   // |x| <= 0.4995
+      rr_sincosm1_small((R)(RR_TWOPI * ur), s, cm1);
     } else {
       s = rr_sinpi((R)(2.0 * ur));
     }
     front = fabs(ur) < 0.25;
     R zc0, zc1;
-    k.pair(K_ZC0, zc0, zc1);
+    K::template pair<K_ZC0>(zc0, zc1);
     return fma(s * s, zc1, zc0);
   }
-  const R dM = (R)(RR_TWOPI * ur);
   R s2, cm2;
   bool done = false;
+  R dM;
   {
     R c4, c3, c2, ky, B, C, A, tol;
-    k.pair(K_C4, c4, c3);
-    k.pair(K_C2, c2, ky);
+    K::template pair<K_C4>(c4, c3);
+    K::template pair<K_C2>(c2, ky);
     const R y = (R)ur * ky;                            // dM / A
     R d = y * fma(y, fma(y, fma(y, c4, c3), c2), (R)1);
-    k.pair(K_B, B, C);
-    k.pair(K_A, A, tol);
+    K::template pair<K_B>(B, C);
+    K::template pair<K_A>(A, tol);
+    // 2 pi ur: fp64 takes it from y (one FP64 instruction, no 64-bit constant); fp32 rounds the
+    // fp64 product once (y A would add two fp32 roundings to the Kepler residual)
+    dM = sizeof(R) == 8 ? y * A : (R)(RR_TWOPI * ur);
     // Halley steps from the series starter while d stays in the polynomial range; the first one
     // is accepted for ~94 % of config 4's eccentric sub-samples
 #pragma unroll 1
@@ -379,11 +385,15 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
       d += dd;
     }
   }
-  if (!done) iters += rr_kepler_robust<R>(k[K_E], k[K_SE], k[K_CE], dM, &s2, &cm2);
+  if (!done) {
+    R e, sE;
+    K::template pair<K_E>(e, sE);
+    iters += rr_kepler_robust<R>(e, sE, K::template get<K_CE>(), (R)(RR_TWOPI * ur), &s2, &cm2);
+  }
   R X1, X2, Y1, Y2, Y0, aci2;
-  k.pair(K_X1, X1, X2);
-  k.pair(K_Y1, Y1, Y2);
-  k.pair(K_Y0, Y0, aci2);
+  K::template pair<K_X1>(X1, X2);
+  K::template pair<K_Y1>(Y1, Y2);
+  K::template pair<K_Y0>(Y0, aci2);
   const R xs = fma(X1, cm2, X2 * s2);
   const R ys = Y0 + fma(Y1, cm2, Y2 * s2);
   front = ys > (R)0;
@@ -392,8 +402,8 @@ __device__ __forceinline__ R rr_separation2(const Cst<R> k, double ur, bool &fro
 
 // ---- kernel 3 core: occulted light ip * ap of one sub-sample with z < 1+k ------
 // Table cell of y = g/dg in [0, ng-1]: lower node ig and weight ag = y - ig.  The staged row carries
-// one extra node ldw[ng] = ldw[ng-1], so that y = ng-1 (z = 1+k to rounding) needs no clamp: it
-// lands in cell ng-1 with ag = 0 (reading R10: the same value as cell ng-2 with ag = 1).
+// one extra cell (node ldw[ng-1], slope 0), so that y = ng-1 (z = 1+k to rounding) needs no clamp
+// (reading R10: the same value as cell ng-2 with ag = 1).
 __device__ __forceinline__ void rr_cell(double y, int &ig, double &ag) {
   ig = __double2int_rd(y);                   // conversion unit, not the FP64 pipe
   ag = y - __int2double_rn(ig);
@@ -404,36 +414,42 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
 }
 
 template <typename R>
-__device__ __forceinline__ R rr_deficit(R z2, const Cst<R> k, const R *__restrict__ ldw, int ng,
-                                        int &ningress) {
-  R z = rr_sqrt_pos(z2);
+__device__ __forceinline__ R rr_deficit(R z2, int &ningress) {
+  using K = Cst<R>;
+  const R z = rr_sqrt3_pos(z2);
   int ig;
   R ag;
-  R gscale, kk;
-  k.pair(K_GSCALE, gscale, kk);
+  R gscale, opk;
+  K::template pair<K_GSCALE>(gscale, opk);
   rr_cell(z * gscale, ig, ag);
-  R l0, l1;
-  k.nodes(ig, l0, l1);              // = ldw[ig], ldw[ig + 1]
-  R ip = fma(ag, l1 - l0, l0);              // mean occulted brightness
+  R l0, sl;
+  K::cell(ig, l0, sl);                      // ldw[ig], ldw[ig+1] - ldw[ig]
+  const R ip = fma(ag, sl, l0);             // mean occulted brightness
   R ap;
   R omk2, afull;
-  k.pair(K_OMK2, omk2, afull);
+  K::template pair<K_OMK2>(omk2, afull);
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
   } else {
-    // lens of the unit disc and the disc of radius k at distance z (reading R9, atan2 form):
-    // two sectors minus the kite, kite = 4 x area of the triangle (1, k, z)
-    R opk, k2;
-    k.pair(K_OPK, opk, k2);
-    R kite = rr_sqrt((opk - z) * (z + (R)1 - kk) * (z - (R)1 + kk) * (z + opk));
-    // half-angle at the star's centre: at most asin k, so for k <= sin(pi/8) (block-uniform) its
-    // tangent needs no octant reduction
-    const R x1 = fma(z - kk, z + kk, (R)1);
-    R th1;
-    if (k2 <= (R)0.1464) th1 = rr_atan_small(kite, x1);
-    else th1 = rr_atan2_pos(kite, x1);
-    R th2 = rr_atan2_pos(kite, fma(z - (R)1, z + (R)1, k2));
-    ap = th1 + k2 * th2 - (R)0.5 * kite;
+    // Lens of the unit disc and the disc of radius k at distance z (reading R9): two sectors minus
+    // the kite.  With A = 1+k-z, B = z+1-k, C = z-1+k, D = z+1+k (all >= 0 here):
+    //   kite = sqrt(A B C D) = 4 x area of the triangle (1, k, z),
+    //   half-angle at the star's centre   th1/2 = atan(kite / (B D))   [tan^2 = A C / (B D)],
+    //   half-angle at the planet's centre th2/2 = atan(kite / (C D))   [tan^2 = A B / (C D)],
+    // the half-angle formulas of the triangle: both arguments are >= 0 (no sign cases), th1/2 <=
+    // asin(k)/2 needs no octant reduction for k^2 <= 1/2 and th2/2 in [0, pi/2] needs one of three
+    // cases.  ap = th1 + k^2 th2 - kite/2.
+    R omks, k2;
+    K::template pair<K_OMKS>(omks, k2);
+    const R A = opk - z, B = z + omks, C = z - omks, D = z + opk;
+    const R AB = fabs(A * B), S = fabs(C * D), Q = B * D;
+    const R kite = rr_sqrt3_pos(AB * S);
+    R h1;
+    if (k2 <= (R)0.5) h1 = rr_atan_t(rr_div3(kite, Q));
+    else h1 = rr_atan_quadrant<R>(kite, Q, fabs(A * C));
+    const R h2 = rr_atan_quadrant<R>(kite, S, AB);
+    const R tk2 = K::template get<K_2K2>();
+    ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
     ++ningress;
   }
   return ip * ap;
@@ -491,7 +507,6 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
 template <typename R, bool COUNT, bool CIRC, bool NOWRAP>
 __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
-                                          const Cst<R> k, const R *__restrict__ ldw, int ng,
                                           unsigned long long *cnt) {
   // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
   const double wr = NOWRAP ? w : w - rr_round(w);
@@ -499,9 +514,9 @@ __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
   if (fabs(wr) <= hwid) {
     bool front;
     int it = 0, ing = 0;
-    R z2 = rr_separation2<R, CIRC>(k, wr + u_mid, front, it);
-    if (front && z2 < k[K_OPK2]) {
-      def = rr_deficit<R>(z2, k, ldw, ng, ing);
+    R z2 = rr_separation2<R, CIRC>(wr + u_mid, front, it);
+    if (front && z2 < Cst<R>::template get<K_OPK2>()) {
+      def = rr_deficit<R>(z2, ing);
       if (COUNT) { cnt[3]++; cnt[4] += ing; }
     }
     if (COUNT) { cnt[CIRC ? 1 : 2]++; cnt[5] += it; }
@@ -518,8 +533,8 @@ template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP>
 __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__restrict__ out,
                                         int count, int ns, int shuffle, double t0, double inv_p,
                                         double u_mid, double hwid, double hw, O scale,
-                                        const Cst<R> k, const R *__restrict__ ldw, int ng,
                                         unsigned long long *cnt) {
+  using K = Cst<R>;
   const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
   const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
   const double hskip = hwid + hw;
@@ -532,11 +547,9 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
       const double wc = fma(tcur - t0, inv_p, -u_mid);
       const double wr = wc - rr_round(wc);           // exposure centre from the window centre
       O f;
-      if (fabs(wr) > hskip) {
-        f = (O)1;
+      if (!(fabs(wr) <= hskip)) {
+        f = (wr == wr) ? (O)1 : rr_nan<O>();         // out of the window; NaN time: reading R15
         if (COUNT) cnt[0] += ns;
-      } else if (!(wr == wr)) {
-        f = rr_nan<O>();
       } else {
         O acc = (O)0;
         if (CIRC && sizeof(R) == 8) {
@@ -546,7 +559,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
           // sub-sample: a rotation's ABSOLUTE rounding error times a is too much for z there.)
           const double ur0 = (wr + off0) + u_mid;
           R sn, cs;
-          if (fabs(ur0) <= 0.0795) {
+          if (fabs(ur0) <= 0.07949995994567871) {    // 0x3FB45A1C'00000000: 2 pi u <= 0.4995
             R cm1;
             rr_sincosm1_small((R)(RR_TWOPI * ur0), sn, cm1);
             cs = (R)1 + cm1;
@@ -557,14 +570,14 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
             cs = (R)c_;
           }
           R zc0, zc1, cd, sd;
-          k.pair(K_ZC0, zc0, zc1);
-          k.pair(K_CD, cd, sd);
-          const R opk2 = k[K_OPK2];
+          K::template pair<K_ZC0>(zc0, zc1);
+          K::template pair<K_CD>(cd, sd);
+          const R opk2 = K::template get<K_OPK2>();
           for (int s = 0; s < ns; ++s) {
             const R z2 = fma(sn * sn, zc1, zc0);
             if (cs > (R)0 && z2 < opk2) {
               int ing = 0;
-              acc += rr_deficit<R>(z2, k, ldw, ng, ing);
+              acc += rr_deficit<R>(z2, ing);
               if (COUNT) { cnt[3]++; cnt[4] += ing; }
             }
             const R s1 = fma(sn, cd, cs * sd);
@@ -575,7 +588,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC, NOWRAP>(w, u_mid, hwid, k, ldw, ng, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP>(w, u_mid, hwid, cnt);
         }
         f = fma(-acc, scale, (O)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
@@ -598,8 +611,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         if (fabs(wr) <= hskip) {
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
-            acc += rr_subsample<R, COUNT, CIRC, false>(fma(du, (double)s, w0), u_mid, hwid, k, ldw, ng,
-                                                cnt);
+            acc += rr_subsample<R, COUNT, CIRC, false>(fma(du, (double)s, w0), u_mid, hwid, cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
         }
@@ -614,14 +626,13 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
 // The pv's constants are staged once per block, the k-collapsed table row once per light curve the
 // chunk meets; tiles outside the transit window are merged into contiguous runs and written as
 // flux = 1 with 16-byte stores, without touching the orbit.
-// Shared memory: cst[K_SMEM] (constants, working precision) | ldw[ng+1] (k-collapsed table row).
+// Shared memory (rr_dyn): cst[K_SMEM] (constants, working precision) | ldw2[ldw_len] (node, slope)
+// pairs of the k-collapsed table row.
 template <typename R, typename O, bool COUNT>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
-  extern __shared__ __align__(16) unsigned char rr_smem[];
-  R *cst = reinterpret_cast<R *>(rr_smem);             // fixed offsets: immediates in the loads
-  R *ldw = cst + K_SMEM;
-  const Cst<R> k(cst);
+  using K = Cst<R>;
+  using R2 = typename K::R2;
   __shared__ unsigned tflags[FT / 32];
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
@@ -692,41 +703,53 @@ rr_flux_kernel(const FluxParams P) {
       }
       if (COUNT) ceval += (threadIdx.x == 0);
       if (tlc != staged_lc) {
-        // stage the k-collapsed table row ldw[ng] and the constants in shared memory
+        // stage the k-collapsed table row ldw[ng] as (node, slope) cells, and the
+        // constants, in shared memory
         const int kb = (P.nkpb == 1) ? 0 : lc.pb;
         const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
         const int64_t trow = (int64_t)v * P.npb + lc.pb;
+        R2 *ldw2 = K::row();
         __syncthreads();
         if (P.rows) {                                  // lazy mode: the row was collapsed for this k
           const R *rw = reinterpret_cast<const R *>(P.rows) + trow * (int64_t)P.ng;
-          for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) ldw[ig] = rw[min(ig, P.ng - 1)];
+          for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) {
+            const R a = rw[min(ig, P.ng - 1)], b = rw[min(ig + 1, P.ng - 1)];
+            R2 c;
+            c.x = a;
+            c.y = b - a;
+            ldw2[ig] = c;
+          }
         } else {
           const R *T0 = reinterpret_cast<const R *>(P.T) + (trow * P.nk + pb.ik) * (int64_t)P.ng;
           const R *T1 = T0 + P.ng;
           const R ak = (R)pb.ak;
           for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) {
-            const int jg = min(ig, P.ng - 1);          // ldw[ng..] = ldw[ng-1]: see rr_cell
-            ldw[ig] = fma(ak, T1[jg] - T0[jg], T0[jg]);
+            const int jg = min(ig, P.ng - 1), jh = min(ig + 1, P.ng - 1);   // cells >= ng-1: flat
+            const R a = fma(ak, T1[jg] - T0[jg], T0[jg]), b = fma(ak, T1[jh] - T0[jh], T0[jh]);
+            R2 c;
+            c.x = a;
+            c.y = b - a;
+            ldw2[ig] = c;
           }
         }
-        rr_stage_constants<R>(cst, po, pb, 2.0 * hw / lc.ns);
-        if (threadIdx.x == K_COUNT)
-          cst[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
+        rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns);
+        if (threadIdx.x == K_SCALE)
+          K::base()[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
         __syncthreads();
-        scale = (O)k[K_SCALE];
+        scale = (O)K::template get<K_SCALE>();
         staged_lc = tlc;
       }
       const int shuffle = lc.ns >= P.shuffle_min_ns;
       const bool nowrap = hwid + 2.0 * hw < 0.499;
       if (circular)
         rr_tile<R, O, COUNT, true, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                       inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+                                          inv_p, u_mid, hwid, hw, scale, cnt);
       else if (nowrap)
         rr_tile<R, O, COUNT, false, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                       inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+                                          inv_p, u_mid, hwid, hw, scale, cnt);
       else
         rr_tile<R, O, COUNT, false, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                        inv_p, u_mid, hwid, hw, scale, k, ldw, P.ng, cnt);
+                                           inv_p, u_mid, hwid, hw, scale, cnt);
     }
   }
   if (f0 >= 0) rr_fill<O>(row + f0, f1 - f0, (O)1);
@@ -750,8 +773,6 @@ __global__ void __launch_bounds__(FT)
 rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ tiles,
                 const RRLc *__restrict__ lcs, const RRPvOrbit *__restrict__ pvo, int64_t ntiles,
                 int64_t npv, int64_t nsub, double *__restrict__ zout) {
-  __shared__ __align__(16) R cst[K_TOTAL];
-  const Cst<R> k(cst);
   const int64_t total = ntiles * npv;
   for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
     const int64_t v = w / ntiles;
@@ -768,7 +789,7 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
     }
     RRPvBand nob = {};
     __syncthreads();
-    rr_stage_constants<R>(cst, po, nob, 0.0);
+    rr_stage_constants<R>(po, nob, 0.0);
     __syncthreads();
     const double hw = 0.5 * lc.exptime * po.inv_p;
     const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0);
@@ -778,8 +799,8 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
       double ur = us - rint(us);
       bool front;
       int it = 0;
-      R z2 = po.circular ? rr_separation2<R, true>(k, ur, front, it)
-                         : rr_separation2<R, false>(k, ur, front, it);
+      R z2 = po.circular ? rr_separation2<R, true>(ur, front, it)
+                         : rr_separation2<R, false>(ur, front, it);
       double z = (double)rr_sqrt(z2);
       out[j] = front ? z : -z;
     }
@@ -914,7 +935,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8);
   if (ctx->counters_on)
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
   using Kernel = void (*)(const FluxParams);
@@ -937,10 +958,10 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
   if (fp32_math)
-    rr_orbit_kernel<float><<<grid, FT, 0, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
+    rr_orbit_kernel<float><<<grid, FT, K_SMEM * sizeof(float), st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
                                                 ctx->ntiles, npv, ctx->nsub, d_z);
   else
-    rr_orbit_kernel<double><<<grid, FT, 0, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
+    rr_orbit_kernel<double><<<grid, FT, K_SMEM * sizeof(double), st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
