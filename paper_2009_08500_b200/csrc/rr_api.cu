@@ -113,6 +113,7 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * 8);
   if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, sizeof(unsigned long long) * 8);
   if (e != cudaSuccess) rc = RR_ECUDA_BASE - (int)e;
+  if (rc == RR_OK) rc = rr_smem_probe(&ctx->smem_abs);
   if (rc == RR_OK) rc = rr_geometry_build(ctx);
   if (rc != RR_OK) {
     cudaGetLastError();

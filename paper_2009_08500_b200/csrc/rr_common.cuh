@@ -92,6 +92,7 @@ struct rr_ctx {
   int nz;
   int device;
   int sm_count;
+  int smem_abs;         // 1: the flux kernels may address shared memory absolutely (rr_smem_probe)
   // geometry (a0)
   double *d_ze, *d_zm, *d_mu, *d_q, *d_W;
   std::vector<double> h_ze, h_mu;
@@ -162,3 +163,4 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
 int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_math,
                     cudaStream_t st);
 int rr_fma_peak_launch(int precision, double *h_fma_per_s, cudaStream_t st);   // rr_flux.cu
+int rr_smem_probe(int *abs_ok);                                                // rr_flux.cu

@@ -235,35 +235,101 @@ template <typename T> struct Vec2T;
 template <> struct Vec2T<double> { using type = double2; };
 template <> struct Vec2T<float> { using type = float2; };
 
-// Shared memory of the flux and orbit kernels: cst[K_SMEM] | ldw2[ldw_len] (node, slope) pairs.
-template <typename R> struct Cst {
+// Shared memory of the flux and orbit kernels (all dynamic, the kernels have no static shared
+// memory): cst[K_SMEM] | tile flags (16 B) | ldw2[ldw_len] (node, slope) pairs.
+// How the loads are addressed (template parameter M of Cst):
+//   RR_SM_SYMBOL  by the PTX symbol rr_dyn + immediate: ptxas derives the shared-window base where it
+//                 needs it (S2UR + ULEA, or S2R + LEA inside loops: 3-5 instructions per use site)
+//   RR_SM_HELD    off a base address held in one register, made opaque to ptxas by a warp shuffle
+//                 so that it is neither rematerialised nor copy-propagated away (costs a register)
+//   RR_SM_ABS     absolute shared::cta addresses RR_SMEM_ABS + offset as immediates: one LDS per load,
+//                 no address arithmetic, no register.  rr_dyn starts at the bytes the runtime reserves
+//                 (cudaDevAttrReservedSharedMemoryPerBlock = 1024 on sm_100) because these kernels
+//                 have no static shared memory; rr_create verifies that with a probe kernel (and
+//                 falls back to RR_SM_SYMBOL otherwise), and every block re-checks and traps.
+// Measured (config 4, flux kernel): fp64 symbol 5.75 ms, held 6.07 ms (the 64-register budget is full:
+// the held register spills); fp32 symbol 3.93 ms, held 3.83 ms.
+enum { RR_SM_SYMBOL = 0, RR_SM_HELD = 1, RR_SM_ABS = 2 };
+#define RR_SMEM_ABS 1024
+#ifndef RR_SM_FALLBACK_F64
+#define RR_SM_FALLBACK_F64 RR_SM_SYMBOL
+#endif
+#ifndef RR_SM_FALLBACK_F32
+#define RR_SM_FALLBACK_F32 RR_SM_HELD
+#endif
+template <typename R, int M> struct Cst {
+  static constexpr int ES = (int)sizeof(R);
+  static constexpr int OFF_FLAGS = K_SMEM * ES, OFF_ROW = OFF_FLAGS + 16;
+  unsigned sb;   // RR_SM_HELD: shared-window address of rr_dyn; RR_SM_ABS: 0
+  __device__ __forceinline__ Cst() {
+    if constexpr (M == RR_SM_HELD) {
+      sb = __shfl_sync(0xffffffffu, (unsigned)__cvta_generic_to_shared(rr_dyn), 0);
+    } else {
+      sb = 0;
+      if constexpr (M == RR_SM_ABS)
+        if ((unsigned)__cvta_generic_to_shared(rr_dyn) != RR_SMEM_ABS) __trap();
+    }
+  }
   static __device__ __forceinline__ R *base() { return reinterpret_cast<R *>(rr_dyn); }
-  template <int I> static __device__ __forceinline__ R get() {
+  static __device__ __forceinline__ unsigned *flags() {
+    return reinterpret_cast<unsigned *>(rr_dyn + OFF_FLAGS);
+  }
+  template <int I> __device__ __forceinline__ R get() const {
     R v;
-    if constexpr (sizeof(R) == 8)
-      asm volatile("ld.volatile.shared.f64 %0, [rr_dyn+%1];" : "=d"(v) : "n"(8 * I));
-    else
-      asm volatile("ld.volatile.shared.f32 %0, [rr_dyn+%1];" : "=f"(v) : "n"(4 * I));
+    if constexpr (M == RR_SM_SYMBOL) {
+      if constexpr (ES == 8)
+        asm volatile("ld.volatile.shared.f64 %0, [rr_dyn+%1];" : "=d"(v) : "n"(8 * I));
+      else
+        asm volatile("ld.volatile.shared.f32 %0, [rr_dyn+%1];" : "=f"(v) : "n"(4 * I));
+    } else {
+      constexpr int off = (M == RR_SM_ABS ? RR_SMEM_ABS : 0) + ES * I;
+      if constexpr (ES == 8)
+        asm volatile("ld.volatile.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(sb), "n"(off));
+      else
+        asm volatile("ld.volatile.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(sb), "n"(off));
+    }
     return v;
   }
   // two neighbouring constants (I even) with one 16-/8-byte shared load
-  template <int I> static __device__ __forceinline__ void pair(double &a, double &b) {
+  template <int I> __device__ __forceinline__ void pair(double &a, double &b) const {
     static_assert(I % 2 == 0, "pair");
-    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [rr_dyn+%2];" : "=d"(a), "=d"(b) : "n"(8 * I));
+    if constexpr (M == RR_SM_SYMBOL)
+      asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [rr_dyn+%2];" : "=d"(a), "=d"(b) : "n"(8 * I));
+    else
+      asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b)
+                   : "r"(sb), "n"((M == RR_SM_ABS ? RR_SMEM_ABS : 0) + 8 * I));
   }
-  template <int I> static __device__ __forceinline__ void pair(float &a, float &b) {
+  template <int I> __device__ __forceinline__ void pair(float &a, float &b) const {
     static_assert(I % 2 == 0, "pair");
-    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [rr_dyn+%2];" : "=f"(a), "=f"(b) : "n"(4 * I));
+    if constexpr (M == RR_SM_SYMBOL)
+      asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [rr_dyn+%2];" : "=f"(a), "=f"(b) : "n"(4 * I));
+    else
+      asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(a), "=f"(b)
+                   : "r"(sb), "n"((M == RR_SM_ABS ? RR_SMEM_ABS : 0) + 4 * I));
   }
   // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
   using R2 = typename Vec2T<R>::type;
-  static __device__ __forceinline__ R2 *row() { return reinterpret_cast<R2 *>(rr_dyn) + K_SMEM / 2; }
-  static __device__ __forceinline__ void cell(int ig, R &l0, R &sl) {
-    const R2 v = row()[ig];
-    l0 = v.x;
-    sl = v.y;
+  static __device__ __forceinline__ R2 *row() { return reinterpret_cast<R2 *>(rr_dyn + OFF_ROW); }
+  __device__ __forceinline__ void cell(int ig, R &l0, R &sl) const {
+    if constexpr (M == RR_SM_SYMBOL) {
+      const R2 v = row()[ig];
+      l0 = v.x;
+      sl = v.y;
+    } else {
+      const unsigned a = sb + (unsigned)(2 * ES) * (unsigned)ig;
+      constexpr int off = (M == RR_SM_ABS ? RR_SMEM_ABS : 0) + OFF_ROW;
+      if constexpr (ES == 8)
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(l0), "=d"(sl) : "r"(a), "n"(off));
+      else
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(l0), "=f"(sl) : "r"(a), "n"(off));
+    }
   }
 };
+
+// rr_create's probe: the shared::cta address of rr_dyn in a kernel without static shared memory
+__global__ void rr_smem_probe_kernel(unsigned *out) {
+  if (threadIdx.x == 0) out[0] = (unsigned)__cvta_generic_to_shared(rr_dyn);
+}
 
 template <typename R>
 __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRPvBand &b, double du) {
@@ -288,7 +354,7 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
     case K_2K2: v = 2.0 * b.k2; break;
     default: break;
   }
-  if (t < K_COUNT) Cst<R>::base()[t] = (R)v;
+  if (t < K_COUNT) reinterpret_cast<R *>(rr_dyn)[t] = (R)v;
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
@@ -329,9 +395,8 @@ __device__ RR_ROBUST_INLINE int rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out
 
 // ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
 // Returns z^2; front = planet between observer and star.  iters counts sincos evaluations.
-template <typename R, bool CIRC>
-__device__ __forceinline__ R rr_separation2(double ur, bool &front, int &iters) {
-  using K = Cst<R>;
+template <typename R, bool CIRC, int M>
+__device__ __forceinline__ R rr_separation2(const Cst<R, M> K, double ur, bool &front, int &iters) {
   if (CIRC) {
     // e = 0: z^2 = a^2 (sin^2 phi + cos^2 phi cos^2 i) = a^2 cos^2 i + a^2 sin^2 i sin^2 phi
     R s;
@@ -343,7 +408,7 @@ __device__ __forceinline__ R rr_separation2(double ur, bool &front, int &iters) 
     }
     front = fabs(ur) < 0.25;
     R zc0, zc1;
-    K::template pair<K_ZC0>(zc0, zc1);
+    K.template pair<K_ZC0>(zc0, zc1);
     return fma(s * s, zc1, zc0);
   }
   R s2, cm2;
@@ -351,12 +416,12 @@ __device__ __forceinline__ R rr_separation2(double ur, bool &front, int &iters) 
   R dM;
   {
     R c4, c3, c2, ky, B, C, A, tol;
-    K::template pair<K_C4>(c4, c3);
-    K::template pair<K_C2>(c2, ky);
+    K.template pair<K_C4>(c4, c3);
+    K.template pair<K_C2>(c2, ky);
     const R y = (R)ur * ky;                            // dM / A
     R d = y * fma(y, fma(y, fma(y, c4, c3), c2), (R)1);
-    K::template pair<K_B>(B, C);
-    K::template pair<K_A>(A, tol);
+    K.template pair<K_B>(B, C);
+    K.template pair<K_A>(A, tol);
     // 2 pi ur: fp64 takes it from y (one FP64 instruction, no 64-bit constant); fp32 rounds the
     // fp64 product once (y A would add two fp32 roundings to the Kepler residual)
     dM = sizeof(R) == 8 ? y * A : (R)(RR_TWOPI * ur);
@@ -387,13 +452,13 @@ __device__ __forceinline__ R rr_separation2(double ur, bool &front, int &iters) 
   }
   if (!done) {
     R e, sE;
-    K::template pair<K_E>(e, sE);
-    iters += rr_kepler_robust<R>(e, sE, K::template get<K_CE>(), (R)(RR_TWOPI * ur), &s2, &cm2);
+    K.template pair<K_E>(e, sE);
+    iters += rr_kepler_robust<R>(e, sE, K.template get<K_CE>(), (R)(RR_TWOPI * ur), &s2, &cm2);
   }
   R X1, X2, Y1, Y2, Y0, aci2;
-  K::template pair<K_X1>(X1, X2);
-  K::template pair<K_Y1>(Y1, Y2);
-  K::template pair<K_Y0>(Y0, aci2);
+  K.template pair<K_X1>(X1, X2);
+  K.template pair<K_Y1>(Y1, Y2);
+  K.template pair<K_Y0>(Y0, aci2);
   const R xs = fma(X1, cm2, X2 * s2);
   const R ys = Y0 + fma(Y1, cm2, Y2 * s2);
   front = ys > (R)0;
@@ -413,21 +478,20 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
   ag = y - (float)ig;
 }
 
-template <typename R>
-__device__ __forceinline__ R rr_deficit(R z2, int &ningress) {
-  using K = Cst<R>;
+template <typename R, int M>
+__device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) {
   const R z = rr_sqrt3_pos(z2);
   int ig;
   R ag;
   R gscale, opk;
-  K::template pair<K_GSCALE>(gscale, opk);
+  K.template pair<K_GSCALE>(gscale, opk);
   rr_cell(z * gscale, ig, ag);
   R l0, sl;
-  K::cell(ig, l0, sl);                      // ldw[ig], ldw[ig+1] - ldw[ig]
+  K.cell(ig, l0, sl);                      // ldw[ig], ldw[ig+1] - ldw[ig]
   const R ip = fma(ag, sl, l0);             // mean occulted brightness
   R ap;
   R omk2, afull;
-  K::template pair<K_OMK2>(omk2, afull);
+  K.template pair<K_OMK2>(omk2, afull);
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
   } else {
@@ -440,7 +504,7 @@ __device__ __forceinline__ R rr_deficit(R z2, int &ningress) {
     // asin(k)/2 needs no octant reduction for k^2 <= 1/2 and th2/2 in [0, pi/2] needs one of three
     // cases.  ap = th1 + k^2 th2 - kite/2.
     R omks, k2;
-    K::template pair<K_OMKS>(omks, k2);
+    K.template pair<K_OMKS>(omks, k2);
     const R A = opk - z, B = z + omks, C = z - omks, D = z + opk;
     const R AB = fabs(A * B), S = fabs(C * D), Q = B * D;
     const R kite = rr_sqrt3_pos(AB * S);
@@ -448,7 +512,7 @@ __device__ __forceinline__ R rr_deficit(R z2, int &ningress) {
     if (k2 <= (R)0.5) h1 = rr_atan_t(rr_div3(kite, Q));
     else h1 = rr_atan_quadrant<R>(kite, Q, fabs(A * C));
     const R h2 = rr_atan_quadrant<R>(kite, S, AB);
-    const R tk2 = K::template get<K_2K2>();
+    const R tk2 = K.template get<K_2K2>();
     ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
     ++ningress;
   }
@@ -505,8 +569,8 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 
 // Occulted light of the sub-sample at phase w (turns, measured from the window centre).
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
-template <typename R, bool COUNT, bool CIRC, bool NOWRAP>
-__device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
+template <typename R, bool COUNT, bool CIRC, bool NOWRAP, int M>
+__device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_mid, double hwid,
                                           unsigned long long *cnt) {
   // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
   const double wr = NOWRAP ? w : w - rr_round(w);
@@ -514,9 +578,9 @@ __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
   if (fabs(wr) <= hwid) {
     bool front;
     int it = 0, ing = 0;
-    R z2 = rr_separation2<R, CIRC>(wr + u_mid, front, it);
-    if (front && z2 < Cst<R>::template get<K_OPK2>()) {
-      def = rr_deficit<R>(z2, ing);
+    R z2 = rr_separation2<R, CIRC, M>(K, wr + u_mid, front, it);
+    if (front && z2 < K.template get<K_OPK2>()) {
+      def = rr_deficit<R, M>(K, z2, ing);
       if (COUNT) { cnt[3]++; cnt[4] += ing; }
     }
     if (COUNT) { cnt[CIRC ? 1 : 2]++; cnt[5] += it; }
@@ -529,12 +593,11 @@ __device__ __forceinline__ R rr_subsample(double w, double u_mid, double hwid,
 // The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
 // R = arithmetic type of z and ip*ap; O = type of the sub-sample sum, the final 1 - sum/(Istar ns)
 // and the stored flux (O = double with R = float is RR_MIXED, the scheme of PAPER.md:293).
-template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP>
+template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__restrict__ out,
                                         int count, int ns, int shuffle, double t0, double inv_p,
                                         double u_mid, double hwid, double hw, O scale,
-                                        unsigned long long *cnt) {
-  using K = Cst<R>;
+                                        const Cst<R, M> K, unsigned long long *cnt) {
   const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
   const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
   const double hskip = hwid + hw;
@@ -570,14 +633,14 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
             cs = (R)c_;
           }
           R zc0, zc1, cd, sd;
-          K::template pair<K_ZC0>(zc0, zc1);
-          K::template pair<K_CD>(cd, sd);
-          const R opk2 = K::template get<K_OPK2>();
+          K.template pair<K_ZC0>(zc0, zc1);
+          K.template pair<K_CD>(cd, sd);
+          const R opk2 = K.template get<K_OPK2>();
           for (int s = 0; s < ns; ++s) {
             const R z2 = fma(sn * sn, zc1, zc0);
             if (cs > (R)0 && z2 < opk2) {
               int ing = 0;
-              acc += rr_deficit<R>(z2, ing);
+              acc += rr_deficit<R, M>(K, z2, ing);
               if (COUNT) { cnt[3]++; cnt[4] += ing; }
             }
             const R s1 = fma(sn, cd, cs * sd);
@@ -588,7 +651,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC, NOWRAP>(w, u_mid, hwid, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, cnt);
         }
         f = fma(-acc, scale, (O)1);                  // mean of (Istar - ip ap)/Istar over ns
       }
@@ -611,7 +674,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         if (fabs(wr) <= hskip) {
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
-            acc += rr_subsample<R, COUNT, CIRC, false>(fma(du, (double)s, w0), u_mid, hwid, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
         }
@@ -628,12 +691,12 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
 // flux = 1 with 16-byte stores, without touching the orbit.
 // Shared memory (rr_dyn): cst[K_SMEM] (constants, working precision) | ldw2[ldw_len] (node, slope)
 // pairs of the k-collapsed table row.
-template <typename R, typename O, bool COUNT>
+template <typename R, typename O, bool COUNT, int M>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
-  using K = Cst<R>;
-  using R2 = typename K::R2;
-  __shared__ unsigned tflags[FT / 32];
+  const Cst<R, M> K;
+  using R2 = typename Cst<R, M>::R2;
+  unsigned *tflags = Cst<R, M>::flags();
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
@@ -708,7 +771,7 @@ rr_flux_kernel(const FluxParams P) {
         const int kb = (P.nkpb == 1) ? 0 : lc.pb;
         const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
         const int64_t trow = (int64_t)v * P.npb + lc.pb;
-        R2 *ldw2 = K::row();
+        R2 *ldw2 = Cst<R, M>::row();
         __syncthreads();
         if (P.rows) {                                  // lazy mode: the row was collapsed for this k
           const R *rw = reinterpret_cast<const R *>(P.rows) + trow * (int64_t)P.ng;
@@ -734,22 +797,22 @@ rr_flux_kernel(const FluxParams P) {
         }
         rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns);
         if (threadIdx.x == K_SCALE)
-          K::base()[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
+          Cst<R, M>::base()[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
         __syncthreads();
-        scale = (O)K::template get<K_SCALE>();
+        scale = (O)K.template get<K_SCALE>();
         staged_lc = tlc;
       }
       const int shuffle = lc.ns >= P.shuffle_min_ns;
       const bool nowrap = hwid + 2.0 * hw < 0.499;
       if (circular)
-        rr_tile<R, O, COUNT, true, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                          inv_p, u_mid, hwid, hw, scale, cnt);
+        rr_tile<R, O, COUNT, true, false, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                          inv_p, u_mid, hwid, hw, scale, K, cnt);
       else if (nowrap)
-        rr_tile<R, O, COUNT, false, true>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                          inv_p, u_mid, hwid, hw, scale, cnt);
+        rr_tile<R, O, COUNT, false, true, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                          inv_p, u_mid, hwid, hw, scale, K, cnt);
       else
-        rr_tile<R, O, COUNT, false, false>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
-                                           inv_p, u_mid, hwid, hw, scale, cnt);
+        rr_tile<R, O, COUNT, false, false, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+                                           inv_p, u_mid, hwid, hw, scale, K, cnt);
     }
   }
   if (f0 >= 0) rr_fill<O>(row + f0, f1 - f0, (O)1);
@@ -773,6 +836,7 @@ __global__ void __launch_bounds__(FT)
 rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ tiles,
                 const RRLc *__restrict__ lcs, const RRPvOrbit *__restrict__ pvo, int64_t ntiles,
                 int64_t npv, int64_t nsub, double *__restrict__ zout) {
+  const Cst<R, RR_SM_SYMBOL> K;
   const int64_t total = ntiles * npv;
   for (int64_t w = blockIdx.x; w < total; w += gridDim.x) {
     const int64_t v = w / ntiles;
@@ -799,8 +863,8 @@ rr_orbit_kernel(const double *__restrict__ times, const RRTile *__restrict__ til
       double ur = us - rint(us);
       bool front;
       int it = 0;
-      R z2 = po.circular ? rr_separation2<R, true>(ur, front, it)
-                         : rr_separation2<R, false>(ur, front, it);
+      R z2 = po.circular ? rr_separation2<R, true, RR_SM_SYMBOL>(K, ur, front, it)
+                         : rr_separation2<R, false, RR_SM_SYMBOL>(K, ur, front, it);
       double z = (double)rr_sqrt(z2);
       out[j] = front ? z : -z;
     }
@@ -935,16 +999,19 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8);
+  const size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8) + 16;
   if (ctx->counters_on)
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
   using Kernel = void (*)(const FluxParams);
   const int pi = c.precision == RR_FP32 ? 1 : (c.precision == RR_MIXED ? 2 : 0);
-  static const Kernel kernels[3][2] = {
-      {rr_flux_kernel<double, double, false>, rr_flux_kernel<double, double, true>},
-      {rr_flux_kernel<float, float, false>, rr_flux_kernel<float, float, true>},
-      {rr_flux_kernel<float, double, false>, rr_flux_kernel<float, double, true>}};
-  const Kernel kern = kernels[pi][ctx->counters_on ? 1 : 0];
+#define RR_KROW(R, O, M) {rr_flux_kernel<R, O, false, M>, rr_flux_kernel<R, O, true, M>}
+  static const Kernel kernels[2][3][2] = {
+      {RR_KROW(double, double, RR_SM_FALLBACK_F64), RR_KROW(float, float, RR_SM_FALLBACK_F32),
+       RR_KROW(float, double, RR_SM_FALLBACK_F32)},
+      {RR_KROW(double, double, RR_SM_ABS), RR_KROW(float, float, RR_SM_ABS),
+       RR_KROW(float, double, RR_SM_ABS)}};
+#undef RR_KROW
+  const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : 0];
   if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory
     RR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, FT, smem, st>>>(P);
@@ -958,12 +1025,28 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
   if (fp32_math)
-    rr_orbit_kernel<float><<<grid, FT, K_SMEM * sizeof(float), st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
+    rr_orbit_kernel<float><<<grid, FT, K_SMEM * sizeof(float) + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
                                                 ctx->ntiles, npv, ctx->nsub, d_z);
   else
-    rr_orbit_kernel<double><<<grid, FT, K_SMEM * sizeof(double), st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
+    rr_orbit_kernel<double><<<grid, FT, K_SMEM * sizeof(double) + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
+// 1 if rr_dyn sits at shared::cta address RR_SMEM_ABS in a kernel without static shared memory
+// (what the RR_SM_ABS kernels assume), 0 if not; < 0: error.  Synchronous; called by rr_create.
+int rr_smem_probe(int *abs_ok) {
+  unsigned *d = nullptr, h = 0;
+  *abs_ok = 0;
+  RR_CUDA(cudaMalloc(&d, sizeof(unsigned)));
+  rr_smem_probe_kernel<<<1, 32, 256>>>(d);
+  cudaError_t e = cudaMemcpy(&h, d, sizeof(unsigned), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return RR_ECUDA_BASE - (int)e;
+#ifndef RR_NO_SMEM_ABS
+  *abs_ok = h == (unsigned)RR_SMEM_ABS;
+#endif
   return RR_OK;
 }
 
