@@ -337,7 +337,8 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
   double v = 0.0;
   switch (t) {
     case K_CD: v = cospi(2.0 * du); break;   case K_SD: v = sinpi(2.0 * du); break;
-    case K_ZC0: v = o.zc0; break;       case K_ZC1: v = o.zc1; break;
+    case K_ZC0: v = o.zc0 + (sizeof(R) == 8 ? RR_TINY_D : 1e-30); break;   // z^2 > 0
+    case K_ZC1: v = o.zc1; break;
     case K_E: v = o.e; break;           case K_SE: v = o.sE; break;
     case K_CE: v = o.cE; break;         case K_A: v = o.A; break;
     case K_B: v = o.B; break;           case K_C: v = o.C; break;
@@ -462,7 +463,8 @@ __device__ __forceinline__ R rr_separation2(const Cst<R, M> K, double ur, bool &
   const R xs = fma(X1, cm2, X2 * s2);
   const R ys = Y0 + fma(Y1, cm2, Y2 * s2);
   front = ys > (R)0;
-  return fma(xs, xs, aci2 * (ys * ys));
+  const R tiny = sizeof(R) == 8 ? (R)RR_TINY_D : (R)1e-30f;       // z^2 > 0: the sqrt seed stays finite
+  return fma(xs, xs, fma(aci2 * ys, ys, tiny));
 }
 
 // ---- kernel 3 core: occulted light ip * ap of one sub-sample with z < 1+k ------
@@ -480,7 +482,7 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
 
 template <typename R, int M>
 __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) {
-  const R z = rr_sqrt3_pos(z2);
+  const R z = rr_sqrt3(z2);                 // z2 > 0: both orbit branches add 2^-1000
   int ig;
   R ag;
   R gscale, opk;
@@ -514,6 +516,9 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) 
     const R h2 = rr_atan_quadrant<R>(kite, S, AB);
     const R tk2 = K.template get<K_2K2>();
     ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
+    // fp32: the three terms cancel at the first contact; keep ap >= 0 so that flux <= 1 (RR_MIXED
+    // stores the sum in fp64, where a deficit of -1e-13 would show)
+    if constexpr (sizeof(R) == 4) ap = fmaxf(ap, 0.0f);
     ++ningress;
   }
   return ip * ap;
@@ -603,10 +608,21 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double hskip = hwid + hw;
   if (!shuffle) {
     // ---- one thread per exposure, in-thread loop over its sub-samples ----
-    double tnext = ((int)threadIdx.x < count) ? times[threadIdx.x] : 0.0;
-    for (int i = threadIdx.x; i < count; i += FT) {
+    // The time and flux pointers advance by opaque 64-bit adds: otherwise the compiler, short of
+    // registers, rebuilds both addresses from the kernel parameters at every exposure (15
+    // instructions).
+    uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
+    uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
+    int left = count - (int)threadIdx.x;             // exposures of this thread still to do, x FT
+    double tnext = left > 0 ? *reinterpret_cast<const double *>(tp) : 0.0;
+    // circular: the in-front test is only needed when the evaluated phases can reach a quarter turn
+    // (lane-0 broadcast: opaque, or the compiler recomputes the fp64 test in the inner loop)
+    const bool need_front = __shfl_sync(0xffffffffu, (int)!(hskip + hw < 0.25), 0) != 0;
+    while (left > 0) {
       const double tcur = tnext;
-      if (i + FT < count) tnext = times[i + FT];     // in flight while this exposure is evaluated
+      left -= FT;
+      asm volatile("add.u64 %0, %0, %1;" : "+l"(tp) : "n"(FT * 8));
+      if (left > 0) tnext = *reinterpret_cast<const double *>(tp);   // in flight during this exposure
       const double wc = fma(tcur - t0, inv_p, -u_mid);
       const double wr = wc - rr_round(wc);           // exposure centre from the window centre
       O f;
@@ -637,15 +653,18 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
           K.template pair<K_CD>(cd, sd);
           const R opk2 = K.template get<K_OPK2>();
           for (int s = 0; s < ns; ++s) {
-            const R z2 = fma(sn * sn, zc1, zc0);
-            if (cs > (R)0 && z2 < opk2) {
+            const R z2 = fma(sn * sn, zc1, zc0);     // zc0 carries +2^-1000: z2 > 0
+            bool occ = z2 < opk2;
+            if (need_front) occ = occ && cs > (R)0;
+            // the next sub-sample's rotation first: independent work under the deficit's latency
+            const R s1 = fma(sn, cd, cs * sd);
+            cs = fma(cs, cd, -sn * sd);
+            sn = s1;
+            if (occ) {
               int ing = 0;
               acc += rr_deficit<R, M>(K, z2, ing);
               if (COUNT) { cnt[3]++; cnt[4] += ing; }
             }
-            const R s1 = fma(sn, cd, cs * sd);
-            cs = fma(cs, cd, -sn * sd);
-            sn = s1;
           }
           if (COUNT) cnt[1] += ns;
         } else {
@@ -653,9 +672,11 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
           for (int s = 0; s < ns; ++s, w += du)
             acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, cnt);
         }
-        f = fma(-acc, scale, (O)1);                  // mean of (Istar - ip ap)/Istar over ns
+        // mean of (Istar - ip ap)/Istar over ns; fp64 staged the table already times 1/(Istar ns)
+        f = sizeof(R) == 8 ? (O)1 - acc : fma(-acc, scale, (O)1);
       }
-      RR_STORE(out + i, f);
+      RR_STORE(reinterpret_cast<O *>(op), f);
+      asm volatile("add.u64 %0, %0, %1;" : "+l"(op) : "n"(FT * (int)sizeof(O)));
     }
   } else {
     // ---- sub-samples across lanes, warp-shuffle sum ----
@@ -680,7 +701,8 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         }
       }
       for (int o = G >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if (live && sl == 0) out[i] = (wr == wr) ? fma(-acc, scale, (O)1) : rr_nan<O>();
+      if (live && sl == 0)
+        out[i] = (wr == wr) ? (sizeof(R) == 8 ? (O)1 - acc : fma(-acc, scale, (O)1)) : rr_nan<O>();
     }
   }
 }
@@ -758,7 +780,11 @@ rr_flux_kernel(const FluxParams P) {
         f0 = -1;
       }
       const RRTile *tp = P.tiles + base + q;
-      const int tstart = tp->start, tcount = tp->count, tlc = tp->lc;
+      // warp-uniform by construction; the lane-0 broadcast lets ptxas keep them (and the tile's base
+      // pointers) in uniform registers
+      const int tstart = __shfl_sync(0xffffffffu, tp->start, 0);
+      const int tcount = __shfl_sync(0xffffffffu, tp->count, 0);
+      const int tlc = __shfl_sync(0xffffffffu, tp->lc, 0);
       if (tlc != desc_lc) {
         lc = P.lcs[tlc];
         desc_lc = tlc;
@@ -772,14 +798,18 @@ rr_flux_kernel(const FluxParams P) {
         const RRPvBand &pb = P.pvb[(int64_t)v * P.nkpb + kb];
         const int64_t trow = (int64_t)v * P.npb + lc.pb;
         R2 *ldw2 = Cst<R, M>::row();
+        // fp64: the cells carry the factor 1/(Istar ns), so that flux = 1 - sum(ip ap) needs no
+        // final scaling; fp32 keeps it apart (one rounding less on the occulted light)
+        const double sc_d = 1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns);
+        const R sc = sizeof(R) == 8 ? (R)sc_d : (R)1;
         __syncthreads();
         if (P.rows) {                                  // lazy mode: the row was collapsed for this k
           const R *rw = reinterpret_cast<const R *>(P.rows) + trow * (int64_t)P.ng;
           for (int ig = threadIdx.x; ig < P.ldw_len; ig += FT) {
             const R a = rw[min(ig, P.ng - 1)], b = rw[min(ig + 1, P.ng - 1)];
             R2 c;
-            c.x = a;
-            c.y = b - a;
+            c.x = a * sc;
+            c.y = (b - a) * sc;
             ldw2[ig] = c;
           }
         } else {
@@ -790,14 +820,13 @@ rr_flux_kernel(const FluxParams P) {
             const int jg = min(ig, P.ng - 1), jh = min(ig + 1, P.ng - 1);   // cells >= ng-1: flat
             const R a = fma(ak, T1[jg] - T0[jg], T0[jg]), b = fma(ak, T1[jh] - T0[jh], T0[jh]);
             R2 c;
-            c.x = a;
-            c.y = b - a;
+            c.x = a * sc;
+            c.y = (b - a) * sc;
             ldw2[ig] = c;
           }
         }
         rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns);
-        if (threadIdx.x == K_SCALE)
-          Cst<R, M>::base()[K_SCALE] = (R)(1.0 / ((double)reinterpret_cast<const R *>(P.istar)[trow] * lc.ns));
+        if (threadIdx.x == K_SCALE) Cst<R, M>::base()[K_SCALE] = (R)sc_d;
         __syncthreads();
         scale = (O)K.template get<K_SCALE>();
         staged_lc = tlc;
