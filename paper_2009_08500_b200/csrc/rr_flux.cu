@@ -510,12 +510,18 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) 
     const R A = opk - z, B = z + omks, C = z - omks, D = z + opk;
     const R AB = fabs(A * B), S = fabs(C * D), Q = B * D;
     const R kite = rr_sqrt3_pos(AB * S);
-    R h1;
-    if (k2 <= (R)0.5) h1 = rr_atan_t(rr_div3(kite, Q));
-    else h1 = rr_atan_quadrant<R>(kite, Q, fabs(A * C));
-    const R h2 = rr_atan_quadrant<R>(kite, S, AB);
     const R tk2 = K.template get<K_2K2>();
-    ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
+    // (the k^2 > 1/2 case is a path of its own so that the common one is a single basic block:
+    // the two arctangents are independent and interleave)
+    if (k2 <= (R)0.5) {
+      const R h1 = rr_atan_t(rr_div3(kite, Q));
+      const R h2 = rr_atan_quadrant<R>(kite, S, AB);
+      ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
+    } else {
+      const R h1 = rr_atan_quadrant<R>(kite, Q, fabs(A * C));
+      const R h2 = rr_atan_quadrant<R>(kite, S, AB);
+      ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
+    }
     // fp32: the three terms cancel at the first contact; keep ap >= 0 so that flux <= 1 (RR_MIXED
     // stores the sum in fp64, where a deficit of -1e-13 would show)
     if constexpr (sizeof(R) == 4) ap = fmaxf(ap, 0.0f);
