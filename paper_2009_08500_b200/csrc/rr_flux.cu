@@ -582,7 +582,7 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
 template <typename R, bool COUNT, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_mid, double hwid,
-                                          unsigned long long *cnt) {
+                                          bool need_front, unsigned long long *cnt) {
   // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
   const double wr = NOWRAP ? w : w - rr_round(w);
   R def = (R)0;
@@ -590,7 +590,11 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
     bool front;
     int it = 0, ing = 0;
     R z2 = rr_separation2<R, CIRC, M>(K, wr + u_mid, front, it);
-    if (front && z2 < K.template get<K_OPK2>()) {
+    // inside a transit window (hwid < 1/2) the true anomaly is within a quarter turn of
+    // conjunction: the planet is in front, and the test is only needed without a window
+    bool occ = z2 < K.template get<K_OPK2>();
+    if (need_front) occ = occ && front;
+    if (occ) {
       def = rr_deficit<R, M>(K, z2, ing);
       if (COUNT) { cnt[3]++; cnt[4] += ing; }
     }
@@ -623,7 +627,8 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
     double tnext = left > 0 ? *reinterpret_cast<const double *>(tp) : 0.0;
     // circular: the in-front test is only needed when the evaluated phases can reach a quarter turn
     // (lane-0 broadcast: opaque, or the compiler recomputes the fp64 test in the inner loop)
-    const bool need_front = __shfl_sync(0xffffffffu, (int)!(hskip + hw < 0.25), 0) != 0;
+    const bool need_front =
+        __shfl_sync(0xffffffffu, (int)(CIRC ? !(hskip + hw < 0.25) : !(hwid < 0.49)), 0) != 0;
     while (left > 0) {
       const double tcur = tnext;
       left -= FT;
@@ -676,7 +681,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, need_front, cnt);
         }
         // mean of (Istar - ip ap)/Istar over ns; fp64 staged the table already times 1/(Istar ns)
         f = sizeof(R) == 8 ? (O)1 - acc : fma(-acc, scale, (O)1);
@@ -701,7 +706,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         if (fabs(wr) <= hskip) {
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
-            acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, true, cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
         }
