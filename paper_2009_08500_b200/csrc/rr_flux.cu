@@ -482,18 +482,18 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
 
 template <typename R, int M>
 __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) {
+  // the constants first: their shared-memory latency passes under the square root
+  R gscale, opk, omk2, afull;
+  K.template pair<K_GSCALE>(gscale, opk);
+  K.template pair<K_OMK2>(omk2, afull);
   const R z = rr_sqrt3(z2);                 // z2 > 0: both orbit branches add 2^-1000
   int ig;
   R ag;
-  R gscale, opk;
-  K.template pair<K_GSCALE>(gscale, opk);
   rr_cell(z * gscale, ig, ag);
   R l0, sl;
   K.cell(ig, l0, sl);                      // ldw[ig], ldw[ig+1] - ldw[ig]
   const R ip = fma(ag, sl, l0);             // mean occulted brightness
   R ap;
-  R omk2, afull;
-  K.template pair<K_OMK2>(omk2, afull);
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
   } else {
