@@ -155,7 +155,8 @@ int rr_build_ld_table(rr_ctx *ctx, const void *d_ldp, const void *d_istar, int64
  * takes Istar = 2 pi int_0^1 mu I dmu in closed form ("integrated analytically", PAPER.md:156;
  * RR_LD_EXPONENTIAL has none: reading R6), and then behaves as rr_build_ld_table in the current
  * table mode.  The paper names the laws without printing them: the forms above are the textbook
- * ones of its footnote 4.  RR_ESIZE if nldc does not fit the law.  Synchronous on `stream`.      */
+ * ones of its footnote 4.  RR_ESIZE if nldc does not fit the law.  Asynchronous on `stream`
+ * (buffers grow only when a larger npv arrives).                                                 */
 int rr_build_ld_table_law(rr_ctx *ctx, int32_t law, const double *d_ldc, int32_t nldc, int64_t npv,
                           void *stream);
 /* RR_TABLE_*; takes effect at the next rr_build_ld_table.  RR_TABLE_DIRECT needs nz <= 2000.     */
@@ -216,7 +217,7 @@ int64_t rr_num_tiles(const rr_ctx *ctx);        /* dispatch tiles of the current
 int rr_get_tiles(const rr_ctx *ctx, int32_t *h_start, int32_t *h_count, int32_t *h_lc,
                  double *h_tmin, double *h_tmax);
 
-/* Supersample reduction layout (RR_REDUCE_*); takes effect at the next rr_set_data.             */
+/* Supersample reduction layout (RR_REDUCE_*); read at every rr_evaluate.                        */
 int rr_set_reduction(rr_ctx *ctx, int32_t mode);
 
 /* ---- whole step with HOST buffers (the end-to-end call) --------------------------------------------

@@ -70,6 +70,9 @@ def load():
     lib.oracle_direct_rows.restype = None
     lib.oracle_direct_rows_sp.argtypes = [_D, _D, C.c_int, C.c_int, _D, _D, C.c_int64, C.c_double, _D]
     lib.oracle_direct_rows_sp.restype = None
+    lib.oracle_direct_rows_pv.argtypes = [_D, _D, C.c_int, C.c_int, _D, C.c_int32, C.c_int32,
+                                          C.c_int64, C.c_int32, _D, C.c_double, _D]
+    lib.oracle_direct_rows_pv.restype = None
     lib.oracle_profile_at.argtypes = [C.c_double, _D, _D, C.c_int]
     lib.oracle_profile_at.restype = C.c_double
     lib.oracle_flux_from_row.argtypes = [C.c_double, C.c_double, _D, C.c_int, C.c_double]
@@ -215,18 +218,15 @@ class OracleDirectModel:
 
     def rows(self, ldp, pv, mean_k_weights=False, small_planet_k=0.0):
         """ldw[npv][npb][ng] and Istar[npv][npb] for the k of every (pv, passband); with
-        mean_k_weights the weights of every passband are taken at the pv's mean k (PAPER.md:188-190;
-        the selection of which k to pass is the only thing done here)."""
+        mean_k_weights the weights of every passband are taken at the pv's mean k.
+        Rows of pvs with an invalid k are NaN (oracle_direct_rows_pv)."""
         ldp = _f64(ldp).reshape(-1, self.npb, self.nz)
         pv = _f64(pv).reshape(-1, self.nkpb + 6)
         npv = ldp.shape[0]
-        kcol = [0] * self.npb if self.nkpb == 1 else list(range(self.npb))
-        k = _f64(pv[:, kcol])                                   # [npv][npb]
-        if mean_k_weights:
-            k = _f64(np.repeat(pv[:, :self.nkpb].mean(axis=1)[:, None], self.npb, axis=1))
         out = np.empty((npv, self.npb, self.ng))
-        load().oracle_direct_rows_sp(_dp(self.ze), _dp(self.zm), self.nz, self.ng, _dp(k), _dp(ldp),
-                                     npv * self.npb, float(small_planet_k), _dp(out))
+        load().oracle_direct_rows_pv(_dp(self.ze), _dp(self.zm), self.nz, self.ng, _dp(pv),
+                                     self.nkpb, self.npb, npv, int(bool(mean_k_weights)), _dp(ldp),
+                                     float(small_planet_k), _dp(out))
         return out, istar(self.ze, ldp)
 
     def evaluate(self, times, lc_index, passband_index, supersampling, exposure_time, pv, ldp,
@@ -234,10 +234,7 @@ class OracleDirectModel:
         times, pv = _f64(times), _f64(pv).reshape(-1, self.nkpb + 6)
         lc_index, passband_index = _i32(lc_index), _i32(passband_index)
         supersampling, exposure_time = _i32(supersampling), _f64(exposure_time)
-        ok = np.all(np.isfinite(pv[:, :self.nkpb]) & (pv[:, :self.nkpb] > 0), axis=1)
-        safe = pv.copy()
-        safe[~ok, :self.nkpb] = 0.1                              # rows of invalid pvs are not used
-        rows, ist = self.rows(ldp, safe, mean_k_weights, small_planet_k)
+        rows, ist = self.rows(ldp, pv, mean_k_weights, small_planet_k)
         npv, npt = pv.shape[0], times.size
         flux = np.empty((npv, npt))
         status = np.empty(npv, np.int32)

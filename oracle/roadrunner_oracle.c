@@ -460,3 +460,34 @@ void oracle_direct_rows_sp(const double *ze, const double *zm, int nz, int ng, c
         }
     }
 }
+
+/* Direct-model rows[npv][npb][ng] straight from the parameter vectors: the weight radius of row
+ * (pv, pb) is the pv's k for that passband, or, with mean_k_weights, the mean of the pv's radius
+ * ratios (reading R13).  Rows of pvs whose k is not finite and > 0 (reading R12:
+ * NaN flux rows, never read by oracle_evaluate_direct) are filled with NaN. */
+void oracle_direct_rows_pv(const double *ze, const double *zm, int nz, int ng, const double *pv,
+                           int32_t nkpb, int32_t npb, int64_t npv, int32_t mean_k_weights,
+                           const double *ldp /*[npv][npb][nz]*/, double k_small,
+                           double *rows /*[npv][npb][ng]*/)
+{
+    for (int64_t v = 0; v < npv; ++v) {
+        const double *row = pv + v * (nkpb + 6);
+        int ok = 1;
+        double kmean = 0.0;
+        for (int q = 0; q < nkpb; ++q) {
+            if (!isfinite(row[q]) || !(row[q] > 0.0)) ok = 0;
+            kmean += row[q];
+        }
+        kmean /= (double)nkpb;
+        for (int pb = 0; pb < npb; ++pb) {
+            int64_t r = v * npb + pb;
+            if (!ok) {
+                for (int ig = 0; ig < ng; ++ig) rows[r * ng + ig] = NAN;
+                continue;
+            }
+            double k = mean_k_weights ? kmean : row[nkpb == 1 ? 0 : pb];
+            oracle_direct_rows_sp(ze, zm, nz, ng, &k, ldp + r * nz, 1, k_small, rows + r * ng);
+        }
+    }
+}
+

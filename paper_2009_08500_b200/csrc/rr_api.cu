@@ -188,7 +188,7 @@ int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, i
     lcs[l].ns = h_supersampling[l];
     lcs[l].pb = h_passband_index[l];
     lcs[l].tile_len = tile_len_for(h_supersampling[l]);
-    lcs[l].shuffle = 0;
+    lcs[l].pad = 0;
   }
   cudaStream_t st = (cudaStream_t)stream;
   free_data(ctx);
@@ -262,6 +262,9 @@ int rr_set_table_mode(rr_ctx *ctx, int32_t mode) {
 
 const void *rr_table_ptr(rr_ctx *ctx) {
   if (!ctx || ctx->work[0].table_npv <= 0) return nullptr;
+  // the profile copy of rr_build_ld_table was queued on the caller's stream, which the legacy
+  // stream used below does not order with
+  if (cudaDeviceSynchronize() != cudaSuccess) return nullptr;
   if (rr_ld_full_from_profile(ctx, &ctx->work[0], nullptr) != RR_OK) return nullptr;
   if (cudaDeviceSynchronize() != cudaSuccess) return nullptr;
   return ctx->work[0].T;
@@ -305,22 +308,31 @@ int rr_evaluate(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, void
   if (ctx->ntiles < 0 || ctx->work[0].table_npv != npv) return RR_ESTATE;
   if (ctx->k_small > 0.0 && !ctx->work[0].lazy) return RR_ESTATE;   // needs the row builders
   cudaStream_t st = (cudaStream_t)stream;
-  int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, d_status, st);
+  int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, d_status,
+                             ctx->cfg.precision != RR_FP64, st);
   if (rc != RR_OK) return rc;
+  // Kernel timing: a triple of events (before rows, before flux, after flux) joins ctx->tev only
+  // when all three were recorded; any failure destroys them here.
   cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
-  const bool timed = ctx->timing_on && ctx->tev.size() < 3 * 4096;
-  if (timed) {
-    for (auto &e : ev) RR_CUDA(cudaEventCreate(&e));
+  bool timed = ctx->timing_on && ctx->tev.size() < 3 * 4096;
+  if (timed)
+    for (auto &e : ev)
+      if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; timed = false; }
+  cudaError_t ce = cudaSuccess;
+  if (timed) ce = cudaEventRecord(ev[0], st);
+  if (ce == cudaSuccess && ctx->work[0].lazy) rc = rr_ld_rows_launch(ctx, &ctx->work[0], npv, st);
+  if (ce == cudaSuccess && rc == RR_OK && ctx->work[0].lazy && ctx->k_small > 0.0)
+    rc = rr_ld_rows_small_launch(ctx, &ctx->work[0], npv, st);
+  if (ce == cudaSuccess && rc == RR_OK && timed) ce = cudaEventRecord(ev[1], st);
+  if (ce == cudaSuccess && rc == RR_OK) rc = rr_flux_launch(ctx, &ctx->work[0], npv, d_flux, st);
+  if (ce == cudaSuccess && rc == RR_OK && timed) ce = cudaEventRecord(ev[2], st);
+  if (ce != cudaSuccess && rc == RR_OK) rc = RR_ECUDA_BASE - (int)ce;
+  if (timed && rc == RR_OK) {
     for (auto e : ev) ctx->tev.push_back(e);
-    RR_CUDA(cudaEventRecord(ev[0], st));
+  } else {
+    for (auto e : ev)
+      if (e) cudaEventDestroy(e);
   }
-  if (ctx->work[0].lazy && (rc = rr_ld_rows_launch(ctx, &ctx->work[0], npv, st)) != RR_OK) return rc;
-  if (ctx->work[0].lazy && ctx->k_small > 0.0 &&
-      (rc = rr_ld_rows_small_launch(ctx, &ctx->work[0], npv, st)) != RR_OK)
-    return rc;
-  if (timed) RR_CUDA(cudaEventRecord(ev[1], st));
-  rc = rr_flux_launch(ctx, &ctx->work[0], npv, d_flux, st);
-  if (timed) RR_CUDA(cudaEventRecord(ev[2], st));
   return rc;
 }
 
@@ -340,7 +352,7 @@ int rr_orbit_z(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, doubl
   if (npv <= 0 || npar != ctx->cfg.nkpb + 6) return RR_ESIZE;
   if (ctx->ntiles < 0) return RR_ESTATE;
   cudaStream_t st = (cudaStream_t)stream;
-  int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, nullptr, st);
+  int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, nullptr, fp32_math != 0, st);
   if (rc != RR_OK) return rc;
   return rr_orbit_launch(ctx, &ctx->work[0], npv, d_z, fp32_math, st);
 }
@@ -400,25 +412,30 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
     double *d_pv = (double *)ctx->d_host_stage[s][1];
     void *d_flux = ctx->d_host_stage[s][2];
     int32_t *d_status = (int32_t *)ctx->d_host_stage[s][3];
-    RR_CUDA(cudaMemcpyAsync(d_ldp, (const char *)h_ldp + v0 * ldp_row, nv * ldp_row,
-                            cudaMemcpyHostToDevice, st));
-    RR_CUDA(cudaMemcpyAsync(d_pv, (const char *)h_pv + v0 * pv_row, nv * pv_row,
-                            cudaMemcpyHostToDevice, st));
+    // (no early return from here on: copies and kernels of the other slot may still be in flight
+    // against the caller's host buffers, and the epilogue below waits for both streams)
+    cudaError_t ce = cudaMemcpyAsync(d_ldp, (const char *)h_ldp + v0 * ldp_row, nv * ldp_row,
+                                     cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess)
+      ce = cudaMemcpyAsync(d_pv, (const char *)h_pv + v0 * pv_row, nv * pv_row,
+                           cudaMemcpyHostToDevice, st);
+    if (ce != cudaSuccess) { rc = RR_ECUDA_BASE - (int)ce; break; }
     RRWork *wk = &ctx->work[1 + s];
     if (lazy_ok(ctx)) {   // the staging buffer lives until this chunk's kernels are done
       if ((rc = rr_ld_profile_launch(ctx, wk, d_ldp, nullptr, nv, 0, st)) != RR_OK) break;
     } else if ((rc = rr_ld_table_launch(ctx, wk, d_ldp, nullptr, nv, st)) != RR_OK) {
       break;
     }
-    if ((rc = rr_pv_prep_launch(ctx, wk, d_pv, nv, d_status, st)) != RR_OK) break;
+    if ((rc = rr_pv_prep_launch(ctx, wk, d_pv, nv, d_status, ctx->cfg.precision != RR_FP64, st)) != RR_OK) break;
     if (wk->lazy && (rc = rr_ld_rows_launch(ctx, wk, nv, st)) != RR_OK) break;
     if (wk->lazy && ctx->k_small > 0.0 && (rc = rr_ld_rows_small_launch(ctx, wk, nv, st)) != RR_OK)
       break;
     if ((rc = rr_flux_launch(ctx, wk, nv, d_flux, st)) != RR_OK) break;
-    RR_CUDA(cudaMemcpyAsync((char *)h_flux + v0 * flux_row, d_flux, nv * flux_row,
-                            cudaMemcpyDeviceToHost, st));
-    if (h_status)
-      RR_CUDA(cudaMemcpyAsync(h_status + v0, d_status, nv * 4, cudaMemcpyDeviceToHost, st));
+    ce = cudaMemcpyAsync((char *)h_flux + v0 * flux_row, d_flux, nv * flux_row,
+                         cudaMemcpyDeviceToHost, st);
+    if (ce == cudaSuccess && h_status)
+      ce = cudaMemcpyAsync(h_status + v0, d_status, nv * 4, cudaMemcpyDeviceToHost, st);
+    if (ce != cudaSuccess) { rc = RR_ECUDA_BASE - (int)ce; break; }
   }
   for (int s = 0; s < 2; ++s) {
     cudaError_t e = cudaStreamSynchronize(ctx->hs[s]);

@@ -18,7 +18,7 @@ struct RRLc {
   int32_t ns;        // sub-samples per exposure
   int32_t pb;        // passband
   int32_t tile_len;  // exposures per dispatch tile
-  int32_t shuffle;   // 1: sub-samples across lanes (warp-shuffle reduction)
+  int32_t pad;
 };
 
 // One dispatch tile (kernel 4 output): a run of exposures of ONE light curve.
@@ -109,7 +109,6 @@ struct rr_ctx {
   int64_t *d_scratch;   // dispatch scratch
   int64_t scratch_cap;
   int32_t reduction;
-  int32_t any_shuffle;
   int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL | RR_TABLE_DIRECT
   int32_t mean_k;       // 1: LD weights at the mean k of the passbands
   double k_small;       // small-planet approximation for kw <= k_small; 0: off
@@ -158,7 +157,7 @@ int rr_ld_rows_direct_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t 
 int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st);   // rr_geometry.cu
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st);                           // rr_dispatch.cu
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
-                      int32_t *d_status, cudaStream_t st);                     // rr_flux.cu
+                      int32_t *d_status, int fp32_tol, cudaStream_t st);       // rr_flux.cu
 int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStream_t st);
 int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_math,
                     cudaStream_t st);

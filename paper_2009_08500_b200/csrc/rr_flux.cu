@@ -960,16 +960,19 @@ int fma_peak_typed(double *h_fma_per_s, cudaStream_t st) {
 
 // Extra nodes of the staged table row beyond ng - 1 (all equal to the limb node): 1 normally; with
 // mean-k weights and chromatic k, g = z/(1+kw) of a passband with k > kw runs up to (1+k)/(1+kw).
-static int rr_row_pad(const rr_ctx *ctx) {
+// The mode is that of the table actually built (wk->lazy), not the one set for the next build.
+static int rr_row_pad(const rr_ctx *ctx, const RRWork *wk) {
   const rr_config &c = ctx->cfg;
   if (!(ctx->mean_k && c.nkpb > 1)) return 1;
-  if (ctx->table_mode == RR_TABLE_DIRECT) return c.ng + 2;    // no k limits: up to k = 1 + 2 kw
+  if (wk->lazy == 2) return c.ng + 2;    // direct model, no k limits: up to k = 1 + 2 kw
   return (int)ceil((c.ng - 1) * (c.k1 - c.k0) / (1.0 + c.k0)) + 3;
 }
 
 // ---- host launchers -------------------------------------------------------------------------------
+// fp32_tol: Halley acceptance tolerance of the fp32 arithmetic (the RR_FP32 / RR_MIXED flux kernels
+// and rr_orbit_z(fp32_math = 1)); the fp64 orbit kernel needs the fp64 one on any ctx.
 int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
-                      int32_t *d_status, cudaStream_t st) {
+                      int32_t *d_status, int fp32_tol, cudaStream_t st) {
   const rr_config &c = ctx->cfg;
   if (npv > wk->pv_cap) {
     if (wk->pvo) cudaFree(wk->pvo);
@@ -988,7 +991,7 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
   const bool direct = wk->lazy == 2;
   rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
       d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, direct ? 1e-300 : c.k0, direct ? 1e300 : c.k1, c.ng,
-      c.precision != RR_FP64, ctx->mean_k, rr_row_pad(ctx), wk->pvo, wk->pvb, d_status);
+      fp32_tol, ctx->mean_k, rr_row_pad(ctx, wk), wk->pvo, wk->pvb, d_status);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
@@ -1022,7 +1025,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   // shuffle; lanes-over-sub-samples multiplies the parallelism by ns, which only pays when
   // npv x npt alone cannot fill the GPU.
   const int64_t resident = (int64_t)ctx->sm_count * 2048;
-  P.ldw_len = c.ng + rr_row_pad(ctx);
+  P.ldw_len = c.ng + rr_row_pad(ctx, wk);
   if (ctx->reduction == RR_REDUCE_THREAD) P.shuffle_min_ns = 0x7fffffff;
   else if (ctx->reduction == RR_REDUCE_SHUFFLE) P.shuffle_min_ns = 2;
   else P.shuffle_min_ns = (npv * ctx->npt < 2 * resident) ? 4 : 0x7fffffff;

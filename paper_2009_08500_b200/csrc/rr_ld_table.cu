@@ -159,7 +159,8 @@ __device__ double rr_law_value(int law, const double *c, int nc, double mu) {
   }
 }
 
-// Istar / pi in closed form; < 0: none (the caller falls back to the discretised integral, R6).
+// Istar / pi in closed form (every law but RR_LD_EXPONENTIAL, for which the host launcher asks for
+// the discretised integral of reading R6 instead and this function is not called).
 __device__ double rr_law_istar_over_pi(int law, const double *c, int nc) {
   switch (law) {
     case RR_LD_UNIFORM: return 1.0;
@@ -189,18 +190,14 @@ __device__ double rr_law_istar_over_pi(int law, const double *c, int nc) {
 template <typename TR>
 __global__ void rr_ld_law_kernel(int law, const double *__restrict__ ldc, int nc,
                                  const double *__restrict__ mu, int64_t M, int nz,
-                                 TR *__restrict__ ldp, TR *__restrict__ istar, int *no_closed_form) {
+                                 TR *__restrict__ ldp, TR *__restrict__ istar_or_null) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= M * nz) return;
   const int64_t row = idx / nz;
   const int j = (int)(idx - row * nz);
   const double *c = ldc + row * nc;
   ldp[idx] = (TR)rr_law_value(law, c, nc, mu[j]);
-  if (j == 0) {
-    const double s = rr_law_istar_over_pi(law, c, nc);
-    if (s >= 0.0) istar[row] = (TR)(RR_PI * s);
-    else if (row == 0) *no_closed_form = 1;
-  }
+  if (j == 0 && istar_or_null) istar_or_null[row] = (TR)(RR_PI * rr_law_istar_over_pi(law, c, nc));
 }
 
 // Lazy mode: the k-collapsed row of one (pv, passband),
@@ -366,6 +363,7 @@ int launch_typed(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void *d_istar
   rr_ld_table_kernel<TR, TR><<<grid, NT, 0, st>>>((const TR *)d_ldp, ctx->d_W, (TR *)wk->T, M,
                                                   N, K);
   RR_LAUNCH_CHECK(ctx);
+  if (d_istar == wk->istar) return RR_OK;          // already in place (named law, closed form)
   int64_t threads = M * 32;
   rr_istar_kernel<TR, TR><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
       (const TR *)d_ldp, ctx->d_q, (const TR *)d_istar, (TR *)wk->istar, M, K);
@@ -434,13 +432,17 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
     wk->ldp_src = d_ldp;
   }
   const int64_t threads = M * 32;
-  if (c.precision != RR_FP64)
+  if (d_istar == wk->istar) {
+    // already in place (named law with a closed form)
+  } else if (c.precision != RR_FP64) {
     rr_istar_kernel<float, float><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const float *)d_ldp, ctx->d_q, (const float *)d_istar, (float *)wk->istar, M, ctx->nz);
-  else
+    RR_LAUNCH_CHECK(ctx);
+  } else {
     rr_istar_kernel<double, double><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
         (const double *)d_ldp, ctx->d_q, (const double *)d_istar, (double *)wk->istar, M, ctx->nz);
-  RR_LAUNCH_CHECK(ctx);
+    RR_LAUNCH_CHECK(ctx);
+  }
   wk->table_npv = npv;
   wk->lazy = ctx->table_mode == RR_TABLE_DIRECT ? 2 : 1;
   wk->have_full = 0;
@@ -531,39 +533,36 @@ int rr_ld_full_from_profile(rr_ctx *ctx, RRWork *wk, cudaStream_t st) {
 
 
 // Named law -> profile (into the ctx-owned copy) + analytic Istar, then as rr_build_ld_table.
+// Asynchronous on st: whether the law has a closed-form disc integral is known on the host from the
+// law alone (only RR_LD_EXPONENTIAL has none: reading R6 then), and the kernel writes Istar straight
+// into the ctx-owned buffer; buffers grow (cudaMalloc) only when a larger npv arrives.
 int rr_ld_law_launch(rr_ctx *ctx, RRWork *wk, int law, const double *d_ldc, int nc, int64_t npv,
                      cudaStream_t st) {
   const rr_config &c = ctx->cfg;
   const int64_t esz = c.precision != RR_FP64 ? 4 : 8;
   const int64_t M = npv * c.npb;
+  const bool full = !(ctx->table_mode != RR_TABLE_FULL && ctx->nz <= 2000);
   wk->table_npv = -1;
   int rc = grow_buf(&wk->ldp, &wk->ldp_cap, M * ctx->nz * esz);
   if (rc == RR_OK) rc = grow_buf(&wk->istar, &wk->istar_cap, M * esz);
-  void *given = nullptr;                           // analytic Istar, handed on as the override
-  int64_t given_cap = 0;
-  if (rc == RR_OK) rc = grow_buf(&given, &given_cap, M * esz + 16);
   if (rc != RR_OK) return rc;
-  int *flag = (int *)((char *)given + M * esz);
-  RR_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+  const bool closed = law != RR_LD_EXPONENTIAL;
   const int64_t n = M * ctx->nz;
   const unsigned grid = (unsigned)((n + 255) / 256);
   if (c.precision != RR_FP64)
     rr_ld_law_kernel<float><<<grid, 256, 0, st>>>(law, d_ldc, nc, ctx->d_mu, M, ctx->nz,
-                                                  (float *)wk->ldp, (float *)given, flag);
+                                                  (float *)wk->ldp,
+                                                  closed ? (float *)wk->istar : nullptr);
   else
     rr_ld_law_kernel<double><<<grid, 256, 0, st>>>(law, d_ldc, nc, ctx->d_mu, M, ctx->nz,
-                                                   (double *)wk->ldp, (double *)given, flag);
+                                                   (double *)wk->ldp,
+                                                   closed ? (double *)wk->istar : nullptr);
   RR_LAUNCH_CHECK(ctx);
-  int h_flag = 0;
-  RR_CUDA(cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
-  RR_CUDA(cudaStreamSynchronize(st));
-  const void *ist = h_flag ? nullptr : given;      // no closed form: discretised integral (R6)
-  if (ctx->table_mode != RR_TABLE_FULL && ctx->nz <= 2000)
+  const void *ist = closed ? wk->istar : nullptr;  // no closed form: discretised integral (R6)
+  if (!full)
     rc = rr_ld_profile_launch(ctx, wk, wk->ldp, ist, npv, 0, st);
   else
     rc = rr_ld_table_launch(ctx, wk, wk->ldp, ist, npv, st);
   if (rc == RR_OK && wk->lazy) wk->ldp_src = wk->ldp;
-  cudaStreamSynchronize(st);
-  cudaFree(given);
   return rc;
 }
