@@ -138,17 +138,52 @@ def _host(a, dtype):
     return np.ascontiguousarray(a, dtype=dtype)
 
 
+# What the library was told about each ctx (rr_create, rr_set_data, rr_build_ld_table*), kept so
+# that the wrappers can refuse a tensor of the wrong dtype or size BEFORE the kernels read or write
+# out of bounds: the C side sees raw pointers only.
+_CTX: dict[int, dict] = {}
+
+
+def _info(ctx: int, where: str) -> dict:
+    try:
+        return _CTX[int(ctx)]
+    except KeyError:
+        raise ValueError(f"{where}: unknown ctx handle (not made by rr_create, or destroyed)") from None
+
+
+def _torch_dtype(code: str):
+    import torch
+    return {"f64": torch.float64, "f32": torch.float32}[code]
+
+
+def _in_code(info) -> str:       # ldp, istar, table
+    return "f32" if info["precision"] != RR_FP64 else "f64"
+
+
+def _flux_code(info) -> str:     # flux (fp64 in RR_MIXED)
+    return "f32" if info["precision"] == RR_FP32 else "f64"
+
+
+def _numel(t, n: int, name: str, where: str):
+    if int(t.numel() if hasattr(t, "numel") else t.size) != int(n):
+        have = int(t.numel() if hasattr(t, "numel") else t.size)
+        raise ValueError(f"{where}: {name} must hold {n} elements, got {have}")
+
+
 # ---- one-to-one wrappers of the C entry points ----------------------------------------------------
 def rr_create(nzin=50, nzlimb=50, zcut=0.7, ng=100, nk=50, k0=0.02, k1=0.2, npb=1, nkpb=1,
               precision=RR_FP64) -> int:
     cfg = rr_config(nzin, nzlimb, zcut, ng, nk, k0, k1, npb, nkpb, precision)
     h = _VP()
     _check(load().rr_create(C.byref(cfg), C.byref(h)), "rr_create")
+    _CTX[int(h.value)] = dict(precision=int(precision), nz=int(nzin) + int(nzlimb), ng=int(ng),
+                              nk=int(nk), npb=int(npb), nkpb=int(nkpb), npt=0, npv=0)
     return h.value
 
 
 def rr_destroy(ctx: int):
     _check(load().rr_destroy(ctx), "rr_destroy")
+    _CTX.pop(int(ctx), None)
 
 
 def rr_get_mu(ctx: int, nz: int) -> np.ndarray:
@@ -183,33 +218,55 @@ def rr_set_data(ctx: int, times, lc_index, passband_index, supersampling, exposu
                               _dev(lc_index, torch.int32, "lc_index"), times.numel(),
                               pb.ctypes.data, ns.ctypes.data, et.ctypes.data, pb.size,
                               _stream(stream)), "rr_set_data")
+    _info(ctx, "rr_set_data")["npt"] = int(times.numel())
 
 
 def rr_build_ld_table(ctx: int, ldp, npv: int, istar=None, stream=None):
-    """ldp [npv][npb][nz] CUDA tensor in the ctx precision."""
-    _check(load().rr_build_ld_table(ctx, _dev(ldp, ldp.dtype, "ldp"),
-                                    None if istar is None else _dev(istar, ldp.dtype, "istar"),
-                                    npv, _stream(stream)), "rr_build_ld_table")
+    """ldp [npv][npb][nz] CUDA tensor in the ctx input precision (fp32 for RR_FP32 / RR_MIXED);
+    istar [npv][npb] optional, same dtype.  TypeError / ValueError on a dtype or size mismatch."""
+    info = _info(ctx, "rr_build_ld_table")
+    dt = _torch_dtype(_in_code(info))
+    npv = int(npv)
+    pl = _dev(ldp, dt, "ldp")
+    _numel(ldp, npv * info["npb"] * info["nz"], "ldp [npv][npb][nz]", "rr_build_ld_table")
+    pi = None
+    if istar is not None:
+        pi = _dev(istar, dt, "istar")
+        _numel(istar, npv * info["npb"], "istar [npv][npb]", "rr_build_ld_table")
+    _check(load().rr_build_ld_table(ctx, pl, pi, npv, _stream(stream)), "rr_build_ld_table")
+    info["npv"] = npv
 
 
 def rr_build_ld_table_law(ctx: int, law, ldc, npv: int, stream=None):
     """law: RR_LD_* code or a name of LD_LAWS; ldc f64 CUDA tensor [npv][npb][nldc] (or None for
     the uniform law)."""
     import torch
+    info = _info(ctx, "rr_build_ld_table_law")
     code = LD_LAWS[law] if isinstance(law, str) else int(law)
     nldc = 0 if ldc is None else int(ldc.shape[-1])
-    _check(load().rr_build_ld_table_law(ctx, code,
-                                        None if ldc is None else _dev(ldc, torch.float64, "ldc"),
-                                        nldc, npv, _stream(stream)), "rr_build_ld_table_law")
+    npv = int(npv)
+    pc = None
+    if ldc is not None:
+        pc = _dev(ldc, torch.float64, "ldc")
+        _numel(ldc, npv * info["npb"] * nldc, "ldc [npv][npb][nldc]", "rr_build_ld_table_law")
+    _check(load().rr_build_ld_table_law(ctx, code, pc, nldc, npv, _stream(stream)),
+           "rr_build_ld_table_law")
+    info["npv"] = npv
 
 
 def rr_evaluate(ctx: int, pv, flux, status=None, stream=None):
     """pv f64 [npv][npar] -> flux [npv][npt] (ctx precision), status i32 [npv] optional."""
     import torch
+    info = _info(ctx, "rr_evaluate")
     npv, npar = pv.shape
-    _check(load().rr_evaluate(ctx, _dev(pv, torch.float64, "pv"), npar, npv,
-                              _dev(flux, flux.dtype, "flux"),
-                              None if status is None else _dev(status, torch.int32, "status"),
+    pf = _dev(flux, _torch_dtype(_flux_code(info)), "flux")
+    if info["npt"] > 0 and npar == info["nkpb"] + 6:     # otherwise the library reports the state
+        _numel(flux, npv * info["npt"], "flux [npv][npt]", "rr_evaluate")
+    ps = None
+    if status is not None:
+        ps = _dev(status, torch.int32, "status")
+        _numel(status, npv, "status [npv]", "rr_evaluate")
+    _check(load().rr_evaluate(ctx, _dev(pv, torch.float64, "pv"), npar, npv, pf, ps,
                               _stream(stream)), "rr_evaluate")
 
 
@@ -218,22 +275,36 @@ def rr_evaluate_flat(ctx: int, times, lc_index, passband_index, supersampling, e
     import torch
     pb, ns, et = _host(passband_index, np.int32), _host(supersampling, np.int32), \
         _host(exposure_time, np.float64)
+    info = _info(ctx, "rr_evaluate_flat")
     npv, npar = pv.shape
-    _check(load().rr_evaluate_flat(ctx, _dev(times, torch.float64, "times"),
-                                   _dev(lc_index, torch.int32, "lc_index"), times.numel(),
-                                   pb.ctypes.data, ns.ctypes.data, et.ctypes.data, pb.size,
-                                   _dev(pv, torch.float64, "pv"), npar, npv,
-                                   _dev(flux, flux.dtype, "flux"),
-                                   None if status is None else _dev(status, torch.int32, "status"),
-                                   _stream(stream)), "rr_evaluate_flat")
+    if not (pb.size == ns.size == et.size):
+        raise ValueError("passband_index, supersampling, exposure_time must have nlc entries each")
+    if times.numel() != lc_index.numel():
+        raise ValueError("times and lc_index must have npt entries each")
+    pf = _dev(flux, _torch_dtype(_flux_code(info)), "flux")
+    _numel(flux, npv * int(times.numel()), "flux [npv][npt]", "rr_evaluate_flat")
+    ps = None
+    if status is not None:
+        ps = _dev(status, torch.int32, "status")
+        _numel(status, npv, "status [npv]", "rr_evaluate_flat")
+    rc = load().rr_evaluate_flat(ctx, _dev(times, torch.float64, "times"),
+                                 _dev(lc_index, torch.int32, "lc_index"), times.numel(),
+                                 pb.ctypes.data, ns.ctypes.data, et.ctypes.data, pb.size,
+                                 _dev(pv, torch.float64, "pv"), npar, npv, pf, ps, _stream(stream))
+    if rc == 0 or rc == -5:      # RR_ESTATE comes from rr_evaluate: the data were set
+        info["npt"] = int(times.numel())
+    _check(rc, "rr_evaluate_flat")
 
 
 def rr_orbit_z(ctx: int, pv, z, fp32_math=False, stream=None):
     import torch
     npv, npar = pv.shape
-    _check(load().rr_orbit_z(ctx, _dev(pv, torch.float64, "pv"), npar, npv,
-                             _dev(z, torch.float64, "z"), int(bool(fp32_math)), _stream(stream)),
-           "rr_orbit_z")
+    pz = _dev(z, torch.float64, "z")
+    nsub = rr_num_subsamples(ctx)
+    if nsub >= 0:
+        _numel(z, npv * nsub, "z [npv][nsub]", "rr_orbit_z")
+    _check(load().rr_orbit_z(ctx, _dev(pv, torch.float64, "pv"), npar, npv, pz,
+                             int(bool(fp32_math)), _stream(stream)), "rr_orbit_z")
 
 
 def rr_num_subsamples(ctx: int) -> int:
@@ -286,12 +357,22 @@ def rr_get_kernel_times(ctx: int) -> dict:
 def rr_evaluate_host(ctx: int, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray,
                      status: np.ndarray | None = None):
     """Whole step from HOST arrays (numpy, or the .numpy() view of a pinned torch tensor)."""
+    info = _info(ctx, "rr_evaluate_host")
     if not (ldp.flags.c_contiguous and pv.flags.c_contiguous and flux.flags.c_contiguous):
         raise TypeError("host arrays must be C-contiguous")
-    if pv.dtype != np.float64 or ldp.dtype not in (np.float32, np.float64) \
-            or flux.dtype not in (np.float32, np.float64):
-        raise TypeError("pv must be float64; ldp and flux float32/float64 as the ctx precision asks")
+    want_in = np.float32 if info["precision"] != RR_FP64 else np.float64
+    want_out = np.float32 if info["precision"] == RR_FP32 else np.float64
+    if pv.dtype != np.float64 or ldp.dtype != want_in or flux.dtype != want_out:
+        raise TypeError(f"pv must be float64, ldp {np.dtype(want_in)} and flux {np.dtype(want_out)} "
+                        f"for this ctx; got {pv.dtype}, {ldp.dtype}, {flux.dtype}")
     npv, npar = pv.shape
+    _numel(ldp, npv * info["npb"] * info["nz"], "ldp [npv][npb][nz]", "rr_evaluate_host")
+    if info["npt"] > 0 and npar == info["nkpb"] + 6:
+        _numel(flux, npv * info["npt"], "flux [npv][npt]", "rr_evaluate_host")
+    if status is not None:
+        if status.dtype != np.int32 or not status.flags.c_contiguous:
+            raise TypeError("status must be C-contiguous int32")
+        _numel(status, npv, "status [npv]", "rr_evaluate_host")
     _check(load().rr_evaluate_host(ctx, ldp.ctypes.data, pv.ctypes.data, npar, npv,
                                    flux.ctypes.data,
                                    None if status is None else status.ctypes.data),
@@ -369,10 +450,12 @@ class RoadRunner:
         """ldp: CUDA tensor or array [npv][npb][nz]."""
         import torch
         if not isinstance(ldp, torch.Tensor):
-            ldp = torch.as_tensor(np.ascontiguousarray(ldp)).to(self.dtype).cuda()
-        ldp = ldp.reshape(-1, self.npb, self.nz).contiguous()
-        if istar is not None and not isinstance(istar, torch.Tensor):
-            istar = torch.as_tensor(np.ascontiguousarray(istar)).to(self.dtype).cuda()
+            ldp = torch.as_tensor(np.ascontiguousarray(ldp))
+        ldp = ldp.to(device="cuda", dtype=self.dtype).reshape(-1, self.npb, self.nz).contiguous()
+        if istar is not None:
+            if not isinstance(istar, torch.Tensor):
+                istar = torch.as_tensor(np.ascontiguousarray(istar))
+            istar = istar.to(device="cuda", dtype=self.dtype).contiguous()
         self.npv = ldp.shape[0]
         rr_build_ld_table(self.ctx, ldp, self.npv, istar)
 

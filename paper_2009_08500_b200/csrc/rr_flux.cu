@@ -430,10 +430,21 @@ __device__ __forceinline__ R rr_separation2(const Cst<R, M> K, double ur, bool &
     // is accepted for ~94 % of config 4's eccentric sub-samples
 #pragma unroll 1
     for (int it = 0; it < 3 && fabs(d) <= (R)RR_TRIG_SMALL; ++it) {
-      R s, cm1;
-      rr_sincosm1_small(d, s, cm1);
-      const R t = fma(B, cm1, C * s);              // e [sin E - sin E_tr]
-      const R g = (d - dM) - t;
+      R s, cm1, t, g;
+      if constexpr (sizeof(R) == 8) {
+        rr_sincosm1_small(d, s, cm1);
+        t = fma(B, cm1, C * s);                    // e [sin E - sin E_tr]
+        g = (d - dM) - t;
+      } else {
+        // fp32: d - t = A d - C (sin d - d) - B (cos d - 1), A = 1 - e cos E_tr rounded once from
+        // fp64.  Formed this way the residual carries eps |dM| instead of eps |d| ~ eps |dM| / A
+        // (the direct form loses 1/(1 - e) near a periastron transit: 4e-7 in flux at e = 0.99).
+        R sres;
+        rr_sincosm1_small(d, s, cm1, sres);
+        const R bc = B * cm1;
+        t = fma(C, s, bc);
+        g = fma(A, d, -dM) - fma(C, sres, bc);
+      }
       const R gp = A - fma(C, cm1, -B * s);        // 1 - e cos E
       const R gpp = B + t;                         // e sin E
       // Halley: -2 g g' / (2 g'^2 - g g'') = -(g g') / (g'^2 - g g''/2)

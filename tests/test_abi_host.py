@@ -147,3 +147,27 @@ def test_bench_reference_arm_runs_on_cpu():
     assert line["impl"] == "reference" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_binding_refuses_unknown_handles_and_wrong_sizes_without_a_device():
+    """The wrappers check dtype and element counts against what rr_create / rr_set_data were told
+    before any pointer reaches the library (the C side sees raw pointers only)."""
+    import paper_2009_08500_b200 as rr
+    with pytest.raises(ValueError, match="unknown ctx"):
+        rr.rr_evaluate_host(123456, np.ones((1, 1, 100)), np.ones((1, 7)), np.ones((1, 10)))
+    rr._CTX[999] = dict(precision=rr.RR_FP32, nz=100, ng=100, nk=50, npb=1, nkpb=1, npt=10, npv=0)
+    try:
+        pv = np.ones((2, 7))
+        with pytest.raises(TypeError, match="float32"):       # fp64 profile for an fp32 ctx
+            rr.rr_evaluate_host(999, np.ones((2, 1, 100)), pv, np.ones((2, 10), np.float32))
+        with pytest.raises(ValueError, match="flux"):         # short flux buffer
+            rr.rr_evaluate_host(999, np.ones((2, 1, 100), np.float32), pv,
+                                np.ones((2, 9), np.float32))
+        with pytest.raises(ValueError, match="ldp"):          # profile of another resolution
+            rr.rr_evaluate_host(999, np.ones((2, 1, 50), np.float32), pv,
+                                np.ones((2, 10), np.float32))
+        with pytest.raises(TypeError, match="status"):
+            rr.rr_evaluate_host(999, np.ones((2, 1, 100), np.float32), pv,
+                                np.ones((2, 10), np.float32), np.zeros(2, np.int64))
+    finally:
+        rr._CTX.pop(999)
