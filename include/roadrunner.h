@@ -255,6 +255,25 @@ int rr_get_kernel_times(rr_ctx *ctx, double *h_ms /*[2]*/, int64_t *h_calls);
  * Synchronous.                                                                                   */
 int rr_measure_fma_peak(int32_t precision, double *h_fma_per_s, void *stream);
 
+/* ---- test aid: the device math of the hot path, element by element ------------------------------
+ * The flux kernel's own square root, division, arctangents, sin / cos - 1 polynomials and table-cell
+ * split (csrc/rr_math.cuh; ranges and error bounds in DESIGN.md section 6) applied to d_a[n] (and
+ * d_b[n] for the two-argument functions), in fp64 or - fp32_math != 0 - in the fp32 arithmetic of the
+ * RR_FP32 kernel (inputs rounded to fp32, results widened).  d_out1 (optional) receives the second
+ * result of RR_PROBE_SINCOSM1 (cos x - 1) and RR_PROBE_CELL (the weight a = y - floor y).
+ * Asynchronous on `stream`.  Tests compare the results with 50-digit arithmetic.                  */
+#define RR_PROBE_SQRT3          0  /* sqrt(a), a > 0: seed + one third-order step                  */
+#define RR_PROBE_SQRT           1  /* sqrt(a), any a (0 for a <= 0): seed + two Goldschmidt steps  */
+#define RR_PROBE_DIV3           2  /* a / b, b > 0                                                 */
+#define RR_PROBE_RCP            3  /* 1 / a to ~1e-12 (fp64) / ~1e-7 (fp32)                        */
+#define RR_PROBE_ATAN_T         4  /* atan(a), |a| <= tan(pi/8)                                    */
+#define RR_PROBE_ATAN_QUADRANT  5  /* atan(sqrt(b/a)) in [0, pi/2] from S = a > 0, P = b >= 0      */
+#define RR_PROBE_ATAN2_POS      6  /* atan2(a, b), a >= 0: the angle in [0, pi]                    */
+#define RR_PROBE_SINCOSM1       7  /* sin a, cos a - 1, |a| <= 0.5                                 */
+#define RR_PROBE_CELL           8  /* floor(a) and a - floor(a), 0 <= a < 2^31                     */
+int rr_math_probe(int32_t op, int32_t fp32_math, const double *d_a, const double *d_b, int64_t n,
+                  double *d_out0, double *d_out1, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -36,8 +36,10 @@ SYMBOLS = (
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
-    "rr_set_small_planet", "rr_build_ld_table_law",
+    "rr_set_small_planet", "rr_build_ld_table_law", "rr_math_probe",
 )
+PROBE_OPS = {"sqrt3": 0, "sqrt": 1, "div3": 2, "rcp": 3, "atan_t": 4, "atan_quadrant": 5,
+             "atan2_pos": 6, "sincosm1": 7, "cell": 8}
 
 
 class RoadRunnerError(RuntimeError):
@@ -100,6 +102,7 @@ def load() -> C.CDLL:
         "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
         "rr_set_small_planet": (C.c_int, [_VP, _DBL]),
         "rr_build_ld_table_law": (C.c_int, [_VP, _I32, _VP, _I32, _I64, _VP]),
+        "rr_math_probe": (C.c_int, [_I32, _I32, _VP, _VP, _I64, _VP, _VP, _VP]),
         "rr_enable_kernel_timing": (C.c_int, [_VP, _I32]),
         "rr_get_kernel_times": (C.c_int, [_VP, _VP, C.POINTER(_I64)]),
     }
@@ -377,6 +380,22 @@ def rr_evaluate_host(ctx: int, ldp: np.ndarray, pv: np.ndarray, flux: np.ndarray
                                    flux.ctypes.data,
                                    None if status is None else status.ctypes.data),
            "rr_evaluate_host")
+
+
+def rr_math_probe(op, a, b=None, fp32_math=False, stream=None):
+    """Device math of the hot path applied element by element (tests): a, b fp64 CUDA tensors of
+    n entries -> (out0, out1) fp64 CUDA tensors."""
+    import torch
+    code = PROBE_OPS[op] if isinstance(op, str) else int(op)
+    n = a.numel()
+    if b is not None and b.numel() != n:
+        raise ValueError("rr_math_probe: a and b must have the same number of elements")
+    o0 = torch.empty(n, dtype=torch.float64, device=a.device)
+    o1 = torch.zeros(n, dtype=torch.float64, device=a.device)
+    _check(load().rr_math_probe(code, int(bool(fp32_math)), _dev(a, torch.float64, "a"),
+                                None if b is None else _dev(b, torch.float64, "b"), n,
+                                o0.data_ptr(), o1.data_ptr(), _stream(stream)), "rr_math_probe")
+    return o0, o1
 
 
 def rr_enable_counters(ctx: int, on: bool):

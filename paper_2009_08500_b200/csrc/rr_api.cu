@@ -489,6 +489,17 @@ int rr_get_kernel_times(rr_ctx *ctx, double *h_ms, int64_t *h_calls) {
   return rc;
 }
 
+int rr_math_probe(int32_t op, int32_t fp32_math, const double *d_a, const double *d_b, int64_t n,
+                  double *d_out0, double *d_out1, void *stream) {
+  if (!d_a || !d_out0) return RR_ENULL;
+  if (op < RR_PROBE_SQRT3 || op > RR_PROBE_CELL) return RR_ECONFIG;
+  const bool two = op == RR_PROBE_DIV3 || op == RR_PROBE_ATAN_QUADRANT || op == RR_PROBE_ATAN2_POS;
+  if (two && !d_b) return RR_ENULL;
+  if (n <= 0) return RR_ESIZE;
+  return rr_math_probe_launch(op, fp32_math != 0, d_a, two ? d_b : nullptr, n, d_out0, d_out1,
+                              (cudaStream_t)stream);
+}
+
 int rr_measure_fma_peak(int32_t precision, double *h_fma_per_s, void *stream) {
   if (!h_fma_per_s) return RR_ENULL;
   if (precision != RR_FP64 && precision != RR_FP32 && precision != RR_MIXED) return RR_ECONFIG;

@@ -163,3 +163,5 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
                     cudaStream_t st);
 int rr_fma_peak_launch(int precision, double *h_fma_per_s, cudaStream_t st);   // rr_flux.cu
 int rr_smem_probe(int *abs_ok);                                                // rr_flux.cu
+int rr_math_probe_launch(int op, int fp32, const double *d_a, const double *d_b, int64_t n,
+                         double *d_o0, double *d_o1, cudaStream_t st);         // rr_flux.cu

@@ -967,7 +967,47 @@ int fma_peak_typed(double *h_fma_per_s, cudaStream_t st) {
   return RR_OK;
 }
 
+// ---- device math probe (tests): the functions of rr_math.cuh applied element by element ------------
+template <typename R>
+__global__ void rr_math_probe_kernel(int op, const double *__restrict__ a, const double *__restrict__ b,
+                                     int64_t n, double *__restrict__ o0, double *__restrict__ o1) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const R x = (R)a[i], y = b ? (R)b[i] : (R)0;
+  R r0 = (R)0, r1 = (R)0;
+  switch (op) {
+    case RR_PROBE_SQRT3: r0 = rr_sqrt3(x); break;
+    case RR_PROBE_SQRT: r0 = rr_sqrt(x); break;
+    case RR_PROBE_DIV3: r0 = rr_div3(x, y); break;
+    case RR_PROBE_RCP: r0 = rr_rcp(x); break;
+    case RR_PROBE_ATAN_T: r0 = rr_atan_t(x); break;
+    case RR_PROBE_ATAN_QUADRANT: r0 = rr_atan_quadrant<R>(rr_sqrt3_pos(x * y), x, y); break;
+    case RR_PROBE_ATAN2_POS: r0 = rr_atan2_pos(x, y); break;
+    case RR_PROBE_SINCOSM1: rr_sincosm1_small(x, r0, r1); break;
+    case RR_PROBE_CELL: {
+      int ig;
+      R ag;
+      rr_cell(x, ig, ag);
+      r0 = (R)ig;
+      r1 = ag;
+      break;
+    }
+    default: break;
+  }
+  o0[i] = (double)r0;
+  if (o1) o1[i] = (double)r1;
+}
+
 }  // namespace
+
+int rr_math_probe_launch(int op, int fp32, const double *d_a, const double *d_b, int64_t n,
+                         double *d_o0, double *d_o1, cudaStream_t st) {
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  if (fp32) rr_math_probe_kernel<float><<<grid, 256, 0, st>>>(op, d_a, d_b, n, d_o0, d_o1);
+  else rr_math_probe_kernel<double><<<grid, 256, 0, st>>>(op, d_a, d_b, n, d_o0, d_o1);
+  RR_CUDA(cudaGetLastError());
+  return RR_OK;
+}
 
 // Extra nodes of the staged table row beyond ng - 1 (all equal to the limb node): 1 normally; with
 // mean-k weights and chromatic k, g = z/(1+kw) of a passband with k > kw runs up to (1+k)/(1+kw).

@@ -1,0 +1,115 @@
+"""The polynomial tables of the device math (paper_2009_08500_b200/csrc/rr_math.cuh) against their
+generator (tests/golden/make_device_poly.py, mpmath only) and against mpmath's atan / sin / cos in
+50-digit arithmetic over the ranges the kernels use them on.  CPU only: the literals are parsed
+from the source file; nothing here runs CUDA code."""
+import os
+import re
+import sys
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, os.path.join(ROOT, "tests", "golden"))
+import make_device_poly as gen  # noqa: E402
+
+SRC = open(os.path.join(ROOT, "paper_2009_08500_b200", "csrc", "rr_math.cuh")).read()
+
+
+def parsed(name):
+    m = re.search(r"__constant__\s+(double|float)\s+" + name + r"\[(\d+)\]\s*=\s*\{(.*?)\};", SRC, re.S)
+    assert m, name
+    ty, n, body = m.group(1), int(m.group(2)), m.group(3)
+    vals = []
+    for tok in body.replace("\n", " ").split(","):
+        tok = tok.strip()
+        if "/" in tok:                               # "-1.0 / 6.0", "1.0f / 120.0f"
+            a, b = (float(x.strip().rstrip("f")) for x in tok.split("/"))
+            vals.append(np.float32(np.float32(a) / np.float32(b)) if ty == "float" else a / b)
+        else:
+            vals.append(np.float32(tok.rstrip("f")) if ty == "float" else float(tok))
+    assert len(vals) == n
+    return ty, vals
+
+
+@pytest.mark.parametrize("name", sorted(gen.TABLES))
+def test_tables_equal_the_generator(name):
+    """Every literal equals the generator's value rounded to the table's type."""
+    ty, have = parsed(name)
+    want = gen.table(name)
+    assert gen.TABLES[name][2] == ty and len(want) == len(have)
+    for h, w in zip(have, want):
+        w_r = np.float32(float(w)) if ty == "float" else float(w)
+        assert h == w_r, (name, h, w_r)
+
+
+def _horner(coefs, u):
+    q = mp.mpf(0)
+    for c in reversed(coefs):
+        q = q * u + mp.mpf(float(c))
+    return q
+
+
+def _grid(hi, n=1501):
+    return [mp.mpf(hi) * i / (n - 1) for i in range(n)]
+
+
+@pytest.mark.parametrize("name,bound", [("RR_ATAN_D", 3e-18), ("RR_ATAN_F", 1e-9)])
+def test_atan_polynomial_error(name, bound):
+    """atan t = t + t u Q(u) on |t| <= tan(pi/8), and a little beyond (rr_atan_quadrant's T^2 is
+    rounded down, so the reduced argument passes tan(pi/8) by <= 2.1e-7 relative)."""
+    mp.mp.dps = 50
+    _, coefs = parsed(name)
+    worst = mp.mpf(0)
+    for t in _grid(mp.tan(mp.pi / 8) * (1 + mp.mpf("1e-6"))):
+        u = t * t
+        worst = max(worst, abs(t + t * u * _horner(coefs, u) - mp.atan(t)))
+    assert worst <= bound, mp.nstr(worst, 5)
+
+
+@pytest.mark.parametrize("sname,cname,bs,bc", [("RR_SIN_D", "RR_COS_D", 5.2e-17, 7.1e-18),
+                                               ("RR_SIN_F", "RR_COS_F", 1.3e-8, 2.9e-9)])
+def test_trig_polynomial_error(sname, cname, bs, bc):
+    """sin x = x + x^3 S(x^2) (relative error) and cos x - 1 = x^2 C(x^2) (relative to x^2/2) on
+    |x| <= 0.5: the truncation bounds stated in rr_math.cuh."""
+    mp.mp.dps = 50
+    _, cs = parsed(sname)
+    _, cc = parsed(cname)
+    ws = wc = mp.mpf(0)
+    for x in _grid(gen.TRIG_RANGE)[1:]:
+        x2 = x * x
+        ws = max(ws, abs(x + x * x2 * _horner(cs, x2) - mp.sin(x)) / mp.sin(x))
+        wc = max(wc, abs(x2 * _horner(cc, x2) - (mp.cos(x) - 1)) / (x2 / 2))
+    assert ws <= bs and wc <= bc, (mp.nstr(ws, 5), mp.nstr(wc, 5))
+
+
+def test_third_order_seed_corrections():
+    """rr_sqrt3 / rr_div3 (rr_math.cuh): one third-order step from a hardware seed of relative error
+    |d| <= 2^-20 leaves < 3e-18 (sqrt) and < 1e-18 (reciprocal); checked on the formulas as the file
+    states them, in exact arithmetic."""
+    mp.mp.dps = 50
+    for x in (mp.mpf("0.37"), mp.mpf(2), mp.mpf("1.7e-3"), mp.mpf(977)):
+        for d in (mp.mpf(2) ** -20, -mp.mpf(2) ** -20, mp.mpf(2) ** -21, -mp.mpf(2) ** -23):
+            y = (1 + d) / mp.sqrt(x)                      # rsqrt seed
+            g, h = x * y, y / 2
+            r = mp.mpf("0.5") - h * g
+            s = g * r * (mp.mpf("1.5") * r + 1) + g
+            assert abs(s / mp.sqrt(x) - 1) < 3e-18
+            rc = (1 + d) / x                              # rcp seed
+            e = 1 - x * rc
+            rc3 = rc * (e * e + e) + rc
+            assert abs(rc3 * x - 1) < 1e-18
+
+
+def test_octant_threshold_literal():
+    """rr_atan_quadrant's T2: tan^2(pi/8) rounded DOWN to a double with a zero low word (an
+    immediate operand); the reduced argument t then passes tan(pi/8) by at most 2.1e-7."""
+    mp.mp.dps = 30
+    m = re.search(r"\(R\)(0\.1715728\d+)\s*:\s*\(R\)(0\.1715728\d+)f", SRC)
+    assert m
+    t2d = float(m.group(1))
+    exact = mp.tan(mp.pi / 8) ** 2
+    assert np.float64(t2d).view(np.uint64) & np.uint64(0xffffffff) == 0
+    assert 0 <= mp.sqrt(exact / mp.mpf(t2d)) - 1 < 2.1e-7
+    assert abs(mp.mpf(float(np.float32(m.group(2)))) / exact - 1) < 1e-7

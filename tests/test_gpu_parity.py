@@ -1050,3 +1050,81 @@ def test_named_law_build_is_asynchronous_and_repeatable(rr):
     for a, b in zip(ref, outs):
         assert torch.equal(a, b)
     gm.close()
+
+
+# ---- the device math of the hot path, function by function (rr_math.cuh through rr_math_probe) ----------
+def _mp_vec(f, *cols):
+    import mpmath as mp
+    mp.mp.dps = 40
+    return np.array([float(f(*[mp.mpf(float(x)) for x in row])) for row in zip(*cols)])
+
+
+@pytest.mark.parametrize("fp32", [False, True])
+def test_device_math_against_multiprecision(rr, fp32):
+    """rr_sqrt3 / rr_sqrt / rr_div3 / rr_rcp / rr_atan_t / rr_atan_quadrant / rr_atan2_pos /
+    rr_sincosm1_small / rr_cell on the ranges the kernels use them on, against 40-digit arithmetic:
+    fp64 within a few ulp, fp32 within a few fp32 ulp (the bounds DESIGN.md s6 states)."""
+    import mpmath as mp
+    import torch
+    rng = np.random.default_rng(31)
+    n = 4000
+    ulp = 2.0 ** -23 if fp32 else 2.0 ** -52
+
+    def dev(x):
+        x = np.asarray(x, np.float64)
+        if fp32:
+            x = x.astype(np.float32).astype(np.float64)        # the probe rounds its inputs to fp32
+        return x, torch.as_tensor(x).cuda()
+
+    def run(op, a, b=None):
+        o0, o1 = rr.rr_math_probe(op, a, b, fp32_math=fp32)
+        return o0.cpu().numpy(), o1.cpu().numpy()
+
+    # square roots: z^2 from 1e-12 to 1e4, and exact squares
+    x, xd = dev(np.concatenate([10.0 ** rng.uniform(-12, 4, n), np.arange(1.0, 30.0) ** 2]))
+    want = _mp_vec(mp.sqrt, x)
+    for op in ("sqrt3", "sqrt"):
+        got, _ = run(op, xd)
+        assert np.max(np.abs(got / want - 1.0)) <= 2.0 * ulp, op
+    got, _ = run("sqrt", torch.as_tensor(np.array([0.0, -1.0, -1e-300])).cuda())
+    assert np.array_equal(got, np.zeros(3))
+    # division and reciprocal
+    a, ad = dev(rng.uniform(-3, 3, n))
+    b, bd = dev(10.0 ** rng.uniform(-6, 3, n))
+    got, _ = run("div3", ad, bd)
+    assert np.max(np.abs(got - _mp_vec(lambda p, q: p / q, a, b)) / np.maximum(np.abs(a / b), 1e-300)) \
+        <= 2.0 * ulp
+    got, _ = run("rcp", bd)
+    assert np.max(np.abs(got * b - 1.0)) <= (3e-7 if fp32 else 1e-11)
+    # atan on the reduced range, a little beyond it, and near zero
+    T = float(mp.tan(mp.pi / 8))
+    t, td = dev(np.concatenate([rng.uniform(-T, T, n), [T * (1 + 2e-7), -T, 0.0, 1e-9, 1e-300]]))
+    got, _ = run("atan_t", td)
+    want = _mp_vec(mp.atan, t)
+    assert np.max(np.abs(got - want)) <= 1.5 * ulp * 0.5          # |atan| < 0.4: 1.5 ulp of 0.25..0.5
+    # the lens half-angles: atan(sqrt(P/S)) from (S, P), every octant, the octant boundaries, P = 0
+    S, Sd = dev(np.concatenate([10.0 ** rng.uniform(-8, 1, n), [1.0, 1.0, 1.0, 2.0, 3.0]]))
+    P, Pd = dev(np.concatenate([10.0 ** rng.uniform(-8, 1, n),
+                                [0.0, T * T, 1.0 / (T * T), 2.0, 1e-30]]))
+    got, _ = run("atan_quadrant", Sd, Pd)
+    want = _mp_vec(lambda s_, p_: mp.atan(mp.sqrt(p_ / s_)), S, P)
+    assert np.max(np.abs(got - want)) <= (6.0 if fp32 else 4.0) * ulp
+    # atan2 for y >= 0 (direct-model rows)
+    y, yd = dev(np.concatenate([10.0 ** rng.uniform(-8, 1, n), [0.0, 1.0, 1.0]]))
+    xx, xxd = dev(np.concatenate([rng.uniform(-3, 3, n), [1.0, 0.0, -1.0]]))
+    got, _ = run("atan2_pos", yd, xxd)
+    want = _mp_vec(mp.atan2, y, xx)
+    assert np.max(np.abs(got - want)) <= (8.0 if fp32 else 4.0) * ulp
+    # sin, cos - 1 on |x| <= 0.5: relative accuracy (what the d = E - E_tr formulation relies on)
+    d, dd = dev(np.concatenate([rng.uniform(-0.5, 0.5, n), 10.0 ** rng.uniform(-12, -1, 500),
+                                [0.5, -0.5, 0.0]]))
+    s_g, c_g = run("sincosm1", dd)
+    s_w, c_w = _mp_vec(mp.sin, d), _mp_vec(lambda v: mp.cos(v) - 1, d)
+    nz = d != 0
+    assert np.max(np.abs(s_g[nz] / s_w[nz] - 1.0)) <= 2.0 * ulp
+    assert np.max(np.abs(c_g[nz] / c_w[nz] - 1.0)) <= 2.5 * ulp
+    assert s_g[~nz].item() == 0.0 and c_g[~nz].item() == 0.0
+    # table cell: floor and fractional part, exact
+    yv, yvd = dev(np.concatenate([rng.uniform(0, 5000, n), [0.0, 98.99999999999999, 99.0, 4999.5]]))
+    ig, ag = run("cell", yvd)
+    assert np.array_equal(ig, np.floor(yv)) and np.array_equal(ag, yv - np.floor(yv))
