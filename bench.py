@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py - transit-model evaluations/s of the CUDA library on the BASELINE.json workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--precision fp64|fp32]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4|4b] [--precision fp64|fp32|mixed]
+                    [--scaling weak|strong] [--ld-law quadratic] [--no-all-configs]
     python bench.py --impl reference ...          # the CPU oracle, as it stands, on the host cores
 
 A "step" is one pass of the whole hot path over one batch of synthetic input:
@@ -10,9 +11,14 @@ was built once by rr_set_data, the paper's call pattern PAPER.md:207-218).  Defa
 config 4 of BASELINE.json (the largest population workload, the one the north-star target is
 stated on), fp64.  One JSON line on stdout (rank 0).  See DESIGN.md s8 for every field.
 
-Multi-GPU (torchrun, one process per GPU): the path shards over parameter vectors with no exchange,
-so each rank evaluates its own full population (weak scaling) and the only communication is the
-barrier and the max-over-ranks of the device time.
+After the headline timing the default single-GPU run also times every other BASELINE config and
+precision for a few steps each (``all_configs``: evaluations/s, kernel times, roofline fraction and the
+largest |flux - oracle| on a sample), SURVEY.md 8(d)'s per-config report.
+
+Multi-GPU (torchrun, one process per GPU): the path shards over parameter vectors with no exchange.
+``--scaling weak`` (default): each rank evaluates its own full population; ``--scaling strong``: ONE
+population is split with ``shard.pv_slice``.  The only communication is the barrier and the
+max-over-ranks of the device time.
 """
 from __future__ import annotations
 
@@ -38,6 +44,7 @@ FP64_LANES_PER_SM, FP32_LANES_PER_SM, SM_COUNT = 64, 128, 148
 # algorithmic FMA-pipe instructions (DFMA/DMUL/DADD; fp32 mode: FFMA-class, with the
 # fp64 phase instructions counted twice) per unit of each class of the flux kernel.  Sub-samples in
 # merged out-of-window fill runs cost no arithmetic.
+CIRC_PER_SUBSAMPLE, CIRC_PER_EXPOSURE = 6.0, 19.0   # fp64 circular path: rotation + z^2; phase + sincos
 ALG_OPS = {
     "fp64": dict(skipped=1, circular=16, eccentric_fixed=24, solver_iter=31, occulting=13,
                  ingress=62),
@@ -52,7 +59,8 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", default="4", choices=["0", "1", "2", "3", "4", "4b"],
+                    help="BASELINE.json config; 4b = config 4 with literal 2-minute spacing (SURVEY 8(d))")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"],
                     help="mixed = fp32 z and Ip*Ap, fp64 averaging / subtraction / flux (PAPER.md:293)")
     ap.add_argument("--npv", type=int, default=None, help="shrink the population (debugging)")
@@ -60,9 +68,19 @@ def parse_args():
     ap.add_argument("--table-mode", default="lazy", choices=["lazy", "full", "direct"],
                     help="kernel 1: rows for each pv's k at evaluate time (default), the full table, "
                          "or the paper's direct model (weights at each pv's own k, no k grid)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: a full population per rank (weak) or one population split by "
+                         "shard.pv_slice (strong)")
+    ap.add_argument("--ld-law", default=None, choices=["quadratic"],
+                    help="time the step with rr_build_ld_table_law (the law evaluated on the device "
+                         "from its coefficients, PAPER.md:143-156) instead of rr_build_ld_table")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    return ap.parse_args()
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="skip the per-config / per-precision report after the headline timing")
+    args = ap.parse_args()
+    args.config = args.config if args.config == "4b" else int(args.config)
+    return args
 
 
 def workload_config(wl, precision, extra=None):
@@ -77,17 +95,31 @@ def workload_config(wl, precision, extra=None):
     return cfg
 
 
-def ncu_traffic(workload: str, precision: str):
-    """dram read + write bytes per launch of rr_flux_kernel from the committed ncu capture."""
+def ncu_capture(workload: str, precision: str):
+    """The committed `ncu --set full` capture of rr_flux_kernel for this workload and precision
+    (profiles/flux_kernel_ncu.csv, one row per capture): dram bytes and executed arithmetic
+    thread-instructions per launch, or None."""
     try:
-        with open(os.path.join(ROOT, "profiles", "flux_kernel_dram_traffic.csv")) as f:
-            for line in f.read().splitlines()[1:]:
-                w, p, rd, wr, _ = line.split(",")
-                if w == workload and p == precision:
-                    return int(rd) + int(wr)
-    except (OSError, ValueError):
+        with open(os.path.join(ROOT, "profiles", "flux_kernel_ncu.csv")) as f:
+            rows = [ln.split(",") for ln in f.read().splitlines() if ln and not ln.startswith("#")]
+        cols = rows[0]
+        for r in rows[1:]:
+            d = dict(zip(cols, r))
+            if d["workload"] == workload and d["precision"] == precision:
+                return d
+    except (OSError, ValueError, KeyError, IndexError):
         pass
     return None
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 # ---- clocks ------------------------------------------------------------------------------------
@@ -138,27 +170,53 @@ class ClockSampler:
 
 
 # ---- the reference arm: the oracle on the host cores ---------------------------------------------
-def oracle_rate(wl, target_s: float, nthreads: int = 0):
-    """Oracle (table build + evaluate) on the first n pvs of the workload, n calibrated so that
-    the run takes about target_s.  Returns (evaluations/s, seconds, n_pv)."""
+def oracle_sample(wl, stride: int):
+    """Every stride-th parameter vector of the workload, all exposures."""
+    return wl.subset_pv(np.arange(0, wl.npv, max(1, stride)))
+
+
+def oracle_run(sub, nthreads: int):
+    """Oracle as it stands (table build + evaluate) on a sub-population: evaluations/s, seconds.
+    nthreads = 0: all cores (passed explicitly: the OpenMP thread count is sticky)."""
     import oracle
-    om = oracle.OracleModel.from_config(wl.model)
+    nthreads = nthreads or (os.cpu_count() or 1)
+    om = oracle.OracleModel.from_config(sub.model)
+    t = time.perf_counter()
+    om.build_ld_table(sub.ldp(om.mu))
+    om.evaluate(sub.times, sub.lc_index, sub.passband_index, sub.supersampling,
+                sub.exposure_time, sub.pv, nthreads=nthreads)
+    dt = time.perf_counter() - t
+    return sub.evaluations / dt, dt
 
-    def run(n):
-        sub = wl.subset_pv(np.arange(n))
-        t = time.perf_counter()
-        om.build_ld_table(sub.ldp(om.mu))
-        om.evaluate(sub.times, sub.lc_index, sub.passband_index, sub.supersampling,
-                    sub.exposure_time, sub.pv, nthreads=nthreads)
-        return time.perf_counter() - t, sub.evaluations
 
+def oracle_stride_for(wl, nthreads: int, target_s: float) -> int:
+    """Stride of the pv sample so that one oracle pass takes about target_s (calibrated on a
+    handful of parameter vectors; strides are powers of two, 1 = the whole population)."""
     cores = os.cpu_count() or 1
-    n0 = min(wl.npv, max(1, cores))
-    dt, ev = run(n0)
-    n = int(min(wl.npv, max(n0, n0 * target_s / max(dt, 1e-6))))
-    if n > n0:
-        dt, ev = run(n)
-    return ev / dt, dt, n
+    n0 = min(wl.npv, max(1, cores if nthreads == 0 else 1))
+    rate, _ = oracle_run(wl.subset_pv(np.arange(0, wl.npv, max(1, wl.npv // n0))[:n0]), nthreads)
+    want = max(1.0, rate * target_s / max(1, wl.evaluations_per_pv))     # pvs in target_s
+    stride = 1
+    while wl.npv / stride > want and stride < wl.npv:
+        stride *= 2
+    return stride
+
+
+def cpu_baseline_of(wl, target_s: float = 10.0) -> dict:
+    """the oracle on the GPU box's host cores, 1 thread and all cores, on every
+    stride-th parameter vector (all exposures), extrapolation-free: evaluations of the sample / time."""
+    cores = os.cpu_count() or 1
+    s_all = oracle_stride_for(wl, 0, target_s)
+    s_one = oracle_stride_for(wl, 1, target_s)
+    sub_all, sub_one = oracle_sample(wl, s_all), oracle_sample(wl, s_one)
+    r_all, t_all = oracle_run(sub_all, 0)
+    r_one, t_one = oracle_run(sub_one, 1)
+    return {"value": r_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "all_cores": r_all, "one_thread": r_one, "cpu_model": cpu_model(),
+            "seconds": {"all_cores": t_all, "one_thread": t_one},
+            "sample": f"every {s_all}th parameter vector ({sub_all.npv} of {wl.npv}) x all {wl.npt} "
+                      f"exposures on {cores} threads (OpenMP over pv); one_thread: every {s_one}th "
+                      f"({sub_one.npv}); table build + evaluate"}
 
 
 def run_reference(args):
@@ -169,23 +227,25 @@ def run_reference(args):
     cores = os.cpu_count() or 1
     steps, warm = max(1, args.steps), max(0, args.warmup)
     target = min(10.0, 150.0 / (steps + warm))
+    stride = oracle_stride_for(wl, 0, target)
+    sub = oracle_sample(wl, stride)
     for _ in range(warm):
-        oracle_rate(wl, target)
-    t_total, ev_total, n_used = 0.0, 0, 0
+        oracle_run(sub, 0)
+    t_total = 0.0
     for _ in range(steps):
-        rate, dt, n = oracle_rate(wl, target)
+        _, dt = oracle_run(sub, 0)
         t_total += dt
-        ev_total += rate * dt
-        n_used = n
-    value = ev_total / t_total
-    sample = f"first {n_used} of {wl.npv} parameter vectors x all {wl.npt} exposures per step"
+    value = sub.evaluations * steps / t_total
+    sample = (f"every {stride}th parameter vector ({sub.npv} of {wl.npv}) x all {wl.npt} exposures; "
+              f"each of the {steps} steps re-runs this same sample (table build + evaluate, "
+              f"~{t_total / steps:.1f} s of oracle on {cores} threads)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": 1e3 * t_total / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": workload_config(wl, "fp64"),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": sample},
+                         "sample": sample, "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -194,6 +254,235 @@ def run_reference(args):
 
 
 # ---- our arm ----------------------------------------------------------------------------------------
+PRECISIONS = {"fp64": 0, "fp32": 1, "mixed": 2}
+DTYPE_NAME = {"fp64": "f64", "fp32": "f32", "mixed": "f32 (sum and flux f64)"}
+
+
+class Case:
+    """One workload in one precision, resident on the device: ctx, inputs, output buffers."""
+
+    def __init__(self, rr, wl, precision: str, table_mode: str, dev, ld_law=None):
+        import torch
+        self.rr, self.wl, self.precision, self.dev = rr, wl, precision, dev
+        code = PRECISIONS[precision]
+        self.npdt = np.float32 if code != rr.RR_FP64 else np.float64
+        self.model = rr.RoadRunner.from_config(wl.model, code)
+        self.ctx = self.model.ctx
+        rr.rr_set_table_mode(self.ctx, {"lazy": rr.RR_TABLE_LAZY, "full": rr.RR_TABLE_FULL,
+                                        "direct": rr.RR_TABLE_DIRECT}[table_mode])
+        self.model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
+                            wl.exposure_time)
+        self.ldp_h = np.ascontiguousarray(wl.ldp(self.model.mu), dtype=self.npdt)
+        self.ldp = torch.as_tensor(self.ldp_h).to(dev)
+        self.pv = torch.as_tensor(wl.pv).to(dev)
+        self.flux = torch.empty((wl.npv, wl.npt), dtype=self.model.flux_dtype, device=dev)
+        self.status = torch.empty(wl.npv, dtype=torch.int32, device=dev)
+        self.ld_law = ld_law
+        self.ldc = None
+        if ld_law is not None:
+            if wl.ld_kind != ld_law:
+                raise SystemExit(f"--ld-law {ld_law}: workload {wl.name} uses the {wl.ld_kind} law")
+            self.ldc = torch.as_tensor(np.ascontiguousarray(wl.ld_coeffs, np.float64)).to(dev)
+
+    def build_table(self):
+        if self.ldc is not None:
+            self.rr.rr_build_ld_table_law(self.ctx, self.ld_law, self.ldc, self.wl.npv)
+        else:
+            self.rr.rr_build_ld_table(self.ctx, self.ldp, self.wl.npv)
+
+    def step(self):
+        self.build_table()
+        self.rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
+
+    def timed(self, steps: int, warm: int, sync, sampler_rank0=None):
+        """W warm-up steps, then K steps between synchronisations: CUDA events around the steps and
+        the library's own events around its kernels.  Returns per-step times in ms."""
+        import torch
+        rr = self.rr
+        for _ in range(warm):
+            self.step()
+        torch.cuda.synchronize()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        launches0 = rr.rr_launch_count(self.ctx)
+        sampler = sampler_rank0() if sampler_rank0 else None
+        sync()
+        rr.rr_enable_kernel_timing(self.ctx, True)   # the library's own CUDA events around its kernels
+        for s in range(steps):
+            ev[s][0].record()
+            self.build_table()
+            ev[s][1].record()
+            rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
+            ev[s][2].record()
+        sync()
+        clocks = sampler.stop() if sampler else None
+        launches = rr.rr_launch_count(self.ctx) - launches0
+        kt = rr.rr_get_kernel_times(self.ctx)
+        rr.rr_enable_kernel_timing(self.ctx, False)
+        return {
+            "ms_total": ev[0][0].elapsed_time(ev[-1][2]),
+            "ms_table": float(np.mean([e[0].elapsed_time(e[1]) for e in ev])),
+            "ms_eval": float(np.mean([e[1].elapsed_time(e[2]) for e in ev])),
+            "ms_flux": kt["flux_ms"] / max(1, kt["calls"]),       # rr_flux_kernel alone
+            "ms_rows": kt["rows_ms"] / max(1, kt["calls"]),
+            "launches": int(launches), "clocks": clocks,
+        }
+
+    def class_counts(self):
+        """Class counts of one evaluation (untimed launch with the kernel's counters on)."""
+        rr = self.rr
+        rr.rr_enable_counters(self.ctx, True)
+        rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
+        counts = rr.rr_get_counters(self.ctx)
+        rr.rr_enable_counters(self.ctx, False)
+        return counts
+
+    def sample_error(self, n_pv=8, n_cols=600):
+        """Largest |flux - oracle| over sampled (pv, exposure) pairs of the flux now in self.flux:
+        n_pv parameter vectors x (n_cols random exposures + the 40 nearest to each one's t0).
+        With --ld-law the oracle takes the law's closed-form Istar as the library does (the
+        paper's "integrated analytically") instead of reading R6."""
+        import oracle
+        import torch
+        wl = self.wl
+        rng = np.random.default_rng(7)
+        pvs = np.sort(rng.choice(wl.npv, min(n_pv, wl.npv), replace=False))
+        cols = rng.choice(wl.npt, min(n_cols, wl.npt), replace=False)
+        t0 = wl.pv[pvs, wl.model.nkpb]
+        near = [np.argsort(np.abs(wl.times - t))[:40] for t in t0]
+        cols = np.unique(np.concatenate([cols] + near))
+        got = self.flux[torch.as_tensor(pvs, device=self.dev)][:, torch.as_tensor(cols, device=self.dev)]
+        got = got.cpu().numpy().astype(np.float64)
+        sub = wl.subset_pv(pvs).subset_times(cols)
+        if self.ld_law is None:
+            want, _ = oracle.evaluate_workload(sub, nthreads=0)
+        else:
+            from oracle import truth
+            om = oracle.OracleModel.from_config(sub.model)
+            ist = np.array([[truth.law(self.ld_law, c)[1] for c in row] for row in sub.ld_coeffs])
+            om.build_ld_table(sub.ldp(om.mu), istar_override=ist)
+            want, _ = om.evaluate(sub.times, sub.lc_index, sub.passband_index, sub.supersampling,
+                                  sub.exposure_time, sub.pv, nthreads=0)
+        ok = ~np.isnan(want)
+        return float(np.max(np.abs(got[ok] - want[ok]))), int(ok.sum()), int((want[ok] < 1).sum())
+
+    def close(self):
+        self.model.close()
+        self.ldp = self.pv = self.flux = self.status = self.ldc = None
+
+
+def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, clocks, peaks):
+    """algorithmic bytes and FMA-pipe instructions per launch of rr_flux_kernel against
+    the HBM and ALU peaks; the larger time bound names the binding roofline."""
+    code = PRECISIONS[precision]
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else \
+        "6650 GB/s (of fallback)"
+    es = 4 if code == rr.RR_FP32 else 8            # flux element
+    nrows = wl.npv * wl.model.npb
+    # algorithmic bytes per launch: flux written once, times read once, two table rows + Istar +
+    # the per-pv constants read once per (pv, passband)
+    alg_bytes = (wl.npv * wl.npt * es + wl.npt * 12 + nrows * (2 * wl.model.ng + 1) * es
+                 + wl.npv * 184)
+    t_flux = max(t["ms_flux"], 1e-6) * 1e-3
+    ops = dict(ALG_OPS["fp64" if precision == "fp64" else "fp32"])
+    if precision == "fp64":
+        # circular orbits: per exposure phase + sin/cos polynomials, per sub-sample one plane
+        # rotation + z^2 (DESIGN.md s7)
+        ops["circular"] = CIRC_PER_SUBSAMPLE + CIRC_PER_EXPOSURE * wl.npt / wl.evaluations_per_pv
+    alg_fma = (counts["skipped"] * ops["skipped"] + counts["circular"] * ops["circular"]
+               + counts["eccentric"] * ops["eccentric_fixed"]
+               + counts["solver_iters"] * ops["solver_iter"]
+               + counts["occulting"] * ops["occulting"] + counts["ingress"] * ops["ingress"])
+    lanes = FP32_LANES_PER_SM if code != rr.RR_FP64 else FP64_LANES_PER_SM
+    sm_max = (clocks or {}).get("sm_max_mhz") or float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak_tflops = 2.0 * lanes * SM_COUNT * sm_max * 1e6 / 1e12
+    hbm_achieved = alg_bytes / t_flux / 1e9
+    alu_achieved = 2.0 * alg_fma / t_flux / 1e12
+    t_hbm, t_alu = alg_bytes / (hbm_peak * 1e9), 2.0 * alg_fma / (alu_peak_tflops * 1e12)
+    if t_hbm >= t_alu:
+        roofline = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": hbm_achieved / hbm_peak, "traffic": None, "peak_source": hbm_src}
+    else:
+        roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak_tflops,
+                    "unit": "TFLOP/s", "frac": alu_achieved / alu_peak_tflops, "traffic": None,
+                    "peak_source": f"{lanes} FMA lanes/clk/SM x {SM_COUNT} SMs x {sm_max:.0f} MHz "
+                                   "x 2 (DESIGN.md s7)"}
+    cap = ncu_capture(wl.name, precision)
+    counter_based = None
+    if cap is not None:
+        roofline["traffic"] = int(cap["dram_read_bytes"]) + int(cap["dram_write_bytes"])
+        executed = int(cap["arith_thread_inst"])
+        # executed arithmetic thread-instructions of the committed capture (DFMA + DADD + DMUL, or
+        # FFMA + FADD + FMUL: a property of the build and the workload, not of the run) over the
+        # lanes x cycles of THIS run's kernel time: the counter-based pipe-feeding fraction
+        counter_based = {"arith_thread_inst_per_launch": executed,
+                         "frac": executed / (lanes * SM_COUNT * sm_max * 1e6 * t_flux),
+                         "algorithmic_over_executed": alg_fma / max(1, executed),
+                         "pipe_cycles_active_pct_ncu": float(cap["pipe_active_pct"]),
+                         "issue_active_pct_ncu": float(cap["issue_active_pct"]),
+                         "capture": cap["capture"]}
+    roofline.update({
+        "kernel": "rr_flux_kernel", "kernel_ms": t["ms_flux"],
+        "ld_table_kernel_ms": t["ms_table"] + t["ms_rows"],
+        "ld_table_parts_ms": {"rr_build_ld_table": t["ms_table"], "rows_in_rr_evaluate": t["ms_rows"]},
+        "rr_evaluate_ms": t["ms_eval"], "table_mode": table_mode,
+        "algorithmic_bytes": int(alg_bytes), "algorithmic_fma": int(alg_fma),
+        "algorithmic_ops_per_unit": ops,
+        "hbm_frac": hbm_achieved / hbm_peak, "alu_frac": alu_achieved / alu_peak_tflops,
+        "counter_based": counter_based,
+        "class_counts": counts,
+    })
+    return roofline
+
+
+def all_configs_report(rr, dev, peaks, args, headline):
+    """every BASELINE config and precision, a few steps each (after the headline
+    timing, rank 0 of a single-GPU run).  Config 0 is launch-latency-bound: microseconds per call, no
+    roofline claim."""
+    import torch
+    out = []
+    plan = [(0, "fp64"), (0, "fp32"), (1, "fp64"), (1, "fp32"), (2, "fp64"), (2, "fp32"),
+            (3, "fp64"), (3, "fp32"), (4, "fp64"), (4, "fp32"), (4, "mixed"), ("4b", "fp64"),
+            ("4b", "fp32")]
+    cache = {}
+    for config, precision in plan:
+        if (config, precision) == headline:
+            continue
+        if config not in cache:
+            cache.clear()
+            cache[config] = workloads.make_workload(config)
+        wl = cache[config]
+        case = Case(rr, wl, precision, "lazy", dev)
+        small = wl.evaluations < 10 ** 6
+        steps = 200 if small else (10 if wl.evaluations < 2 * 10 ** 9 else 5)
+        t = case.timed(steps, 3, torch.cuda.synchronize)
+        counts = case.class_counts()
+        err, n_s, n_in = case.sample_error()
+        value = wl.evaluations * steps / (t["ms_total"] * 1e-3)
+        entry = {"workload": wl.name, "precision": precision, "value": value, "unit": UNIT,
+                 "steps": steps, "ms_per_step": t["ms_total"] / steps, "flux_ms": t["ms_flux"],
+                 "table_ms": t["ms_table"] + t["ms_rows"],
+                 "max_abs_err_vs_oracle_sample": err, "sampled_points": n_s,
+                 "sampled_in_transit": n_in}
+        if small:
+            entry.update({"us_per_call": 1e3 * t["ms_total"] / steps, "bound": "launch latency",
+                          "frac": None})
+        else:
+            r = roofline_of(rr, wl, precision, t, counts, "lazy", headline_clocks(args), peaks)
+            entry.update({"bound": r["bound"], "frac": r["frac"], "hbm_frac": r["hbm_frac"],
+                          "alu_frac": r["alu_frac"], "traffic": r["traffic"],
+                          "counter_frac": (r["counter_based"] or {}).get("frac")})
+        out.append(entry)
+        case.close()
+        del case
+        torch.cuda.empty_cache()
+    return out
+
+
+def headline_clocks(args):
+    return getattr(args, "_clocks", None)
+
+
 def run_ours(args):
     import torch
     import paper_2009_08500_b200 as rr
@@ -208,80 +497,47 @@ def run_ours(args):
         shard.init_process_group("nccl")
     rr.load()
 
-    precision = {"fp64": rr.RR_FP64, "fp32": rr.RR_FP32, "mixed": rr.RR_MIXED}[args.precision]
-    npdt = np.float32 if precision != rr.RR_FP64 else np.float64
     wl = workloads.make_workload(args.config, npv=args.npv, npt=args.npt)
-    if rank:   # weak scaling: every rank gets a full population, rotated so that data differ
+    npv_job = wl.npv
+    if world > 1 and args.scaling == "strong":
+        b, e = shard.pv_slice(wl.npv, rank, world)      # ONE population, split over the ranks
+        wl = wl.subset_pv(np.arange(b, e))
+    elif rank:   # weak scaling: every rank gets a full population, rotated so that data differ
         sh = (rank * 97) % wl.npv
         wl.pv = np.ascontiguousarray(np.roll(wl.pv, sh, axis=0))
         wl.ld_coeffs = np.ascontiguousarray(np.roll(wl.ld_coeffs, sh, axis=0))
 
-    model = rr.RoadRunner.from_config(wl.model, precision)
-    rr.rr_set_table_mode(model.ctx, {"lazy": rr.RR_TABLE_LAZY, "full": rr.RR_TABLE_FULL,
-                                     "direct": rr.RR_TABLE_DIRECT}[args.table_mode])
-    model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling, wl.exposure_time)
-    ldp_h = np.ascontiguousarray(wl.ldp(model.mu), dtype=npdt)
-    ldp = torch.as_tensor(ldp_h).to(dev)
-    pv = torch.as_tensor(wl.pv).to(dev)
-    flux = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype, device=dev)
-    status = torch.empty(wl.npv, dtype=torch.int32, device=dev)
-    ctx = model.ctx
-    npv = wl.npv
-
-    def step():
-        rr.rr_build_ld_table(ctx, ldp, npv)
-        rr.rr_evaluate(ctx, pv, flux, status)
-
+    case = Case(rr, wl, args.precision, args.table_mode, dev, ld_law=args.ld_law)
+    ctx, model = case.ctx, case.model
     steps, warm = max(1, args.steps), max(3, args.warmup)
-    for _ in range(warm):
-        step()
-    torch.cuda.synchronize()
 
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
-    launches0 = rr.rr_launch_count(ctx)
-    sampler = ClockSampler(local_rank) if rank == 0 else None
-    shard.barrier()
-    torch.cuda.synchronize()
-    rr.rr_enable_kernel_timing(ctx, True)    # the library's own CUDA events around its kernels
-    for s in range(steps):
-        ev[s][0].record()
-        rr.rr_build_ld_table(ctx, ldp, npv)
-        ev[s][1].record()
-        rr.rr_evaluate(ctx, pv, flux, status)
-        ev[s][2].record()
-    torch.cuda.synchronize()
-    shard.barrier()
-    clocks = sampler.stop() if sampler else None
-    launches = rr.rr_launch_count(ctx) - launches0
-    ktimes = rr.rr_get_kernel_times(ctx)
-    rr.rr_enable_kernel_timing(ctx, False)
-    ms_total = ev[0][0].elapsed_time(ev[-1][2])
-    ms_table = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    ms_eval = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
-    ms_flux = ktimes["flux_ms"] / max(1, ktimes["calls"])      # rr_flux_kernel alone
-    ms_rows = ktimes["rows_ms"] / max(1, ktimes["calls"])
-    ms_total = shard.max_over_ranks(ms_total, dev)
+    def sync():
+        shard.barrier()
+        torch.cuda.synchronize()
+        shard.barrier()
+
+    t = case.timed(steps, warm, sync, (lambda: ClockSampler(local_rank)) if rank == 0 else None)
+    clocks = t["clocks"]
+    args._clocks = clocks
+    ms_total = shard.max_over_ranks(t["ms_total"], dev)
     evals_all = shard.sum_over_ranks(float(wl.evaluations), dev)
     value = evals_all * steps / (ms_total * 1e-3)
-
-    # ---- class counts of one evaluation (outside the timed region) -> algorithmic work
-    rr.rr_enable_counters(ctx, True)
-    rr.rr_evaluate(ctx, pv, flux, status)
-    counts = rr.rr_get_counters(ctx)
-    rr.rr_enable_counters(ctx, False)
-    n_bad = int((status != 0).sum().item())
+    counts = case.class_counts()
+    n_bad = int((case.status != 0).sum().item())
+    err_sample = case.sample_error() if rank == 0 else None
+    precision = PRECISIONS[args.precision]
 
     # ---- end to end: host buffers in, host flux out, copies inside the timed region
     e2e = None
     if not args.no_e2e:
         try:
             flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype, pin_memory=True)
-            ldp_h_t = torch.as_tensor(ldp_h).pin_memory()
+            ldp_h_t = torch.as_tensor(case.ldp_h).pin_memory()
             pv_h_t = torch.as_tensor(wl.pv).pin_memory()
             pinned = True
         except RuntimeError:
             flux_h_t = torch.empty((wl.npv, wl.npt), dtype=model.flux_dtype)
-            ldp_h_t, pv_h_t = torch.as_tensor(ldp_h), torch.as_tensor(wl.pv)
+            ldp_h_t, pv_h_t = torch.as_tensor(case.ldp_h), torch.as_tensor(wl.pv)
             pinned = False
         status_h = np.empty(wl.npv, np.int32)
         fh, lh, ph = flux_h_t.numpy(), ldp_h_t.numpy(), pv_h_t.numpy()
@@ -302,6 +558,8 @@ def run_ours(args):
                "call": "rr_evaluate_host (H2D ldp+pv, kernels 1-3, D2H flux+status, chunked on 2 streams)",
                "timer": "host perf_counter around the synchronous call (its copies and kernels "
                         "run on the library's own streams), max over ranks",
+               "bound": "PCIe: the flux matrix leaves the device once per step "
+                        f"({fh.nbytes / 1e9:.2f} GB D2H)",
                "flux_checksum": float(fh[::max(1, wl.npv // 64), ::997].astype(np.float64).sum())}
         del flux_h_t, fh
 
@@ -314,82 +572,51 @@ def run_ours(args):
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except (OSError, ValueError):
         pass
-    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else \
-        "6650 GB/s (of fallback)"
-    es = 4 if precision == rr.RR_FP32 else 8            # flux element
-    nrows = wl.npv * wl.model.npb
-    # algorithmic bytes per launch: flux written once, times read once, two table rows + Istar +
-    # the per-pv constants read once per (pv, passband)
-    alg_bytes = (wl.npv * wl.npt * es + wl.npt * 12 + nrows * (2 * wl.model.ng + 1) * es
-                 + wl.npv * 184)
-    t_flux = ms_flux * 1e-3
-    ops = dict(ALG_OPS["fp64" if args.precision == "fp64" else "fp32"])
-    if args.precision == "fp64":
-        # circular orbits: per exposure phase 4 + sin/cos polynomials 15, per sub-sample one plane
-        # rotation 4 + z^2 2
-        ops["circular"] = 6.0 + 19.0 * wl.npt / wl.evaluations_per_pv
-    alg_fma = (counts["skipped"] * ops["skipped"] + counts["circular"] * ops["circular"]
-               + counts["eccentric"] * ops["eccentric_fixed"]
-               + counts["solver_iters"] * ops["solver_iter"]
-               + counts["occulting"] * ops["occulting"] + counts["ingress"] * ops["ingress"])
-    lanes = FP32_LANES_PER_SM if precision != rr.RR_FP64 else FP64_LANES_PER_SM
-    sm_max = (clocks or {}).get("sm_max_mhz") or float(peaks.get("sm_max_mhz", 1965.0))
-    alu_peak_tflops = 2.0 * lanes * SM_COUNT * sm_max * 1e6 / 1e12
-    fma_live = rr.rr_measure_fma_peak(precision)
-    hbm_achieved = alg_bytes / t_flux / 1e9
-    alu_achieved = 2.0 * alg_fma / t_flux / 1e12
-    t_hbm, t_alu = alg_bytes / (hbm_peak * 1e9), 2.0 * alg_fma / (alu_peak_tflops * 1e12)
-    if t_hbm >= t_alu:
-        roofline = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": hbm_achieved / hbm_peak, "traffic": None, "peak_source": hbm_src}
-    else:
-        roofline = {"bound": "alu", "achieved": alu_achieved, "peak": alu_peak_tflops,
-                    "unit": "TFLOP/s", "frac": alu_achieved / alu_peak_tflops, "traffic": None,
-                    "peak_source": f"{lanes} FMA lanes/clk/SM x {SM_COUNT} SMs x {sm_max:.0f} MHz "
-                                   "x 2 (DESIGN.md s7)"}
-    roofline["traffic"] = ncu_traffic(wl.name, args.precision)
-    roofline.update({
-        "kernel": "rr_flux_kernel", "kernel_ms": ms_flux, "ld_table_kernel_ms": ms_table + ms_rows,
-        "ld_table_parts_ms": {"rr_build_ld_table": ms_table, "rows_in_rr_evaluate": ms_rows},
-        "rr_evaluate_ms": ms_eval, "table_mode": args.table_mode,
-        "algorithmic_bytes": int(alg_bytes), "algorithmic_fma": int(alg_fma),
-        "algorithmic_ops_per_unit": ops,
-        "hbm_frac": hbm_achieved / hbm_peak, "alu_frac": alu_achieved / alu_peak_tflops,
-        "fma_peak_measured_live_tflops": 2.0 * fma_live / 1e12,
-        "class_counts": counts,
-        "note": "kernel_ms = CUDA events recorded by the library around rr_flux_kernel on the "
-                "launching stream, inside the timed region, mean over the timed steps; frac = "
-                "achieved / peak; traffic: see profiles/",
-    })
+    roofline = roofline_of(rr, wl, args.precision, t, counts, args.table_mode, clocks, peaks)
+    roofline["fma_peak_measured_live_tflops"] = 2.0 * rr.rr_measure_fma_peak(precision) / 1e12
+    roofline["note"] = ("kernel_ms = CUDA events recorded by the library around rr_flux_kernel on the "
+                        "launching stream, inside the timed region, mean over the timed steps; frac = "
+                        "achieved / peak from the op table of DESIGN.md s7; counter_based.frac = the "
+                        "arithmetic thread-instructions ncu counted for this build and workload "
+                        "(profiles/flux_kernel_ncu.csv) over lanes x cycles of this run's kernel time")
+
+    es = 4 if precision == rr.RR_FP32 else 8
+    line_config = workload_config(wl, args.precision, {
+        "parallelism": f"pv-sharded x{world}, no collective"
+                       + (f" (strong: {npv_job} parameter vectors split)" if world > 1 and
+                          args.scaling == "strong" else ""),
+        "l2": "working set per step (flux + LD table) is far larger than the 126 MB L2; "
+              "no flush needed" if wl.npv * wl.npt * es > 2 ** 28 else
+              "working set fits L2: small config, latency-bound, no roofline claim",
+        "invalid_pv": n_bad,
+        "ld_table_call": "rr_build_ld_table_law" if args.ld_law else "rr_build_ld_table"})
+    case.close()
+    del case
+    torch.cuda.empty_cache()
+
+    all_configs = None
+    if world == 1 and not args.no_all_configs and args.npv is None and args.npt is None:
+        all_configs = all_configs_report(rr, dev, peaks, args, (args.config, args.precision))
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        rate, dt, n = oracle_rate(wl, 24.0)
-        cpu_baseline = {"value": rate, "unit": UNIT, "cores": os.cpu_count() or 1,
-                        "kind": "oracle", "seconds": dt,
-                        "sample": f"first {n} of {wl.npv} parameter vectors x all {wl.npt} "
-                                  f"exposures (table build + evaluate), OpenMP over pv"}
+        cpu_baseline = cpu_baseline_of(wl)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps,
         "warmup": warm, "ms_per_step": ms_total / steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None,
-        "dtype": {"fp64": "f64", "fp32": "f32", "mixed": "f32 (sum and flux f64)"}[args.precision],
-        "data": "synthetic",
-        "config": workload_config(wl, args.precision, {
-            "parallelism": f"pv-sharded x{world}, no collective",
-            "l2": "working set per step (flux + LD table) is far larger than the 126 MB L2; "
-                  "no flush needed" if wl.npv * wl.npt * es > 2 ** 28 else
-                  "working set fits L2: small config, latency-bound, no roofline claim",
-            "invalid_pv": n_bad}),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
+        "dtype": DTYPE_NAME[args.precision], "data": "synthetic",
+        "config": line_config,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": t["launches"], "roofline": roofline,
+        "max_abs_err_vs_oracle_sample": {"value": err_sample[0], "points": err_sample[1],
+                                         "in_transit": err_sample[2]},
         "cpu_baseline": cpu_baseline,
+        "all_configs": all_configs,
         "paper_context": "paper reports no absolute throughput; OpenCL fp32 GPU 10-20x over its "
                          "CPU code on unnamed hardware (PAPER.md:194)",
     }
     print(json.dumps(line))
-    model.close()
     return 0
 
 

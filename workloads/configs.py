@@ -23,6 +23,7 @@ CONFIG_NAMES = {
     3: "config3-heterogeneous",
     4: "config4-stress",
 }
+VARIANT_NAMES = {"4b": "config4b-literal-cadence"}
 
 
 @dataclass(frozen=True)
@@ -161,9 +162,21 @@ def _single_lc(npt, ns, exptime):
             np.array([exptime], np.float64))
 
 
-def make_workload(config: int, npv: int | None = None, npt: int | None = None) -> Workload:
+def make_workload(config, npv: int | None = None, npt: int | None = None) -> Workload:
     """Build config 0..4.  ``npv``/``npt`` shrink the population / time axis for parity tests
-    (same seed, same draw order: a smaller npv is a prefix of the full population)."""
+    (same seed, same draw order: a smaller npv is a prefix of the full population).
+
+    ``"4b"``: the labelled secondary workload of SURVEY 8(d): config 4's population with the
+    literal reading of "2-minute cadence spacing" - 10^5 exposures spaced 2 min apart (138.9 d
+    centred on t = 0) instead of 10^5 exposures over +-0.5 d.  More than 90 % of it is out of
+    transit: it isolates the window test and the flux = 1 fill path."""
+    if str(config) == "4b":
+        wl = make_workload(4, npv=npv, npt=npt)
+        n = wl.npt
+        times = (np.arange(n, dtype=np.float64) - 0.5 * (n - 1)) * (2.0 / 1440.0)
+        return replace(wl, name=VARIANT_NAMES["4b"], times=times,
+                       note="literal 2-minute spacing of the exposures")
+    config = int(config)
     rng = np.random.default_rng(SEED_BASE + config)
     name = CONFIG_NAMES[config]
     if config == 0:
