@@ -131,7 +131,7 @@ int rr_destroy(rr_ctx *ctx) {
   ctx->tev.clear();
   free_data(ctx);
   for (auto &w : ctx->work) free_work(&w);
-  void *bufs[] = {ctx->d_ze, ctx->d_zm, ctx->d_mu, ctx->d_q, ctx->d_W, ctx->d_tiles,
+  void *bufs[] = {ctx->d_ze, ctx->d_zm, ctx->d_mu, ctx->d_q, ctx->d_W, ctx->d_Wsup, ctx->d_tiles,
                   ctx->d_scratch, ctx->d_counters};
   for (void *b : bufs)
     if (b) cudaFree(b);

@@ -95,6 +95,7 @@ struct rr_ctx {
   int smem_abs;         // 1: the flux kernels may address shared memory absolutely (rr_smem_probe)
   // geometry (a0)
   double *d_ze, *d_zm, *d_mu, *d_q, *d_W;
+  void *d_Wsup;         // int2 [nk][ng]: non-zero range [jlo, jhi) of every weight row
   std::vector<double> h_ze, h_mu;
   // data (kernel 4)
   int64_t npt;

@@ -222,6 +222,24 @@ int rr_ld_rows_small_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t s
   return RR_OK;
 }
 
+// Support of every weight row W[ik][ig][.]: the planet at separation g (1+k) covers only the annuli
+// between c - k and c + k, so the row is zero outside [jlo, jhi).  The row builders of
+// kernel 1 skip the zeros (adding w = 0 terms changes no sum).
+__global__ void rr_support_kernel(const double *__restrict__ W, int nrows, int nz,
+                                  int2 *__restrict__ sup) {
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= nrows) return;
+  const double *w = W + (int64_t)r * nz;
+  int lo = nz, hi = 0;
+  for (int j = 0; j < nz; ++j)
+    if (w[j] != 0.0) {
+      lo = min(lo, j);
+      hi = j + 1;
+    }
+  if (lo >= hi) { lo = 0; hi = nz; }               // (cannot happen: the weights sum to 1)
+  sup[r] = make_int2(lo, hi);
+}
+
 int rr_geometry_build(rr_ctx *ctx) {
   const rr_config &c = ctx->cfg;
   int nz = ctx->nz;
@@ -236,6 +254,10 @@ int rr_geometry_build(rr_ctx *ctx) {
   RR_LAUNCH_CHECK(ctx);
   rr_weights_kernel<<<(unsigned)((nW + 255) / 256), 256>>>(c.nk, c.k0, c.k1, c.ng, nz, ctx->d_ze,
                                                            ctx->d_W);
+  RR_LAUNCH_CHECK(ctx);
+  RR_CUDA(cudaMalloc(&ctx->d_Wsup, sizeof(int2) * (size_t)c.nk * c.ng));
+  rr_support_kernel<<<(c.nk * c.ng + 127) / 128, 128>>>(ctx->d_W, c.nk * c.ng, nz,
+                                                        (int2 *)ctx->d_Wsup);
   RR_LAUNCH_CHECK(ctx);
   ctx->h_ze.resize(nz + 1);
   ctx->h_mu.resize(nz);

@@ -245,6 +245,9 @@ rr_ld_rows_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
 // W[ik], W[ik+1] are read once per RB profiles (warp-uniform loads served by L1) instead of once per
 // profile from L2 (2.6 GB of L2 reads at config 4 otherwise).  Lane = row, warp = g nodes.
 constexpr int RB = 32;
+#ifndef RR_ROWS_SMEM4_MAX
+#define RR_ROWS_SMEM4_MAX (110 * 1024)   // NG = 4 while two blocks still fit an SM
+#endif
 
 __device__ __forceinline__ int rr_row_ik(const RRPvBand *__restrict__ pvb, int64_t row, int npb,
                                          int nkpb) {
@@ -284,15 +287,22 @@ __global__ void rr_rows_scatter(const RRPvBand *__restrict__ pvb, int64_t M, int
   list[offs[ik] + atomicAdd(&cursor[ik], 1)] = (int)row;
 }
 
-template <typename TR>
+// Register tile: every warp takes NG g nodes (lane = row), so that one profile value feeds 2 NG FMAs,
+// and the weights are read as 16-byte broadcasts (two j per load) when nz is even: per pair of j,
+// 4 + 2 NG shared-memory wavefronts feed 4 NG FMAs (NG = 4: 0.75 per FMA; one lane = one row = one node
+// needed 2 per FMA and was bound by the LSU at 1/4 of the FP64 pipe).  The sums run over j in order:
+// bit-identical to the per-row builder.
+template <typename TR, int NG>
 __global__ void __launch_bounds__(256)
 rr_ld_rows_bucket_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
+                         const int2 *__restrict__ sup,
                          const RRPvBand *__restrict__ pvb, const int *__restrict__ list,
                          const int *__restrict__ offs, const int *__restrict__ tileoff, int nb,
                          TR *__restrict__ rows, int npb, int nkpb, int ng, int nz, int stride) {
-  extern __shared__ double prof[];                 // [RB][stride], stride odd: conflict-free
+  extern __shared__ __align__(16) double prof[];   // [RB][stride], stride odd: conflict-free
   __shared__ int rid[RB];
   __shared__ double akr[RB];
+  constexpr int CH = 8 * NG;                       // g nodes per chunk: 8 warps x NG
   const int b = blockIdx.x;
   if (b >= tileoff[nb]) return;
   int lo = 0, hi = nb - 1;                         // last bucket whose first tile is <= b
@@ -320,35 +330,84 @@ rr_ld_rows_bucket_kernel(const TR *__restrict__ ldp, const double *__restrict__ 
     const int r = idx / nz, j = idx - r * nz;
     prof[r * stride + j] = (r < nr) ? (double)ldp[(int64_t)rid[r] * nz + j] : 0.0;
   }
-  __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const double *W0 = W + (int64_t)ik * ng * nz;
   const double *W1 = W0 + (int64_t)ng * nz;
   const double *pr = prof + lane * stride;
   const double ak = akr[lane];
   const int64_t orow = (int64_t)rid[lane] * ng;
-  // The weight rows of 8 g nodes at a time go through shared memory: all 256 threads load them
-  // coalesced (deep memory-level parallelism; read straight from L2 one element per FMA they left
-  // the FMA chains waiting on 300-cycle loads), then every warp takes one node, lane = row.
-  double *wb0 = prof + RB * stride, *wb1 = wb0 + 8 * nz;
-  for (int c0 = 0; c0 < ng; c0 += 8) {
-    const int nrow = min(8, ng - c0);
-    __syncthreads();                               // the previous chunk is consumed
-    for (int idx = threadIdx.x; idx < nrow * nz; idx += 256) {
-      wb0[idx] = __ldg(W0 + (int64_t)c0 * nz + idx);
-      wb1[idx] = __ldg(W1 + (int64_t)c0 * nz + idx);
+  // The weight rows of CH g nodes at a time go through shared memory: all 256 threads load them
+  // coalesced (deep memory-level parallelism), then every warp takes NG nodes, lane = row.  Only the
+  // columns [ja, jb) in which some row of the chunk is non-zero are staged, and every warp sums over
+  // the support of its own NG nodes (rr_support_kernel): a planet covers 2k of the stellar radius.
+  __shared__ int jrange[2];
+  double *wb0 = prof + RB * stride;                // 16-byte aligned; wb1 follows at an even offset
+  const int2 *sup0 = sup + (int64_t)ik * ng, *sup1 = sup0 + ng;
+  for (int c0 = 0; c0 < ng; c0 += CH) {
+    const int nrow = min(CH, ng - c0);
+    __syncthreads();                               // the previous chunk is consumed (first: profiles written)
+    if (threadIdx.x == 0) { jrange[0] = nz; jrange[1] = 0; }
+    __syncthreads();
+    if ((int)threadIdx.x < 2 * nrow) {
+      const int2 r = threadIdx.x < nrow ? sup0[c0 + threadIdx.x] : sup1[c0 + threadIdx.x - nrow];
+      atomicMin(&jrange[0], r.x);
+      atomicMax(&jrange[1], r.y);
     }
     __syncthreads();
-    if (warp < nrow) {
-      const double *w0 = wb0 + warp * nz, *w1 = wb1 + warp * nz;
-      double s0 = 0.0, s1 = 0.0;
-#pragma unroll 4
-      for (int j = 0; j < nz; ++j) {
-        const double p = pr[j];
-        s0 = fma(w0[j], p, s0);                    // warp-uniform shared loads: broadcasts
-        s1 = fma(w1[j], p, s1);
+    const int ja = jrange[0] & ~1, jb = min(nz, (jrange[1] + 1) & ~1);
+    const int len = jb - ja, lenp = (len + 1) & ~1;  // row pitch in shared memory, even
+    double *wb1 = wb0 + CH * lenp;
+    for (int idx = threadIdx.x; idx < nrow * len; idx += 256) {
+      const int q = idx / len, j = idx - q * len;
+      wb0[q * lenp + j] = __ldg(W0 + (int64_t)(c0 + q) * nz + ja + j);
+      wb1[q * lenp + j] = __ldg(W1 + (int64_t)(c0 + q) * nz + ja + j);
+    }
+    __syncthreads();
+    const int g0 = warp * NG;
+    if (g0 < nrow) {
+      // support of this warp's nodes (both k rows), inside [ja, jb)
+      int jl = nz, jh = 0;
+#pragma unroll
+      for (int q = 0; q < NG; ++q)
+        if (g0 + q < nrow) {
+          const int2 a = sup0[c0 + g0 + q], c = sup1[c0 + g0 + q];
+          jl = min(jl, min(a.x, c.x));
+          jh = max(jh, max(a.y, c.y));
+        }
+      const double *w0 = wb0 + g0 * lenp - ja, *w1 = wb1 + g0 * lenp - ja;   // indexed by j
+      double s0[NG], s1[NG];
+#pragma unroll
+      for (int q = 0; q < NG; ++q) s0[q] = s1[q] = 0.0;
+      if ((nz & 1) == 0) {                         // ja, lenp even: 16-byte aligned pairs
+        jl &= ~1;                                  // stays >= ja (even)
+        jh = min(jb, (jh + 1) & ~1);
+#pragma unroll 2
+        for (int j = jl; j < jh; j += 2) {
+          const double p0 = pr[j], p1 = pr[j + 1];
+#pragma unroll
+          for (int q = 0; q < NG; ++q) {           // nodes past nrow read stale weights; never stored
+            const double2 a = *reinterpret_cast<const double2 *>(w0 + q * lenp + j);
+            const double2 c = *reinterpret_cast<const double2 *>(w1 + q * lenp + j);
+            s0[q] = fma(a.y, p1, fma(a.x, p0, s0[q]));
+            s1[q] = fma(c.y, p1, fma(c.x, p0, s1[q]));
+          }
+        }
+      } else {
+#pragma unroll 2
+        for (int j = jl; j < jh; ++j) {
+          const double p = pr[j];
+#pragma unroll
+          for (int q = 0; q < NG; ++q) {
+            s0[q] = fma(w0[q * lenp + j], p, s0[q]);
+            s1[q] = fma(w1[q * lenp + j], p, s1[q]);
+          }
+        }
       }
-      if (lane < nr) rows[orow + c0 + warp] = (TR)fma(ak, s1 - s0, s0);
+      if (lane < nr) {
+#pragma unroll
+        for (int q = 0; q < NG; ++q)
+          if (g0 + q < nrow) rows[orow + c0 + g0 + q] = (TR)fma(ak, s1[q] - s0[q], s0[q]);
+      }
     }
   }
 }
@@ -460,8 +519,12 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
   if (wk->lazy == 2) return rr_ld_rows_direct_launch(ctx, wk, npv, st);
   const int nb = c.nk - 1;                         // buckets: lower k row ik in [0, nk-2]
   const int stride = ctx->nz | 1;
-  const size_t smem_b = sizeof(double) * (RB * stride + 16 * ctx->nz);   // profiles + 2 x 8 weight rows
-  if (M >= 2048 && nb <= 4096 && smem_b <= 96 * 1024) {
+  // profiles + 2 x (8 NG) weight rows; NG = 4 when that leaves two blocks per SM, else 2
+  const size_t smem4 = sizeof(double) * (RB * stride + 2 * 32 * ctx->nz);
+  const size_t smem2 = sizeof(double) * (RB * stride + 2 * 16 * ctx->nz);
+  const int NGsel = smem4 <= RR_ROWS_SMEM4_MAX ? 4 : 2;
+  const size_t smem_b = NGsel == 4 ? smem4 : smem2;
+  if (M >= 2048 && nb <= 4096 && smem_b <= 200 * 1024) {
     // bucketed builder
     const int64_t need = sizeof(int32_t) * (4 * (int64_t)nb + 4 + M);
     rc = grow_buf((void **)&wk->bk, &wk->bk_cap, need);
@@ -477,21 +540,22 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
     rr_rows_scatter<<<gb, 256, 0, st>>>(wk->pvb, M, c.npb, c.nkpb, offs, cursor, list);
     RR_LAUNCH_CHECK(ctx);
     const unsigned tiles_max = (unsigned)((M + RB - 1) / RB + nb);
+#define RR_BUCKET_LAUNCH(TR, NG)                                                                   \
+    do {                                                                                           \
+      if (smem_b > 48 * 1024)                                                                      \
+        RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<TR, NG>,                             \
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));   \
+      rr_ld_rows_bucket_kernel<TR, NG><<<tiles_max, 256, smem_b, st>>>(                            \
+          (const TR *)wk->ldp_src, ctx->d_W, (const int2 *)ctx->d_Wsup, wk->pvb, list, offs,      \
+          tileoff, nb, (TR *)wk->rows,                                                            \
+          c.npb, c.nkpb, c.ng, ctx->nz, stride);                                                   \
+    } while (0)
     if (c.precision != RR_FP64) {
-      if (smem_b > 48 * 1024)
-        RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<float>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
-      rr_ld_rows_bucket_kernel<float><<<tiles_max, 256, smem_b, st>>>(
-          (const float *)wk->ldp_src, ctx->d_W, wk->pvb, list, offs, tileoff, nb, (float *)wk->rows,
-          c.npb, c.nkpb, c.ng, ctx->nz, stride);
+      if (NGsel == 4) RR_BUCKET_LAUNCH(float, 4); else RR_BUCKET_LAUNCH(float, 2);
     } else {
-      if (smem_b > 48 * 1024)
-        RR_CUDA(cudaFuncSetAttribute(rr_ld_rows_bucket_kernel<double>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
-      rr_ld_rows_bucket_kernel<double><<<tiles_max, 256, smem_b, st>>>(
-          (const double *)wk->ldp_src, ctx->d_W, wk->pvb, list, offs, tileoff, nb,
-          (double *)wk->rows, c.npb, c.nkpb, c.ng, ctx->nz, stride);
+      if (NGsel == 4) RR_BUCKET_LAUNCH(double, 4); else RR_BUCKET_LAUNCH(double, 2);
     }
+#undef RR_BUCKET_LAUNCH
     RR_LAUNCH_CHECK(ctx);
     return RR_OK;
   }
