@@ -48,7 +48,8 @@ constexpr int FT = RR_FLUX_THREADS;   // threads per flux block
 #define RR_ROBUST_INLINE __forceinline__   // measured: 2 % faster than a call (fewer spills)
 #endif
 #ifndef RR_FLUX_WAVES
-#define RR_FLUX_WAVES 64        // waves of blocks wanted before the tile axis is left uncut
+#define RR_FLUX_WAVES 128       // waves of blocks wanted before the tile axis is left uncut (128 beats
+                                // 64 by 0.5 % and 256 by 1 %: tail against per-block set-up)
 #endif
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
@@ -483,8 +484,8 @@ __device__ __forceinline__ R rr_separation2(const Cst<R, M> K, double ur, bool &
 // one extra cell (node ldw[ng-1], slope 0), so that y = ng-1 (z = 1+k to rounding) needs no clamp
 // (reading R10: the same value as cell ng-2 with ag = 1).
 __device__ __forceinline__ void rr_cell(double y, int &ig, double &ag) {
-  ig = __double2int_rd(y);                   // conversion unit, not the FP64 pipe
-  ag = y - __int2double_rn(ig);
+  ig = __double2int_rd(y);                   // conversion unit, not the FP64 pipe; the index and the
+  ag = y - floor(y);                         // weight do not wait for each other
 }
 __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
   ig = (int)y;
@@ -492,7 +493,7 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
 }
 
 template <typename R, int M>
-__device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) {
+__device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, bool ksmall) {
   // the constants first: their shared-memory latency passes under the square root
   R gscale, opk, omk2, afull;
   K.template pair<K_GSCALE>(gscale, opk);
@@ -516,15 +517,14 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress) 
     // the half-angle formulas of the triangle: both arguments are >= 0 (no sign cases), th1/2 <=
     // asin(k)/2 needs no octant reduction for k^2 <= 1/2 and th2/2 in [0, pi/2] needs one of three
     // cases.  ap = th1 + k^2 th2 - kite/2.
-    R omks, k2;
-    K.template pair<K_OMKS>(omks, k2);
+    const R omks = K.template get<K_OMKS>();
     const R A = opk - z, B = z + omks, C = z - omks, D = z + opk;
     const R AB = fabs(A * B), S = fabs(C * D), Q = B * D;
     const R kite = rr_sqrt3_pos(AB * S);
     const R tk2 = K.template get<K_2K2>();
     // (the k^2 > 1/2 case is a path of its own so that the common one is a single basic block:
     // the two arctangents are independent and interleave)
-    if (k2 <= (R)0.5) {
+    if (ksmall) {                           // k^2 <= 1/2, decided once per tile
       const R h1 = rr_atan_t(rr_div3(kite, Q));
       const R h2 = rr_atan_quadrant<R>(kite, S, AB);
       ap = fma(h1, (R)2, fma(tk2, h2, (R)-0.5 * kite));
@@ -593,7 +593,7 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
 template <typename R, bool COUNT, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_mid, double hwid,
-                                          bool need_front, unsigned long long *cnt) {
+                                          bool need_front, bool ksmall, unsigned long long *cnt) {
   // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
   const double wr = NOWRAP ? w : w - rr_round(w);
   R def = (R)0;
@@ -606,7 +606,7 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
     bool occ = z2 < K.template get<K_OPK2>();
     if (need_front) occ = occ && front;
     if (occ) {
-      def = rr_deficit<R, M>(K, z2, ing);
+      def = rr_deficit<R, M>(K, z2, ing, ksmall);
       if (COUNT) { cnt[3]++; cnt[4] += ing; }
     }
     if (COUNT) { cnt[CIRC ? 1 : 2]++; cnt[5] += it; }
@@ -627,6 +627,8 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double du = 2.0 * hw / ns;                   // sub-sample spacing, turns
   const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
   const double hskip = hwid + hw;
+  // k^2 <= 1/2 (block-uniform; lane-0 broadcast so that it stays a predicate, not a compare per use)
+  const bool ksmall = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5), 0) != 0;
   if (!shuffle) {
     // ---- one thread per exposure, in-thread loop over its sub-samples ----
     // The time and flux pointers advance by opaque 64-bit adds: otherwise the compiler, short of
@@ -684,7 +686,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
             sn = s1;
             if (occ) {
               int ing = 0;
-              acc += rr_deficit<R, M>(K, z2, ing);
+              acc += rr_deficit<R, M>(K, z2, ing, ksmall);
               if (COUNT) { cnt[3]++; cnt[4] += ing; }
             }
           }
@@ -692,7 +694,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, need_front, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, need_front, ksmall, cnt);
         }
         // mean of (Istar - ip ap)/Istar over ns; fp64 staged the table already times 1/(Istar ns)
         f = sizeof(R) == 8 ? (O)1 - acc : fma(-acc, scale, (O)1);
@@ -717,7 +719,8 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         if (fabs(wr) <= hskip) {
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
-            acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, true, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, true,
+                                                          ksmall, cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
         }
@@ -1082,11 +1085,12 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   else P.shuffle_min_ns = (npv * ctx->npt < 2 * resident) ? 4 : 0x7fffffff;
   if (ctx->ntiles <= 0 || npv <= 0) return RR_OK;
   // Blocks: one per (pv, chunk of consecutive tiles).  One chunk per pv when the population alone
-  // gives every SM several waves of blocks (table row and constants staged once per pv);
-  // otherwise the tile axis is cut so that about 8 waves of blocks exist.
+  // gives every SM RR_FLUX_WAVES waves of blocks (table row and constants staged once per pv);
+  // otherwise the tile axis is cut so that about that many waves exist.
   const int64_t want = (int64_t)ctx->sm_count * RR_FLUX_MIN_BLOCKS * RR_FLUX_WAVES;
   int64_t nchunks = (want + npv - 1) / npv;
-  nchunks = std::max<int64_t>(1, std::min<int64_t>(nchunks, ctx->ntiles));
+  // (at least two tiles per block: with one, the per-block set-up shows - config 2 3.5 % slower)
+  nchunks = std::max<int64_t>(1, std::min<int64_t>(nchunks, std::max<int64_t>(1, ctx->ntiles / 2)));
   const int64_t chunk_len = (ctx->ntiles + nchunks - 1) / nchunks;
   nchunks = (ctx->ntiles + chunk_len - 1) / chunk_len;
   if (npv * nchunks > 0x7fffffffLL) return RR_ESIZE;

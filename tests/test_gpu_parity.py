@@ -528,7 +528,7 @@ def test_orbit_high_eccentricity_full_phase(rr):
 
 # ---- kernel 4: dispatch -----------------------------------------------------------------------------------
 def expected_tiles(lc_index, supersampling):
-    """Runs of equal lc_index cut into tiles of 512*R exposures, R = clamp((8+ns//2)//ns, 1, 8)."""
+    """Runs of equal lc_index cut into tiles of 1024*R exposures, R = clamp((8+ns//2)//ns, 1, 8)."""
     tiles = []
     n = len(lc_index)
     b = 0
@@ -537,7 +537,7 @@ def expected_tiles(lc_index, supersampling):
         while e < n and lc_index[e] == lc_index[b]:
             e += 1
         ns = int(supersampling[lc_index[b]])
-        length = 512 * max(1, min(8, (8 + ns // 2) // ns))
+        length = 1024 * max(1, min(8, (8 + ns // 2) // ns))
         for s in range(b, e, length):
             tiles.append((s, min(length, e - s), int(lc_index[b])))
         b = e
