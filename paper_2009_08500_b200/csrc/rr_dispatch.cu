@@ -6,13 +6,13 @@
 // comparable work.  Each tile also gets its [tmin, tmax] time range (lets the flux kernel fill a
 // whole out-of-transit tile without evaluating it) and the offset of its first sub-sample.
 //
-//   1. rr_k4_segments   heads of runs of equal lc_index (any order of light curves is allowed;
+//   1. rr_k4_heads_*    heads of runs of equal lc_index (any order of light curves is allowed;
 //                       a light curve may come in several runs), range check of lc_index
 //   2. rr_k4_tilecount  tiles per run, exclusive scan -> first tile of every run
 //   3. rr_k4_tiles      one thread per tile: binary search of its run, start/count/lc
 //   4. rr_k4_ranges     one warp per tile: min/max time; then scan of count*ns -> sub_off
-// The scans run in a single block (chunked, carry in shared memory): rr_set_data is called once per
-// data set, not per evaluation.
+// The scans over runs and tiles (few) run in a single block (chunked, carry in shared memory); the
+// walk over the exposures uses the whole GPU.
 #include "rr_common.cuh"
 
 namespace {
@@ -46,33 +46,59 @@ __device__ int64_t block_inclusive_scan(int64_t v, int64_t *warp_sums, int64_t *
   return v;
 }
 
-// 1. run heads -> seg_start[nseg]; out[0] = nseg, out[1] = error flag.
+// 1. run heads -> seg_start[nseg]; out[0] = nseg, out[1] = error flag.  Three launches so that the
+// exposure axis is walked by the whole GPU (one block walked it alone in round 1: 0.10 ms at 10^5
+// exposures, 1 ms at 10^6, per rr_set_data and so per rr_evaluate_flat):
+//   1a. one block per SCAN_T exposures: number of run heads in the block, range check of lc_index
+//   1b. one block: exclusive scan of the per-block counts
+//   1c. one block per SCAN_T exposures: scan inside the block, scatter of the run heads
+__device__ __forceinline__ int rr_k4_is_head(const int32_t *__restrict__ lc, int64_t i, int64_t npt,
+                                             int32_t nlc, int *bad) {
+  if (i >= npt) return 0;
+  const int32_t l = lc[i];
+  if (l < 0 || l >= nlc) *bad = 1;
+  return (i == 0 || lc[i - 1] != l) ? 1 : 0;
+}
+
 __global__ void __launch_bounds__(SCAN_T)
-rr_k4_segments(const int32_t *__restrict__ lc, int64_t npt, int32_t nlc,
-               int64_t *__restrict__ seg_start, int64_t *__restrict__ out) {
+rr_k4_heads_count(const int32_t *__restrict__ lc, int64_t npt, int32_t nlc,
+                  int64_t *__restrict__ blk_count, int64_t *__restrict__ out) {
+  int bad = 0;
+  const int head = rr_k4_is_head(lc, (int64_t)blockIdx.x * SCAN_T + threadIdx.x, npt, nlc, &bad);
+  const int n = __syncthreads_count(head);
+  const int anybad = __syncthreads_or(bad);
+  if (threadIdx.x == 0) {
+    blk_count[blockIdx.x] = n;
+    if (anybad) out[1] = 1;                        // (out[0..3] were zeroed by the launcher)
+  }
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+rr_k4_heads_scan(int64_t nblk, const int64_t *__restrict__ blk_count, int64_t *__restrict__ blk_off,
+                 int64_t *__restrict__ out) {
   __shared__ int64_t ws[32];
-  __shared__ int bad;
-  if (threadIdx.x == 0) bad = 0;
-  __syncthreads();
   int64_t carry = 0;
-  for (int64_t base = 0; base < npt; base += SCAN_T) {
-    int64_t i = base + threadIdx.x;
-    int64_t head = 0;
-    if (i < npt) {
-      int32_t l = lc[i];
-      if (l < 0 || l >= nlc) bad = 1;
-      head = (i == 0 || lc[i - 1] != l) ? 1 : 0;
-    }
+  for (int64_t base = 0; base < nblk; base += SCAN_T) {
+    const int64_t b = base + threadIdx.x;
+    const int64_t n = b < nblk ? blk_count[b] : 0;
     int64_t tot;
-    int64_t inc = block_inclusive_scan(head, ws, &tot);
-    if (head) seg_start[carry + inc - 1] = i;
+    const int64_t inc = block_inclusive_scan(n, ws, &tot);
+    if (b < nblk) blk_off[b] = carry + inc - n;
     carry += tot;
   }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    out[0] = carry;
-    out[1] = bad;
-  }
+  if (threadIdx.x == 0) out[0] = carry;
+}
+
+__global__ void __launch_bounds__(SCAN_T)
+rr_k4_heads_scatter(const int32_t *__restrict__ lc, int64_t npt, int32_t nlc,
+                    const int64_t *__restrict__ blk_off, int64_t *__restrict__ seg_start) {
+  __shared__ int64_t ws[32];
+  int bad = 0;
+  const int64_t i = (int64_t)blockIdx.x * SCAN_T + threadIdx.x;
+  const int64_t head = rr_k4_is_head(lc, i, npt, nlc, &bad);
+  int64_t tot;
+  const int64_t inc = block_inclusive_scan(head, ws, &tot);
+  if (head) seg_start[blk_off[blockIdx.x] + inc - 1] = i;
 }
 
 // 2. tiles per run and their exclusive scan; out[2] = ntiles.
@@ -173,8 +199,9 @@ rr_k4_suboff(int64_t ntiles, RRTile *__restrict__ tiles, int64_t *__restrict__ o
 // Needs ctx->d_times, d_lc_index, d_lc, npt, nlc set.  Synchronous on st.
 int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st) {
   int64_t npt = ctx->npt;
-  // scratch: seg_start[npt] | tile_off[npt] | out[4]
-  int64_t need = 2 * npt + 4;
+  // scratch: seg_start[npt] | tile_off[npt] | out[4] | blk_count[nblk] | blk_off[nblk]
+  const int64_t nblk = (npt + SCAN_T - 1) / SCAN_T;
+  int64_t need = 2 * npt + 4 + 2 * nblk;
   if (need > ctx->scratch_cap) {
     if (ctx->d_scratch) cudaFree(ctx->d_scratch);
     ctx->d_scratch = nullptr;
@@ -183,7 +210,14 @@ int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st) {
     ctx->scratch_cap = need;
   }
   int64_t *seg_start = ctx->d_scratch, *tile_off = seg_start + npt, *out = tile_off + npt;
-  rr_k4_segments<<<1, SCAN_T, 0, st>>>(ctx->d_lc_index, npt, ctx->nlc, seg_start, out);
+  int64_t *blk_count = out + 4, *blk_off = blk_count + nblk;
+  RR_CUDA(cudaMemsetAsync(out, 0, sizeof(int64_t) * 4, st));
+  rr_k4_heads_count<<<(unsigned)nblk, SCAN_T, 0, st>>>(ctx->d_lc_index, npt, ctx->nlc, blk_count, out);
+  RR_LAUNCH_CHECK(ctx);
+  rr_k4_heads_scan<<<1, SCAN_T, 0, st>>>(nblk, blk_count, blk_off, out);
+  RR_LAUNCH_CHECK(ctx);
+  rr_k4_heads_scatter<<<(unsigned)nblk, SCAN_T, 0, st>>>(ctx->d_lc_index, npt, ctx->nlc, blk_off,
+                                                         seg_start);
   RR_LAUNCH_CHECK(ctx);
   int64_t h[4] = {0, 0, 0, 0};
   RR_CUDA(cudaMemcpyAsync(h, out, sizeof(int64_t) * 2, cudaMemcpyDeviceToHost, st));

@@ -1128,3 +1128,37 @@ def test_device_math_against_multiprecision(rr, fp32):
     yv, yvd = dev(np.concatenate([rng.uniform(0, 5000, n), [0.0, 98.99999999999999, 99.0, 4999.5]]))
     ig, ag = run("cell", yvd)
     assert np.array_equal(ig, np.floor(yv)) and np.array_equal(ag, yv - np.floor(yv))
+
+
+def test_dispatch_million_exposures(rr):
+    """Kernel 4 on 1.2e6 exposures in 4000 runs of random lengths (the run heads are found by many
+    blocks: their per-block counts, a scan, a scatter): bit-exact against the restatement."""
+    rng = np.random.default_rng(17)
+    nlc = 5
+    cuts = np.sort(rng.choice(np.arange(1, 1_200_000), 3999, replace=False))
+    lens = np.diff(np.concatenate([[0], cuts, [1_200_000]]))
+    ids = rng.integers(0, nlc, lens.size)
+    ids[1:][ids[1:] == ids[:-1]] = (ids[:-1][ids[1:] == ids[:-1]] + 1) % nlc   # neighbours differ
+    lc = np.repeat(ids, lens).astype(np.int32)
+    times = rng.uniform(-10, 10, lc.size)
+    ns = [1, 3, 7, 30, 2]
+    gm = rr.RoadRunner(npb=2)
+    gm.set_data(times, lc, [0, 1, 0, 1, 0], ns, [0.0, 0.01, 0.02, 0.03, 0.001])
+    got = rr.rr_get_tiles(gm.ctx)
+    want = expected_tiles(lc, ns)
+    assert rr.rr_num_tiles(gm.ctx) == len(want)
+    assert np.array_equal(got["start"], [w[0] for w in want])
+    assert np.array_equal(got["count"], [w[1] for w in want])
+    assert np.array_equal(got["lc"], [w[2] for w in want])
+    for j in rng.choice(len(want), 200, replace=False):
+        s0, c, _ = want[j]
+        assert got["tmin"][j] == times[s0:s0 + c].min() and got["tmax"][j] == times[s0:s0 + c].max()
+    assert rr.rr_num_subsamples(gm.ctx) == int(np.asarray(ns)[lc].sum())
+    bad = lc.copy()
+    bad[777_777] = nlc
+    import torch
+    with pytest.raises(rr.RoadRunnerError) as e:
+        rr.rr_set_data(gm.ctx, torch.as_tensor(times).cuda(), torch.as_tensor(bad).cuda(),
+                       [0, 1, 0, 1, 0], ns, [0.0] * 5)
+    assert e.value.code == -4
+    gm.close()
