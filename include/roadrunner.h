@@ -128,7 +128,8 @@ int rr_get_weights(const rr_ctx *ctx, double *h_W /*[nk][ng][nz]*/);
  *                       t + tau*((s+1/2)/n - 1/2)                               (reading R7)
  * The library copies all five and runs the heterogeneous-dispatch kernels (DESIGN.md section 6,
  * kernel 4), which cut the exposure axis into tiles of one light curve each (uniform ns, tau,
- * passband; 1024 R exposures, R = clamp((8 + ns/2)/ns, 1, 8)) with their time range.  Synchronous on `stream` (it reads back the tile count).
+ * passband; at most 1024 R exposures, R = clamp((8 + ns/2)/ns, 1, 8), and at most 0.1 d at the
+ * run's mean cadence, in multiples of 128) with their time range.  Synchronous on `stream` (it reads back the tile count).
  * RR_EINDEX if any index is out of range (nothing is kept then).                                */
 int rr_set_data(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_index, int64_t npt,
                 const int32_t *h_passband_index, const int32_t *h_supersampling,

@@ -101,9 +101,31 @@ rr_k4_heads_scatter(const int32_t *__restrict__ lc, int64_t npt, int32_t nlc,
   if (head) seg_start[blk_off[blockIdx.x] + inc - 1] = i;
 }
 
+// Tile length of a run of exposures [b, e) of one light curve: at most the light curve's tile_len
+// (RR_TILE_UNIT x R exposures, set from ns so that a tile carries ~4096 sub-samples), and no longer
+// than RR_TILE_SPAN days at the run's mean cadence |t[e-1] - t[b]| / (e-b-1), in multiples of 128
+// exposures (one pass of a flux block), at least 128.  A transit lasts hours: with sparse cadences
+// (10^5 exposures two minutes apart) a 3072-exposure tile spans four days, always holds a transit and
+// is never skipped; 0.1-day tiles are.  Times in any order are allowed: the span of an unsorted run is
+// meaningless, which costs speed, not correctness.
+#ifndef RR_TILE_SPAN
+#define RR_TILE_SPAN 0.1
+#endif
+__device__ __forceinline__ int64_t rr_k4_run_tile_len(const double *__restrict__ times, int64_t b,
+                                                      int64_t e, int64_t max_len) {
+  if (e - b < 2) return max_len;
+  const double span = fabs(times[e - 1] - times[b]);
+  const double q = RR_TILE_SPAN / span;                       // IEEE division, then one product:
+  const double n = (double)(e - b - 1) * q;                   // the tests restate these two roundings
+  if (!(n < (double)max_len)) return max_len;                 // also span = 0, NaN, infinite
+  const int64_t len = (((int64_t)n + 127) / 128) * 128;
+  return len < 128 ? 128 : (len > max_len ? max_len : len);
+}
+
 // 2. tiles per run and their exclusive scan; out[2] = ntiles.
 __global__ void __launch_bounds__(SCAN_T)
-rr_k4_tilecount(const int32_t *__restrict__ lc, int64_t npt, const RRLc *__restrict__ lcs,
+rr_k4_tilecount(const int32_t *__restrict__ lc, const double *__restrict__ times, int64_t npt,
+                const RRLc *__restrict__ lcs,
                 const int64_t *__restrict__ seg_start, int64_t *__restrict__ tile_off,
                 int64_t *__restrict__ out) {
   __shared__ int64_t ws[32];
@@ -114,7 +136,7 @@ rr_k4_tilecount(const int32_t *__restrict__ lc, int64_t npt, const RRLc *__restr
     int64_t nt = 0;
     if (s < nseg) {
       int64_t b = seg_start[s], e = (s + 1 < nseg) ? seg_start[s + 1] : npt;
-      int64_t len = lcs[lc[b]].tile_len;
+      int64_t len = rr_k4_run_tile_len(times, b, e, lcs[lc[b]].tile_len);
       nt = (e - b + len - 1) / len;
     }
     int64_t tot;
@@ -126,8 +148,8 @@ rr_k4_tilecount(const int32_t *__restrict__ lc, int64_t npt, const RRLc *__restr
 }
 
 // 3. one thread per tile.
-__global__ void rr_k4_tiles(const int32_t *__restrict__ lc, int64_t npt,
-                            const RRLc *__restrict__ lcs, const int64_t *__restrict__ seg_start,
+__global__ void rr_k4_tiles(const int32_t *__restrict__ lc, const double *__restrict__ times,
+                            int64_t npt, const RRLc *__restrict__ lcs, const int64_t *__restrict__ seg_start,
                             const int64_t *__restrict__ tile_off, int64_t nseg, int64_t ntiles,
                             RRTile *__restrict__ tiles) {
   int64_t tl = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -139,7 +161,7 @@ __global__ void rr_k4_tiles(const int32_t *__restrict__ lc, int64_t npt,
   }
   int64_t b = seg_start[lo], e = (lo + 1 < nseg) ? seg_start[lo + 1] : npt;
   int32_t l = lc[b];
-  int64_t len = lcs[l].tile_len;
+  int64_t len = rr_k4_run_tile_len(times, b, e, lcs[l].tile_len);
   int64_t start = b + (tl - tile_off[lo]) * len;
   int64_t count = e - start < len ? e - start : len;
   RRTile r;
@@ -224,7 +246,8 @@ int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st) {
   RR_CUDA(cudaStreamSynchronize(st));
   if (h[1]) return RR_EINDEX;
   int64_t nseg = h[0];
-  rr_k4_tilecount<<<1, SCAN_T, 0, st>>>(ctx->d_lc_index, npt, ctx->d_lc, seg_start, tile_off, out);
+  rr_k4_tilecount<<<1, SCAN_T, 0, st>>>(ctx->d_lc_index, ctx->d_times, npt, ctx->d_lc, seg_start,
+                                        tile_off, out);
   RR_LAUNCH_CHECK(ctx);
   RR_CUDA(cudaMemcpyAsync(h, out, sizeof(int64_t) * 3, cudaMemcpyDeviceToHost, st));
   RR_CUDA(cudaStreamSynchronize(st));
@@ -237,7 +260,7 @@ int rr_dispatch_build(rr_ctx *ctx, cudaStream_t st) {
     ctx->tiles_cap = ntiles;
   }
   rr_k4_tiles<<<(unsigned)((ntiles + 255) / 256), 256, 0, st>>>(
-      ctx->d_lc_index, npt, ctx->d_lc, seg_start, tile_off, nseg, ntiles, ctx->d_tiles);
+      ctx->d_lc_index, ctx->d_times, npt, ctx->d_lc, seg_start, tile_off, nseg, ntiles, ctx->d_tiles);
   RR_LAUNCH_CHECK(ctx);
   rr_k4_ranges<<<(unsigned)((ntiles * 32 + 255) / 256), 256, 0, st>>>(ctx->d_times, ntiles,
                                                                       ctx->d_tiles);

@@ -48,8 +48,9 @@ constexpr int FT = RR_FLUX_THREADS;   // threads per flux block
 #define RR_ROBUST_INLINE __forceinline__   // measured: 2 % faster than a call (fewer spills)
 #endif
 #ifndef RR_FLUX_WAVES
-#define RR_FLUX_WAVES 128       // waves of blocks wanted before the tile axis is left uncut (128 beats
-                                // 64 by 0.5 % and 256 by 1 %: tail against per-block set-up)
+#define RR_FLUX_WAVES 64        // waves of blocks wanted before the tile axis is left uncut (with the
+                                // bulk fill: config 4 64 = 128 waves, config 3 0.7 % slower, the sparse
+                                // cadence of 4b 14 % faster than with 128: per-block set-up)
 #endif
 
 // ---- per-pv prep ---------------------------------------------------------------------------------
@@ -557,6 +558,7 @@ struct FluxParams {
   int shuffle_min_ns;   // light curves with ns >= this use the lanes-over-sub-samples layout
   int ldw_len;          // staged row length: ng + 1, or more with mean-k weights, where g of a
                         // passband with k > kw passes the last node (reading R13): limb value
+  unsigned ones_off;    // byte offset in rr_dyn of the block's buffer of ones (bulk fill)
   unsigned nchunks;     // blocks per parameter vector
   unsigned chunk_len;   // dispatch tiles per block
 };
@@ -587,6 +589,45 @@ __device__ __forceinline__ void rr_fill(R *out, int64_t count, R val) {
   }
   const int64_t done = head + nvec * VN;
   if ((int64_t)threadIdx.x < count - done) out[done + threadIdx.x] = val;
+}
+
+// Out-of-window runs (flux = 1) written by the TMA engine: a block keeps RR_ONES_BYTES of ones in
+// shared memory and ONE thread issues bulk copies shared -> global (cp.async.bulk, <= RR_ONES_BYTES
+// each) for the 16-byte-aligned body of the run; head and tail elements go out as plain stores.  The
+// other threads go straight on to the next in-window tile: the fill costs the SM one instruction per
+// 8 kB instead of a 16-byte store per thread (config 4 writes 10.9 of its 13.1 GB this way).
+#ifndef RR_ONES_BYTES
+#define RR_ONES_BYTES 8192
+#endif
+#ifndef RR_BULK_FILL
+#define RR_BULK_FILL 1
+#endif
+// Block-uniform call: writes the ones and makes them visible to the async proxy.
+template <typename O>
+__device__ __forceinline__ void rr_ones_setup(unsigned char *ones_p) {
+  for (int i = threadIdx.x; i < RR_ONES_BYTES / (int)sizeof(O); i += FT)
+    reinterpret_cast<O *>(ones_p)[i] = (O)1;
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncthreads();
+}
+template <typename O>
+__device__ __forceinline__ void rr_fill_ones_bulk(O *out, int64_t count, unsigned ones_smem) {
+  const uintptr_t addr = reinterpret_cast<uintptr_t>(out);
+  int64_t head = (int64_t)(((16 - (addr & 15)) & 15) / sizeof(O));
+  if (head > count) head = count;
+  if ((int64_t)threadIdx.x < head) out[threadIdx.x] = (O)1;
+  const int64_t body = ((count - head) * (int64_t)sizeof(O)) & ~(int64_t)15;      // bytes
+  if (threadIdx.x == 0 && body > 0) {
+    const char *dst = reinterpret_cast<const char *>(out + head);
+    for (int64_t off = 0; off < body; off += RR_ONES_BYTES) {
+      const unsigned n = (unsigned)min((int64_t)RR_ONES_BYTES, body - off);
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                   :: "l"(dst + off), "r"(ones_smem), "r"(n) : "memory");
+    }
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+  }
+  const int64_t done = head + body / (int64_t)sizeof(O);
+  if ((int64_t)threadIdx.x < count - done) out[done + threadIdx.x] = (O)1;
 }
 
 // Occulted light of the sub-sample at phase w (turns, measured from the window centre).
@@ -747,6 +788,12 @@ rr_flux_kernel(const FluxParams P) {
   unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
+#if RR_BULK_FILL
+  // ones for the bulk fill, after the staged row (16-byte aligned); written at the block's first fill
+  unsigned char *ones_p = rr_dyn + P.ones_off;
+  const unsigned ones_smem = (unsigned)__cvta_generic_to_shared(ones_p);
+  bool ones_ready = false;
+#endif
   const unsigned v = blockIdx.x / P.nchunks;
   const unsigned chunk = blockIdx.x - v * P.nchunks;
   const int64_t tl0 = (int64_t)chunk * P.chunk_len;
@@ -801,7 +848,12 @@ rr_flux_kernel(const FluxParams P) {
       if (q >= ngrp) break;
       pos = q + 1;
       if (f0 >= 0) {
+#if RR_BULK_FILL
+        if (!ones_ready) { rr_ones_setup<O>(ones_p); ones_ready = true; }
+        rr_fill_ones_bulk<O>(row + f0, f1 - f0, ones_smem);
+#else
         rr_fill<O>(row + f0, f1 - f0, (O)1);
+#endif
         f0 = -1;
       }
       const RRTile *tp = P.tiles + base + q;
@@ -869,7 +921,16 @@ rr_flux_kernel(const FluxParams P) {
                                            inv_p, u_mid, hwid, hw, scale, K, cnt);
     }
   }
+#if RR_BULK_FILL
+  if (f0 >= 0) {
+    if (!ones_ready) { rr_ones_setup<O>(ones_p); ones_ready = true; }
+    rr_fill_ones_bulk<O>(row + f0, f1 - f0, ones_smem);
+  }
+  // the bulk copies read the block's shared memory: it must outlive them
+  if (ones_ready && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+#else
   if (f0 >= 0) rr_fill<O>(row + f0, f1 - f0, (O)1);
+#endif
   if (COUNT) {
 #pragma unroll
     for (int q = 0; q < 6; ++q) {
@@ -1097,7 +1158,12 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  const size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8) + 16;
+  size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8) + 16;
+  smem = (smem + 15) & ~(size_t)15;
+  P.ones_off = (unsigned)smem;
+#if RR_BULK_FILL
+  smem += RR_ONES_BYTES;
+#endif
   if (ctx->counters_on)
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
   using Kernel = void (*)(const FluxParams);

@@ -527,8 +527,13 @@ def test_orbit_high_eccentricity_full_phase(rr):
 
 
 # ---- kernel 4: dispatch -----------------------------------------------------------------------------------
-def expected_tiles(lc_index, supersampling):
-    """Runs of equal lc_index cut into tiles of 1024*R exposures, R = clamp((8+ns//2)//ns, 1, 8)."""
+TILE_UNIT, TILE_SPAN = 1024, 0.1
+
+
+def expected_tiles(lc_index, supersampling, times):
+    """Runs of equal lc_index cut into tiles: at most TILE_UNIT*R exposures, R = clamp((8+ns//2)//ns,
+    1, 8), and no longer than TILE_SPAN days at the run's mean cadence, in multiples of 128 (>= 128);
+    the two floating-point roundings are those of rr_k4_run_tile_len."""
     tiles = []
     n = len(lc_index)
     b = 0
@@ -537,14 +542,21 @@ def expected_tiles(lc_index, supersampling):
         while e < n and lc_index[e] == lc_index[b]:
             e += 1
         ns = int(supersampling[lc_index[b]])
-        length = 1024 * max(1, min(8, (8 + ns // 2) // ns))
+        max_len = TILE_UNIT * max(1, min(8, (8 + ns // 2) // ns))
+        length = max_len
+        if e - b >= 2:
+            with np.errstate(divide="ignore", invalid="ignore"):
+                span = np.abs(np.float64(times[e - 1]) - np.float64(times[b]))
+                cnt = np.float64(e - b - 1) * (np.float64(TILE_SPAN) / span)
+            if cnt < max_len:
+                length = min(max(128, (int(cnt) + 127) // 128 * 128), max_len)
         for s in range(b, e, length):
             tiles.append((s, min(length, e - s), int(lc_index[b])))
         b = e
     return tiles
 
 
-@pytest.mark.parametrize("case", ["config3", "interleaved", "single", "paper"])
+@pytest.mark.parametrize("case", ["config3", "interleaved", "single", "paper", "sparse"])
 def test_dispatch_tiles(rr, case):
     rng = np.random.default_rng(11)
     if case == "config3":
@@ -557,6 +569,10 @@ def test_dispatch_tiles(rr, case):
         lc[1000:3500] = 2
         times = rng.uniform(-1, 1, lc.size)
         pb, ns, et, npb = [0, 1, 0], [1, 7, 30], [0.0, 0.01, 0.02], 2
+    elif case == "sparse":                     # 2-minute cadence over 28 d: 128-exposure tiles
+        lc = np.repeat(np.array([0, 1], np.int32), [20000, 777])
+        times = np.concatenate([np.arange(20000) * (2.0 / 1440.0), 5.0 + np.arange(777) * 0.02])
+        pb, ns, et, npb = [0, 0], [3, 10], [2.0 / 1440.0, 0.02], 1
     elif case == "single":
         lc = np.zeros(1, np.int32)
         times = np.array([0.25])
@@ -568,7 +584,7 @@ def test_dispatch_tiles(rr, case):
     gm = rr.RoadRunner(npb=npb)
     gm.set_data(times, lc, pb, ns, et)
     got = rr.rr_get_tiles(gm.ctx)
-    want = expected_tiles(lc, ns)
+    want = expected_tiles(lc, ns, times)
     assert rr.rr_num_tiles(gm.ctx) == len(want)
     assert [(int(s), int(c), int(l)) for s, c, l in zip(got["start"], got["count"], got["lc"])] \
         == want
@@ -1145,7 +1161,7 @@ def test_dispatch_million_exposures(rr):
     gm = rr.RoadRunner(npb=2)
     gm.set_data(times, lc, [0, 1, 0, 1, 0], ns, [0.0, 0.01, 0.02, 0.03, 0.001])
     got = rr.rr_get_tiles(gm.ctx)
-    want = expected_tiles(lc, ns)
+    want = expected_tiles(lc, ns, times)
     assert rr.rr_num_tiles(gm.ctx) == len(want)
     assert np.array_equal(got["start"], [w[0] for w in want])
     assert np.array_equal(got["count"], [w[1] for w in want])
