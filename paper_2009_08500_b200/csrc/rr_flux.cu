@@ -619,10 +619,14 @@ __device__ __forceinline__ void rr_fill_ones_bulk(O *out, int64_t count, unsigne
   const int64_t body = ((count - head) * (int64_t)sizeof(O)) & ~(int64_t)15;      // bytes
   if (threadIdx.x == 0 && body > 0) {
     const char *dst = reinterpret_cast<const char *>(out + head);
+    // flux is never re-read: evict-first in L2, so that W, the times and the rows stay (config 4
+    // 0.8 %, config 4b 4 % faster than with the default policy)
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     for (int64_t off = 0; off < body; off += RR_ONES_BYTES) {
       const unsigned n = (unsigned)min((int64_t)RR_ONES_BYTES, body - off);
-      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                   :: "l"(dst + off), "r"(ones_smem), "r"(n) : "memory");
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+                   :: "l"(dst + off), "r"(ones_smem), "r"(n), "l"(pol) : "memory");
     }
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
   }
