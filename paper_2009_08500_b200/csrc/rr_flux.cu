@@ -661,6 +661,18 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
   return def;
 }
 
+// Mid-exposure time through the read-only path (global address space known, L1-cacheable: every pv
+// block on the SM reads the same times).
+__device__ __forceinline__ double rr_ld_time(uintptr_t p) {
+#ifdef RR_TIME_GENERIC
+  return *reinterpret_cast<const double *>(p);
+#else
+  double t;
+  asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(t) : "l"(p));
+  return t;
+#endif
+}
+
 // The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
 // R = arithmetic type of z and ip*ap; O = type of the sub-sample sum, the final 1 - sum/(Istar ns)
 // and the stored flux (O = double with R = float is RR_MIXED, the scheme of PAPER.md:293).
@@ -682,7 +694,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
     uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
     uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
     int left = count - (int)threadIdx.x;             // exposures of this thread still to do, x FT
-    double tnext = left > 0 ? *reinterpret_cast<const double *>(tp) : 0.0;
+    double tnext = left > 0 ? rr_ld_time(tp) : 0.0;
     // circular: the in-front test is only needed when the evaluated phases can reach a quarter turn
     // (lane-0 broadcast: opaque, or the compiler recomputes the fp64 test in the inner loop)
     const bool need_front =
@@ -691,7 +703,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
       const double tcur = tnext;
       left -= FT;
       asm volatile("add.u64 %0, %0, %1;" : "+l"(tp) : "n"(FT * 8));
-      if (left > 0) tnext = *reinterpret_cast<const double *>(tp);   // in flight during this exposure
+      if (left > 0) tnext = rr_ld_time(tp);            // in flight during this exposure
       const double wc = fma(tcur - t0, inv_p, -u_mid);
       const double wr = wc - rr_round(wc);           // exposure centre from the window centre
       O f;
