@@ -330,6 +330,26 @@ class Case:
             "launches": int(launches), "clocks": clocks,
         }
 
+    def graph_us_per_step(self, n=300):
+        """One step captured into a CUDA graph and replayed (the step allocates and synchronises
+        nothing in steady state): microseconds per replay."""
+        import torch
+        side, graph = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            self.step()
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph, stream=side):
+                self.step()
+        for _ in range(10):
+            graph.replay()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return 1e3 * e0.elapsed_time(e1) / n
+
     def class_counts(self):
         """Class counts of one evaluation (untimed launch with the kernel's counters on)."""
         rr = self.rr
@@ -469,7 +489,7 @@ def all_configs_report(rr, dev, peaks, args, headline):
                  "sampled_in_transit": n_in}
         if small:
             entry.update({"us_per_call": 1e3 * t["ms_total"] / steps, "bound": "launch latency",
-                          "frac": None})
+                          "frac": None, "us_per_call_cuda_graph": case.graph_us_per_step()})
         else:
             r = roofline_of(rr, wl, precision, t, counts, "lazy", headline_clocks(args), peaks)
             entry.update({"bound": r["bound"], "frac": r["frac"], "hbm_frac": r["hbm_frac"],

@@ -124,6 +124,26 @@ __global__ void rr_istar_kernel(const TA *__restrict__ A, const double *__restri
   if (lane == 0) out[row] = (TC)s;
 }
 
+// Lazy mode: Istar and the ctx-owned copy of the profile in ONE launch (a copy engine call and a
+// kernel were two: small problems are bound by the length of the launch chain).  One warp per row.
+template <typename T>
+__global__ void rr_istar_copy_kernel(const T *__restrict__ A, const double *__restrict__ q,
+                                     const T *__restrict__ given, T *__restrict__ out,
+                                     T *__restrict__ copy, int64_t M, int K) {
+  int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  int lane = threadIdx.x & 31;
+  if (row >= M) return;
+  double s = 0.0;
+  for (int j = lane; j < K; j += 32) {
+    const T a = A[row * K + j];
+    copy[row * K + j] = a;
+    s = fma(q[j], (double)a, s);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if (lane == 0) out[row] = given ? given[row] : (T)s;
+}
+
 // ---- named limb-darkening laws on the device --------------------
 // ldp[row][j] = I(mu_j; ldc[row]) and the analytic disc integral Istar = 2 pi int_0^1 mu I dmu
 // ("all integrated analytically over the stellar disk").  The paper names the laws
@@ -484,14 +504,19 @@ int rr_ld_profile_launch(rr_ctx *ctx, RRWork *wk, const void *d_ldp, const void 
   int rc = grow_buf(&wk->istar, &wk->istar_cap, needI);
   if (rc == RR_OK && copy) rc = grow_buf(&wk->ldp, &wk->ldp_cap, needP);
   if (rc != RR_OK) return rc;
-  if (copy) {
-    RR_CUDA(cudaMemcpyAsync(wk->ldp, d_ldp, (size_t)needP, cudaMemcpyDeviceToDevice, st));
-    wk->ldp_src = wk->ldp;
-  } else {
-    wk->ldp_src = d_ldp;
-  }
+  wk->ldp_src = copy ? wk->ldp : d_ldp;
   const int64_t threads = M * 32;
-  if (d_istar == wk->istar) {
+  if (copy && d_ldp != wk->ldp) {
+    if (c.precision != RR_FP64)
+      rr_istar_copy_kernel<float><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+          (const float *)d_ldp, ctx->d_q, (const float *)d_istar, (float *)wk->istar,
+          (float *)wk->ldp, M, ctx->nz);
+    else
+      rr_istar_copy_kernel<double><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(
+          (const double *)d_ldp, ctx->d_q, (const double *)d_istar, (double *)wk->istar,
+          (double *)wk->ldp, M, ctx->nz);
+    RR_LAUNCH_CHECK(ctx);
+  } else if (d_istar == wk->istar) {
     // already in place (named law with a closed form)
   } else if (c.precision != RR_FP64) {
     rr_istar_kernel<float, float><<<(unsigned)((threads + 255) / 256), 256, 0, st>>>(

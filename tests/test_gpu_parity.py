@@ -1178,3 +1178,43 @@ def test_dispatch_million_exposures(rr):
                        [0, 1, 0, 1, 0], ns, [0.0] * 5)
     assert e.value.code == -4
     gm.close()
+
+
+def test_step_is_cuda_graph_capturable(rr):
+    """rr_build_ld_table + rr_evaluate make no allocation, host round trip or synchronisation in steady
+    state (buffers grow only when a larger npv arrives), so a step can be captured into a CUDA graph
+    and replayed: same flux, also after the inputs changed in place."""
+    import torch
+    wl = small_workload(3)
+    gm = gpu_model(rr, wl)
+    ldp = torch.as_tensor(wl.ldp(gm.mu)).cuda()
+    pv = torch.as_tensor(wl.pv).cuda()
+    flux = torch.empty((wl.npv, wl.npt), dtype=torch.float64, device="cuda")
+    status = torch.empty(wl.npv, dtype=torch.int32, device="cuda")
+
+    def step():
+        rr.rr_build_ld_table(gm.ctx, ldp, wl.npv)
+        rr.rr_evaluate(gm.ctx, pv, flux, status)
+
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        step()                                   # warm-up: every buffer has its size
+        torch.cuda.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+    want, _ = oracle_flux(wl)
+    flux.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.max(np.abs(flux.cpu().numpy() - want)) <= TOL64
+    pv2 = wl.pv.copy()
+    pv2[:, 0] = np.clip(pv2[:, 0] * 1.07, 0.02, 0.2)          # new radius ratios, same buffers
+    pv.copy_(torch.as_tensor(pv2))
+    graph.replay()
+    torch.cuda.synchronize()
+    wl.pv = pv2
+    want2, _ = oracle_flux(wl)
+    assert np.max(np.abs(flux.cpu().numpy() - want2)) <= TOL64
+    assert np.max(np.abs(want2 - want)) > 1e-5
+    gm.close()
