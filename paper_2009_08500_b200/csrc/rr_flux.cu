@@ -238,7 +238,7 @@ template <> struct Vec2T<double> { using type = double2; };
 template <> struct Vec2T<float> { using type = float2; };
 
 // Shared memory of the flux and orbit kernels (all dynamic, the kernels have no static shared
-// memory): cst[K_SMEM] | tile flags (16 B) | ldw2[ldw_len] (node, slope) pairs.
+// memory): cst[K_SMEM] (8-byte slots) | tile flags (16 B) | ldw2[ldw_len] (node, slope) pairs.
 // How the loads are addressed (template parameter M of Cst):
 //   RR_SM_SYMBOL  by the PTX symbol rr_dyn + immediate: ptxas derives the shared-window base where it
 //                 needs it (S2UR + ULEA, or S2R + LEA inside loops: 3-5 instructions per use site)
@@ -259,9 +259,14 @@ enum { RR_SM_SYMBOL = 0, RR_SM_HELD = 1, RR_SM_ABS = 2 };
 #ifndef RR_SM_FALLBACK_F32
 #define RR_SM_FALLBACK_F32 RR_SM_HELD
 #endif
+// Every constant has an 8-byte slot in both precisions: a double, or - fp32 kernels - the float twice,
+// so that one 8-byte load gives the packed (c, c) operand of the two-exposures-per-thread FFMA2 path
+// and the scalar fp32 paths read its first half.
 template <typename R, int M> struct Cst {
   static constexpr int ES = (int)sizeof(R);
-  static constexpr int OFF_FLAGS = K_SMEM * ES, OFF_ROW = OFF_FLAGS + 16;
+  static constexpr int CS = 8;                       // bytes per constant slot
+  static constexpr int OFF_FLAGS = K_SMEM * CS, OFF_ROW = OFF_FLAGS + 16;
+  static constexpr int AB = (M == RR_SM_ABS ? RR_SMEM_ABS : 0);
   unsigned sb;   // RR_SM_HELD: shared-window address of rr_dyn; RR_SM_ABS: 0
   __device__ __forceinline__ Cst() {
     if constexpr (M == RR_SM_HELD) {
@@ -272,7 +277,10 @@ template <typename R, int M> struct Cst {
         if ((unsigned)__cvta_generic_to_shared(rr_dyn) != RR_SMEM_ABS) __trap();
     }
   }
-  static __device__ __forceinline__ R *base() { return reinterpret_cast<R *>(rr_dyn); }
+  static __device__ __forceinline__ void store(int slot, double v) {
+    if constexpr (ES == 8) reinterpret_cast<double *>(rr_dyn)[slot] = v;
+    else reinterpret_cast<float2 *>(rr_dyn)[slot] = make_float2((float)v, (float)v);
+  }
   static __device__ __forceinline__ unsigned *flags() {
     return reinterpret_cast<unsigned *>(rr_dyn + OFF_FLAGS);
   }
@@ -280,34 +288,52 @@ template <typename R, int M> struct Cst {
     R v;
     if constexpr (M == RR_SM_SYMBOL) {
       if constexpr (ES == 8)
-        asm volatile("ld.volatile.shared.f64 %0, [rr_dyn+%1];" : "=d"(v) : "n"(8 * I));
+        asm volatile("ld.volatile.shared.f64 %0, [rr_dyn+%1];" : "=d"(v) : "n"(CS * I));
       else
-        asm volatile("ld.volatile.shared.f32 %0, [rr_dyn+%1];" : "=f"(v) : "n"(4 * I));
+        asm volatile("ld.volatile.shared.f32 %0, [rr_dyn+%1];" : "=f"(v) : "n"(CS * I));
     } else {
-      constexpr int off = (M == RR_SM_ABS ? RR_SMEM_ABS : 0) + ES * I;
       if constexpr (ES == 8)
-        asm volatile("ld.volatile.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(sb), "n"(off));
+        asm volatile("ld.volatile.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(sb), "n"(AB + CS * I));
       else
-        asm volatile("ld.volatile.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(sb), "n"(off));
+        asm volatile("ld.volatile.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(sb), "n"(AB + CS * I));
     }
     return v;
   }
-  // two neighbouring constants (I even) with one 16-/8-byte shared load
+  // two neighbouring constants (I even) with one 16-byte shared load
   template <int I> __device__ __forceinline__ void pair(double &a, double &b) const {
     static_assert(I % 2 == 0, "pair");
     if constexpr (M == RR_SM_SYMBOL)
-      asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [rr_dyn+%2];" : "=d"(a), "=d"(b) : "n"(8 * I));
+      asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [rr_dyn+%2];" : "=d"(a), "=d"(b) : "n"(CS * I));
     else
       asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b)
-                   : "r"(sb), "n"((M == RR_SM_ABS ? RR_SMEM_ABS : 0) + 8 * I));
+                   : "r"(sb), "n"(AB + CS * I));
   }
-  template <int I> __device__ __forceinline__ void pair(float &a, float &b) const {
+  // fp32: the same load, as packed pairs (c, c) ...
+  template <int I> __device__ __forceinline__ void pair2(float2 &a, float2 &b) const {
     static_assert(I % 2 == 0, "pair");
+    unsigned long long u, w;
     if constexpr (M == RR_SM_SYMBOL)
-      asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [rr_dyn+%2];" : "=f"(a), "=f"(b) : "n"(4 * I));
+      asm volatile("ld.volatile.shared.v2.b64 {%0, %1}, [rr_dyn+%2];" : "=l"(u), "=l"(w) : "n"(CS * I));
     else
-      asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2+%3];" : "=f"(a), "=f"(b)
-                   : "r"(sb), "n"((M == RR_SM_ABS ? RR_SMEM_ABS : 0) + 4 * I));
+      asm volatile("ld.volatile.shared.v2.b64 {%0, %1}, [%2+%3];" : "=l"(u), "=l"(w)
+                   : "r"(sb), "n"(AB + CS * I));
+    a = make_float2(__uint_as_float((unsigned)u), __uint_as_float((unsigned)(u >> 32)));
+    b = make_float2(__uint_as_float((unsigned)w), __uint_as_float((unsigned)(w >> 32)));
+  }
+  template <int I> __device__ __forceinline__ float2 get2() const {
+    unsigned long long u;
+    if constexpr (M == RR_SM_SYMBOL)
+      asm volatile("ld.volatile.shared.b64 %0, [rr_dyn+%1];" : "=l"(u) : "n"(CS * I));
+    else
+      asm volatile("ld.volatile.shared.b64 %0, [%1+%2];" : "=l"(u) : "r"(sb), "n"(AB + CS * I));
+    return make_float2(__uint_as_float((unsigned)u), __uint_as_float((unsigned)(u >> 32)));
+  }
+  // ... or as scalars (first halves)
+  template <int I> __device__ __forceinline__ void pair(float &a, float &b) const {
+    float2 x, y;
+    pair2<I>(x, y);
+    a = x.x;
+    b = y.x;
   }
   // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
   using R2 = typename Vec2T<R>::type;
@@ -319,7 +345,7 @@ template <typename R, int M> struct Cst {
       sl = v.y;
     } else {
       const unsigned a = sb + (unsigned)(2 * ES) * (unsigned)ig;
-      constexpr int off = (M == RR_SM_ABS ? RR_SMEM_ABS : 0) + OFF_ROW;
+      constexpr int off = AB + OFF_ROW;
       if constexpr (ES == 8)
         asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(l0), "=d"(sl) : "r"(a), "n"(off));
       else
@@ -367,7 +393,7 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
     case K_2K2: v = 2.0 * b.k2; break;
     default: break;
   }
-  if (t < K_COUNT) reinterpret_cast<R *>(rr_dyn)[t] = (R)v;
+  if (t < K_COUNT) Cst<R, RR_SM_SYMBOL>::store(t, v);
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
@@ -683,10 +709,197 @@ __device__ __forceinline__ double rr_ld_time(uintptr_t p) {
 #endif
 }
 
+// ---- fp32 kernels: two exposures per thread, packed FFMA2 arithmetic ---------------------------------
+// (ax, ay): the element is inside the transit window at this sub-sample.  An inactive element is
+// given the phase 0, computes along and is masked out; nothing here can fault on its values.
+#ifndef RR_FP32_PAIRS
+#define RR_FP32_PAIRS 1
+#endif
+// The phases come as dM = 2 pi ur already in fp32 (rr_tile_pairs: one fp64 phase per exposure, an fp32
+// step per sub-sample when the exposure cannot wrap; else rounded from the fp64 phase each time).
+template <bool CIRC, int M>
+__device__ __forceinline__ F2 rr_separation2_pair(const Cst<float, M> K, F2 dM, bool ax, bool ay,
+                                                  bool &fx, bool &fy) {
+  if (CIRC) {
+    F2 s;
+    const F2 am = abs2(dM);
+    if (am.x <= 0.4995f && am.y <= 0.4995f) {
+      F2 cm1, sres;
+      rr_sincosm1_small2(dM, s, cm1, sres);
+    } else {
+      s = make_float2(sinf(dM.x), sinf(dM.y));
+    }
+    fx = am.x < 1.5707963f;
+    fy = am.y < 1.5707963f;
+    F2 zc0, zc1;
+    K.template pair2<K_ZC0>(zc0, zc1);
+    return fma2(mul2(s, s), zc1, zc0);
+  }
+  F2 s2 = f2(0.0f), cm2 = f2(0.0f);
+  bool okx = !ax, oky = !ay;
+  {
+    F2 c4, c3, c2, ky, B, C, A, tol;
+    K.template pair2<K_C4>(c4, c3);
+    K.template pair2<K_C2>(c2, ky);
+    const F2 y = mul2(dM, mul2(ky, f2(0.15915494309189535f)));           // dM / A (K_KY = 2 pi / A)
+    F2 d = mul2(y, fma2(y, fma2(y, fma2(y, c4, c3), c2), f2(1.0f)));
+    K.template pair2<K_B>(B, C);
+    K.template pair2<K_A>(A, tol);
+    // Halley steps for the pair until every active element has accepted its step (an element that
+    // accepted earlier just takes one more, smaller, step)
+#pragma unroll 1
+    for (int it = 0; it < 3; ++it) {
+      const F2 ad = abs2(d);
+      if ((ax && !(ad.x <= (float)RR_TRIG_SMALL)) || (ay && !(ad.y <= (float)RR_TRIG_SMALL))) break;
+      F2 s, cm1, sres;
+      rr_sincosm1_small2(d, s, cm1, sres);
+      const F2 bc = mul2(B, cm1);
+      const F2 t = fma2(C, s, bc);                                          // e [sin E - sin E_tr]
+      const F2 g = sub2(fma2(A, d, neg2(dM)), fma2(C, sres, bc));           // (rr_separation2, fp32)
+      const F2 gp = sub2(A, fma2(C, cm1, neg2(mul2(B, s))));                // 1 - e cos E
+      const F2 gpp = add2(B, t);                                            // e sin E
+      const F2 dd = mul2(neg2(mul2(g, gp)), rcp2(fma2(mul2(f2(-0.5f), g), gpp, mul2(gp, gp))));
+      const F2 c = add2(f2(1.0f), cm1);
+      const F2 h2 = mul2(mul2(f2(0.5f), dd), dd);
+      s2 = fma2(neg2(s), h2, fma2(c, dd, s));
+      cm2 = fma2(neg2(c), h2, fma2(neg2(s), dd, cm1));
+      const F2 add_ = abs2(dd);
+      okx = !ax || add_.x <= tol.x;
+      oky = !ay || add_.y <= tol.y;
+      if (okx && oky) break;
+      d = add2(d, dd);
+    }
+  }
+  if (!(okx && oky)) {                           // |d| > 0.5 or no convergence: the bracketed solver
+    float e, sE;
+    K.template pair<K_E>(e, sE);
+    const float cE = K.template get<K_CE>();
+    if (!okx) rr_kepler_robust<float>(e, sE, cE, dM.x, &s2.x, &cm2.x);
+    if (!oky) rr_kepler_robust<float>(e, sE, cE, dM.y, &s2.y, &cm2.y);
+  }
+  F2 X1, X2, Y1, Y2, Y0, aci2;
+  K.template pair2<K_X1>(X1, X2);
+  K.template pair2<K_Y1>(Y1, Y2);
+  K.template pair2<K_Y0>(Y0, aci2);
+  const F2 xs = fma2(X1, cm2, mul2(X2, s2));
+  const F2 ys = add2(Y0, fma2(Y1, cm2, mul2(Y2, s2)));
+  fx = ys.x > 0.0f;
+  fy = ys.y > 0.0f;
+  return fma2(xs, xs, fma2(mul2(aci2, ys), ys, f2(1e-30f)));
+}
+
+// Occulted light ip * ap of the pair; (ox, oy): z < 1+k in front of the star.
+template <int M>
+__device__ __forceinline__ F2 rr_deficit_pair(const Cst<float, M> K, F2 z2, bool ox, bool oy,
+                                              bool ksmall) {
+  F2 gscale, opk, omk2, afull;
+  K.template pair2<K_GSCALE>(gscale, opk);
+  K.template pair2<K_OMK2>(omk2, afull);
+  z2 = sel2(ox, oy, z2, f2(0.25f));             // a masked element stays inside the staged row
+  const F2 z = rr_sqrt2(z2);
+  const F2 yv = mul2(z, gscale);
+  const int igx = (int)yv.x, igy = (int)yv.y;
+  const F2 ag = sub2(yv, make_float2((float)igx, (float)igy));
+  float l0x, slx, l0y, sly;
+  K.cell(igx, l0x, slx);
+  K.cell(igy, l0y, sly);
+  const F2 ip = fma2(ag, make_float2(slx, sly), make_float2(l0x, l0y));
+  const bool inx = ox && z2.x > omk2.x, iny = oy && z2.y > omk2.y;
+  F2 ap = afull;
+  if (inx || iny) {                             // lens area (rr_deficit), both elements
+    const F2 omks = K.template get2<K_OMKS>();
+    const F2 A = sub2(opk, z), B = add2(z, omks), C = sub2(z, omks), D = add2(z, opk);
+    const F2 AB = abs2(mul2(A, B)), S = abs2(mul2(C, D)), Q = mul2(B, D);
+    const F2 kite = rr_sqrt2(add2(mul2(AB, S), f2(1e-30f)));
+    const F2 tk2 = K.template get2<K_2K2>();
+    const F2 h2 = rr_atan_quadrant2(kite, S, AB);
+    const F2 h1 = ksmall ? rr_atan_t2(rr_div3_2(kite, Q))
+                         : rr_atan_quadrant2(kite, Q, abs2(mul2(A, C)));
+    const F2 lens = fma2(h1, f2(2.0f), fma2(tk2, h2, mul2(f2(-0.5f), kite)));
+    ap = make_float2(inx ? fmaxf(lens.x, 0.0f) : afull.x, iny ? fmaxf(lens.y, 0.0f) : afull.y);
+  }
+  return sel2(ox, oy, mul2(ip, ap), f2(0.0f));
+}
+
+// The thread-per-exposure loop of rr_tile for the fp32 kernels: exposures i and i + FT together.
+template <typename O, bool CIRC, bool NOWRAP, int M>
+__device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, O *__restrict__ out,
+                                              int count, int ns, double t0, double inv_p,
+                                              double u_mid, double hwid, double hw, O scale,
+                                              const Cst<float, M> K, bool ksmall) {
+  const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0), hskip = hwid + hw;
+  const bool need_front =
+      __shfl_sync(0xffffffffu, (int)(CIRC ? !(hskip + hw < 0.25) : !(hwid < 0.49)), 0) != 0;
+  const F2 da2 = f2((float)(RR_TWOPI * du));
+  const float hwa = (float)(RR_TWOPI * hwid);
+  uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
+  uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
+  int left = count - (int)threadIdx.x;
+  double tna = left > 0 ? rr_ld_time(tp) : 0.0, tnb = left > FT ? rr_ld_time(tp + FT * 8) : tna;
+  for (; left > 0; left -= 2 * FT) {
+    const bool has1 = left > FT;
+    const double ta = tna, tb = tnb;
+    // the next pair's times are in flight during this pair
+    if (left > 2 * FT) {
+      tna = rr_ld_time(tp + 2 * FT * 8);
+      tnb = left > 3 * FT ? rr_ld_time(tp + 3 * FT * 8) : tna;
+    }
+    const double wca = fma(ta - t0, inv_p, -u_mid), wcb = fma(tb - t0, inv_p, -u_mid);
+    const double wra = wca - rr_round(wca), wrb = wcb - rr_round(wcb);
+    const bool ina = fabs(wra) <= hskip, inb = has1 && fabs(wrb) <= hskip;
+    O fa = (wra == wra) ? (O)1 : rr_nan<O>(), fb = (wrb == wrb) ? (O)1 : rr_nan<O>();
+    if (ina || inb) {
+      O acca = (O)0, accb = (O)0;
+      double wa = wra + off0, wb = wrb + off0;
+      const F2 opk2 = K.template get2<K_OPK2>();
+      // NOWRAP (block-uniform: the exposure cannot wrap): the angles 2 pi x phase from the window
+      // centre (aw) and from conjunction (am) of the first sub-sample rounded ONCE from fp64, then an
+      // fp32 step per sub-sample - 2 eps32 |angle|, the size of the rounding of dM the fp32 solver
+      // starts from anyway - instead of six fp64 instructions and two conversions per element
+      const F2 aw0 = make_float2((float)(RR_TWOPI * wa), (float)(RR_TWOPI * wb));
+      const F2 am0 = make_float2((float)(RR_TWOPI * (wa + u_mid)), (float)(RR_TWOPI * (wb + u_mid)));
+      F2 fs = f2(0.0f);
+      for (int s = 0; s < ns; ++s, wa += du, wb += du, fs = add2(fs, f2(1.0f))) {
+        bool ax, ay;
+        F2 dM;
+        if (NOWRAP) {
+          const F2 aw = abs2(fma2(fs, da2, aw0));
+          ax = ina && aw.x <= hwa;
+          ay = inb && aw.y <= hwa;
+          if (!(ax || ay)) continue;
+          dM = fma2(fs, da2, am0);
+        } else {
+          const double was = wa - rr_round(wa), wbs = wb - rr_round(wb);
+          ax = ina && fabs(was) <= hwid;
+          ay = inb && fabs(wbs) <= hwid;
+          if (!(ax || ay)) continue;
+          dM = make_float2((float)(RR_TWOPI * (was + u_mid)), (float)(RR_TWOPI * (wbs + u_mid)));
+        }
+        dM = sel2(ax, ay, dM, f2(0.0f));
+        bool fx, fy;
+        const F2 z2 = rr_separation2_pair<CIRC, M>(K, dM, ax, ay, fx, fy);
+        bool ox = ax && z2.x < opk2.x, oy = ay && z2.y < opk2.y;
+        if (need_front) { ox = ox && fx; oy = oy && fy; }
+        if (ox || oy) {
+          const F2 def = rr_deficit_pair<M>(K, z2, ox, oy, ksmall);
+          acca += (O)def.x;
+          accb += (O)def.y;
+        }
+      }
+      if (ina) fa = fma(-acca, scale, (O)1);
+      if (inb) fb = fma(-accb, scale, (O)1);
+    }
+    RR_STORE(reinterpret_cast<O *>(op), fa);
+    if (has1) RR_STORE(reinterpret_cast<O *>(op + FT * sizeof(O)), fb);
+    asm volatile("add.u64 %0, %0, %1;" : "+l"(tp) : "n"(2 * FT * 8));
+    asm volatile("add.u64 %0, %0, %1;" : "+l"(op) : "n"(2 * FT * (int)sizeof(O)));
+  }
+}
+
 // The exposures of one tile for one pv.  CIRC: e == 0 (block-uniform).
 // R = arithmetic type of z and ip*ap; O = type of the sub-sample sum, the final 1 - sum/(Istar ns)
 // and the stored flux (O = double with R = float is RR_MIXED, the scheme of PAPER.md:293).
-template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP, int M>
+template <typename R, typename O, bool COUNT, bool CIRC, bool NOWRAP, int M, bool PAIRS>
 __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__restrict__ out,
                                         int count, int ns, int shuffle, double t0, double inv_p,
                                         double u_mid, double hwid, double hw, O scale,
@@ -696,6 +909,14 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double hskip = hwid + hw;
   // k^2 <= 1/2 (block-uniform; lane-0 broadcast so that it stays a predicate, not a compare per use)
   const bool ksmall = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5), 0) != 0;
+  if constexpr (PAIRS && sizeof(R) == 4 && !COUNT) {
+    if (!shuffle && count > FT) {   // fp32: two exposures per thread (tiles of <= FT exposures and
+                                    // the counting build keep the scalar loop)
+      rr_tile_pairs<O, CIRC, NOWRAP, M>(times, out, count, ns, t0, inv_p, u_mid, hwid, hw, scale, K,
+                                        ksmall);
+      return;
+    }
+  }
   if (!shuffle) {
     // ---- one thread per exposure, in-thread loop over its sub-samples ----
     // The time and flux pointers advance by opaque 64-bit adds: otherwise the compiler, short of
@@ -805,9 +1026,15 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
 // flux = 1 with 16-byte stores, without touching the orbit.
 // Shared memory (rr_dyn): cst[K_SMEM] (constants, working precision) | ldw2[ldw_len] (node, slope)
 // pairs of the k-collapsed table row.
-template <typename R, typename O, bool COUNT, int M>
+// MODE 0: plain; 1: with the class counters (bench.py's op count); 2: fp32 kernels with the
+// two-exposures-per-thread FFMA2 loop for tiles longer than a block (the launcher picks it when the
+// tiles of the data are, on average, longer than 1.5 FT exposures; a kernel of its own because the
+// extra code costs the scalar loop registers: the sparse cadence 4b ran 8 % slower with both in one).
+template <typename R, typename O, int MODE, int M>
 __global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
+  constexpr bool COUNT = MODE == 1;
+  constexpr bool PAIRS = MODE == 2 && sizeof(R) == 4;
   const Cst<R, M> K;
   using R2 = typename Cst<R, M>::R2;
   unsigned *tflags = Cst<R, M>::flags();
@@ -929,7 +1156,7 @@ rr_flux_kernel(const FluxParams P) {
           }
         }
         rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns);
-        if (threadIdx.x == K_SCALE) Cst<R, M>::base()[K_SCALE] = (R)sc_d;
+        if (threadIdx.x == K_SCALE) Cst<R, M>::store(K_SCALE, sc_d);
         __syncthreads();
         scale = (O)K.template get<K_SCALE>();
         staged_lc = tlc;
@@ -937,13 +1164,13 @@ rr_flux_kernel(const FluxParams P) {
       const int shuffle = lc.ns >= P.shuffle_min_ns;
       const bool nowrap = hwid + 2.0 * hw < 0.499;
       if (circular)
-        rr_tile<R, O, COUNT, true, false, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, true, false, M, PAIRS>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                           inv_p, u_mid, hwid, hw, scale, K, cnt);
       else if (nowrap)
-        rr_tile<R, O, COUNT, false, true, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, false, true, M, PAIRS>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                           inv_p, u_mid, hwid, hw, scale, K, cnt);
       else
-        rr_tile<R, O, COUNT, false, false, M>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
+        rr_tile<R, O, COUNT, false, false, M, PAIRS>(P.times + tstart, row + tstart, tcount, lc.ns, shuffle, t0,
                                            inv_p, u_mid, hwid, hw, scale, K, cnt);
     }
   }
@@ -1184,7 +1411,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  size_t smem = (size_t)(K_SMEM + 2 * P.ldw_len) * (c.precision != RR_FP64 ? 4 : 8) + 16;
+  size_t smem = (size_t)K_SMEM * 8 + 16 + (size_t)2 * P.ldw_len * (c.precision != RR_FP64 ? 4 : 8);
   smem = (smem + 15) & ~(size_t)15;
   P.ones_off = (unsigned)smem;
 #if RR_BULK_FILL
@@ -1194,14 +1421,17 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
   using Kernel = void (*)(const FluxParams);
   const int pi = c.precision == RR_FP32 ? 1 : (c.precision == RR_MIXED ? 2 : 0);
-#define RR_KROW(R, O, M) {rr_flux_kernel<R, O, false, M>, rr_flux_kernel<R, O, true, M>}
-  static const Kernel kernels[2][3][2] = {
+#define RR_KROW(R, O, M) {rr_flux_kernel<R, O, 0, M>, rr_flux_kernel<R, O, 1, M>, rr_flux_kernel<R, O, 2, M>}
+  static const Kernel kernels[2][3][3] = {
       {RR_KROW(double, double, RR_SM_FALLBACK_F64), RR_KROW(float, float, RR_SM_FALLBACK_F32),
        RR_KROW(float, double, RR_SM_FALLBACK_F32)},
       {RR_KROW(double, double, RR_SM_ABS), RR_KROW(float, float, RR_SM_ABS),
        RR_KROW(float, double, RR_SM_ABS)}};
 #undef RR_KROW
-  const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : 0];
+  // fp32 kernels: the pair loop when the data's tiles are long enough to give a thread two exposures
+  const bool pairs = RR_FP32_PAIRS && pi != 0 && 2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
+                     ctx->reduction != RR_REDUCE_SHUFFLE;
+  const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
   if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory
     RR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, FT, smem, st>>>(P);
@@ -1215,10 +1445,10 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
   if (fp32_math)
-    rr_orbit_kernel<float><<<grid, FT, K_SMEM * sizeof(float) + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
+    rr_orbit_kernel<float><<<grid, FT, K_SMEM * 8 + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
                                                 ctx->ntiles, npv, ctx->nsub, d_z);
   else
-    rr_orbit_kernel<double><<<grid, FT, K_SMEM * sizeof(double) + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
+    rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;

@@ -113,3 +113,24 @@ def test_octant_threshold_literal():
     assert np.float64(t2d).view(np.uint64) & np.uint64(0xffffffff) == 0
     assert 0 <= mp.sqrt(exact / mp.mpf(t2d)) - 1 < 2.1e-7
     assert abs(mp.mpf(float(np.float32(m.group(2)))) / exact - 1) < 1e-7
+
+
+@pytest.mark.parametrize("name", ["RR_SIN_F", "RR_COS_F", "RR_ATAN_F"])
+def test_packed_tables_repeat_the_scalar_ones(name):
+    """The fp32 two-exposures-per-thread path (FFMA2) reads its coefficients as (c, c) pairs from
+    RR_*_F2: every pair must hold the scalar table's value twice."""
+    _, scalar = parsed(name)
+    m = re.search(r"__constant__\s+float2\s+" + name + r"2\[(\d+)\]\s*=\s*\{(.*?)\};", SRC, re.S)
+    assert m, name
+    pairs = re.findall(r"\{([^{}]+?),([^{}]+?)\}", m.group(2))
+    assert len(pairs) == int(m.group(1)) == len(scalar)
+
+    def val(tok):
+        tok = tok.strip()
+        if "/" in tok:
+            a, b = (np.float32(x.strip().rstrip("f")) for x in tok.split("/"))
+            return np.float32(a / b)
+        return np.float32(tok.rstrip("f"))
+
+    for (a, b), c in zip(pairs, scalar):
+        assert val(a) == val(b) == c, (name, a, b, c)
