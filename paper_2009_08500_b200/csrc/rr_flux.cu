@@ -830,8 +830,9 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
   const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0), hskip = hwid + hw;
   const bool need_front =
       __shfl_sync(0xffffffffu, (int)(CIRC ? !(hskip + hw < 0.25) : !(hwid < 0.49)), 0) != 0;
-  const F2 da2 = f2((float)(RR_TWOPI * du));
-  const float hwa = (float)(RR_TWOPI * hwid);
+  // (lane-0 broadcasts: opaque, or the compiler recomputes both from fp64 in the sub-sample loop)
+  const F2 da2 = f2(__shfl_sync(0xffffffffu, (float)(RR_TWOPI * du), 0));
+  const float hwa = __shfl_sync(0xffffffffu, (float)(RR_TWOPI * hwid), 0);
   uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
   uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
   int left = count - (int)threadIdx.x;
@@ -856,7 +857,8 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
       // centre (aw) and from conjunction (am) of the first sub-sample rounded ONCE from fp64, then an
       // fp32 step per sub-sample - 2 eps32 |angle|, the size of the rounding of dM the fp32 solver
       // starts from anyway - instead of six fp64 instructions and two conversions per element
-      const F2 aw0 = make_float2((float)(RR_TWOPI * wa), (float)(RR_TWOPI * wb));
+      // (an exposure outside the window gets an angle that never passes the test: no flag to keep)
+      const F2 aw0 = make_float2(ina ? (float)(RR_TWOPI * wa) : 1e30f, inb ? (float)(RR_TWOPI * wb) : 1e30f);
       const F2 am0 = make_float2((float)(RR_TWOPI * (wa + u_mid)), (float)(RR_TWOPI * (wb + u_mid)));
       F2 fs = f2(0.0f);
       for (int s = 0; s < ns; ++s, wa += du, wb += du, fs = add2(fs, f2(1.0f))) {
@@ -864,8 +866,8 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
         F2 dM;
         if (NOWRAP) {
           const F2 aw = abs2(fma2(fs, da2, aw0));
-          ax = ina && aw.x <= hwa;
-          ay = inb && aw.y <= hwa;
+          ax = aw.x <= hwa;
+          ay = aw.y <= hwa;
           if (!(ax || ay)) continue;
           dM = fma2(fs, da2, am0);
         } else {
