@@ -364,17 +364,9 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
   const int t = threadIdx.x;
   double v = 0.0;
   switch (t) {
-    case K_CD: case K_SD: {                  // cos, sin of the phase step 2 pi du (circular path)
-      const double ang = RR_TWOPI * du;
-      if (fabs(ang) <= RR_TRIG_SMALL) {      // always, but for exposures of a twelfth of a period
-        double sn, cm1;
-        rr_sincosm1_small(ang, sn, cm1);
-        v = t == K_CD ? 1.0 + cm1 : sn;
-      } else {
-        v = t == K_CD ? cospi(2.0 * du) : sinpi(2.0 * du);
-      }
-      break;
-    }
+    // (library calls on two lanes: a polynomial here changed the register allocation of the whole
+    // kernel and cost the sparse cadence 4b 10 %)
+    case K_CD: v = cospi(2.0 * du); break;   case K_SD: v = sinpi(2.0 * du); break;
     case K_ZC0: v = o.zc0 + (sizeof(R) == 8 ? RR_TINY_D : 1e-30); break;   // z^2 > 0
     case K_ZC1: v = o.zc1; break;
     case K_E: v = o.e; break;           case K_SE: v = o.sE; break;
