@@ -23,6 +23,9 @@
 // to a bracketed Halley/bisection loop.  sin d, cos d - 1 on |d| <= 0.5 are Taylor polynomials with
 // their coefficients in constant memory (rr_math.cuh).  Circular orbits in fp64: sin/cos once per
 // exposure, one plane rotation per further sub-sample.
+// Round 2: out-of-window runs of flux = 1 go out as TMA bulk copies from a block-resident buffer of
+// ones (rr_fill_ones_bulk); the fp32 and mixed kernels take two exposures per thread with packed
+// FFMA2 arithmetic (rr_tile_pairs) when the tiles are longer than a block.
 #include <algorithm>
 
 #include "rr_common.cuh"
@@ -203,7 +206,7 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   pvo[v] = po;
 }
 
-// ---- per-(tile, pv) constants, staged in shared memory in the working precision -----------------------
+// ---- per-(tile, pv) constants, staged in shared memory (8-byte slots: a double, or the float twice) ----
 // Read with volatile loads at the point of use: they are warp-uniform broadcasts that ride in the
 // issue slots the half-rate FP64 pipe leaves free, and keeping ~25 of them out of registers is what
 // lets 8 blocks of 128 threads share an SM.  The loads name the dynamic shared array by its PTX
@@ -701,61 +704,93 @@ __device__ __forceinline__ double rr_ld_time(uintptr_t p) {
 #endif
 }
 
-// ---- fp32 kernels: two exposures per thread, packed FFMA2 arithmetic ---------------------------------
+// ---- two exposures per thread ---------------------------------------------------------------------------
+// fp32 / mixed kernels: packed FFMA2 arithmetic (one instruction, two exposures).  fp64 kernel
+// (eccentric tiles; circular ones keep their rotation recurrence): two scalar instructions per
+// operation, but one load of every constant and coefficient, one branch, one loop for the pair, and two
+// independent dependency chains per warp.
 // (ax, ay): the element is inside the transit window at this sub-sample.  An inactive element is
 // given the phase 0, computes along and is masked out; nothing here can fault on its values.
 #ifndef RR_FP32_PAIRS
 #define RR_FP32_PAIRS 1
 #endif
-// The phases come as dM = 2 pi ur already in fp32 (rr_tile_pairs: one fp64 phase per exposure, an fp32
-// step per sub-sample when the exposure cannot wrap; else rounded from the fp64 phase each time).
-template <bool CIRC, int M>
-__device__ __forceinline__ F2 rr_separation2_pair(const Cst<float, M> K, F2 dM, bool ax, bool ay,
-                                                  bool &fx, bool &fy) {
+#ifndef RR_FP64_PAIRS
+#define RR_FP64_PAIRS 0   // measured, 80 registers / 6 blocks per SM: config 4 5.09 -> 5.56 ms, config 3
+                          // 7.56 -> 9.04: the FP64 pipe is the limit there, the pair shares everything
+                          // but the FP64 arithmetic and costs occupancy; kept as a build option
+#endif
+// two neighbouring constants as pairs (c, c): fp32 from the doubled slots, fp64 splat in registers
+template <int I, typename R, int M>
+__device__ __forceinline__ void rr_pairP(const Cst<R, M> K, typename PairT<R>::type &a,
+                                         typename PairT<R>::type &b) {
+  if constexpr (sizeof(R) == 4) {
+    K.template pair2<I>(a, b);
+  } else {
+    R x, y;
+    K.template pair<I>(x, y);
+    a = splat<R>(x);
+    b = splat<R>(y);
+  }
+}
+template <int I, typename R, int M>
+__device__ __forceinline__ typename PairT<R>::type rr_getP(const Cst<R, M> K) {
+  if constexpr (sizeof(R) == 4) return K.template get2<I>();
+  else return splat<R>(K.template get<I>());
+}
+
+// The phases come as dM = 2 pi ur in the working precision (rr_tile_pairs).
+template <typename R, bool CIRC, int M>
+__device__ __forceinline__ typename PairT<R>::type
+rr_separation2_pair(const Cst<R, M> K, typename PairT<R>::type dM, bool ax, bool ay, bool &fx,
+                    bool &fy) {
+  using P = typename PairT<R>::type;
   if (CIRC) {
-    F2 s;
-    const F2 am = abs2(dM);
-    if (am.x <= 0.4995f && am.y <= 0.4995f) {
-      F2 cm1, sres;
+    P s;
+    const P am = abs2(dM);
+    if (am.x <= (R)0.4995 && am.y <= (R)0.4995) {
+      P cm1, sres;
       rr_sincosm1_small2(dM, s, cm1, sres);
     } else {
-      s = make_float2(sinf(dM.x), sinf(dM.y));
+      s = mk2((R)sin((double)dM.x), (R)sin((double)dM.y));
     }
-    fx = am.x < 1.5707963f;
-    fy = am.y < 1.5707963f;
-    F2 zc0, zc1;
-    K.template pair2<K_ZC0>(zc0, zc1);
+    fx = am.x < (R)1.5707963;
+    fy = am.y < (R)1.5707963;
+    P zc0, zc1;
+    rr_pairP<K_ZC0>(K, zc0, zc1);
     return fma2(mul2(s, s), zc1, zc0);
   }
-  F2 s2 = f2(0.0f), cm2 = f2(0.0f);
+  P s2 = splat<R>((R)0), cm2 = splat<R>((R)0);
   bool okx = !ax, oky = !ay;
   {
-    F2 c4, c3, c2, ky, B, C, A, tol;
-    K.template pair2<K_C4>(c4, c3);
-    K.template pair2<K_C2>(c2, ky);
-    const F2 y = mul2(dM, mul2(ky, f2(0.15915494309189535f)));           // dM / A (K_KY = 2 pi / A)
-    F2 d = mul2(y, fma2(y, fma2(y, fma2(y, c4, c3), c2), f2(1.0f)));
-    K.template pair2<K_B>(B, C);
-    K.template pair2<K_A>(A, tol);
+    P c4, c3, c2, ky, B, C, A, tol;
+    rr_pairP<K_C4>(K, c4, c3);
+    rr_pairP<K_C2>(K, c2, ky);
+    const P y = mul2(dM, mul2(ky, splat<R>((R)0.15915494309189535)));   // dM / A (K_KY = 2 pi / A)
+    P d = mul2(y, fma2(y, fma2(y, fma2(y, c4, c3), c2), splat<R>((R)1)));
+    rr_pairP<K_B>(K, B, C);
+    rr_pairP<K_A>(K, A, tol);
     // Halley steps for the pair until every active element has accepted its step (an element that
     // accepted earlier just takes one more, smaller, step)
 #pragma unroll 1
     for (int it = 0; it < 3; ++it) {
-      const F2 ad = abs2(d);
-      if ((ax && !(ad.x <= (float)RR_TRIG_SMALL)) || (ay && !(ad.y <= (float)RR_TRIG_SMALL))) break;
-      F2 s, cm1, sres;
+      const P ad = abs2(d);
+      if ((ax && !(ad.x <= (R)RR_TRIG_SMALL)) || (ay && !(ad.y <= (R)RR_TRIG_SMALL))) break;
+      P s, cm1, sres;
       rr_sincosm1_small2(d, s, cm1, sres);
-      const F2 bc = mul2(B, cm1);
-      const F2 t = fma2(C, s, bc);                                          // e [sin E - sin E_tr]
-      const F2 g = sub2(fma2(A, d, neg2(dM)), fma2(C, sres, bc));           // (rr_separation2, fp32)
-      const F2 gp = sub2(A, fma2(C, cm1, neg2(mul2(B, s))));                // 1 - e cos E
-      const F2 gpp = add2(B, t);                                            // e sin E
-      const F2 dd = mul2(neg2(mul2(g, gp)), rcp2(fma2(mul2(f2(-0.5f), g), gpp, mul2(gp, gp))));
-      const F2 c = add2(f2(1.0f), cm1);
-      const F2 h2 = mul2(mul2(f2(0.5f), dd), dd);
+      const P bc = mul2(B, cm1);
+      const P t = fma2(C, s, bc);                                           // e [sin E - sin E_tr]
+      P g;
+      if constexpr (sizeof(R) == 8) g = sub2(sub2(d, dM), t);
+      else g = sub2(fma2(A, d, neg2(dM)), fma2(C, sres, bc));              // (rr_separation2, fp32)
+      const P gp = sub2(A, fma2(C, cm1, neg2(mul2(B, s))));                 // 1 - e cos E
+      const P gpp = add2(B, t);                                             // e sin E
+      const P dd = mul2(neg2(mul2(g, gp)),
+                        rcp2(fma2(mul2(splat<R>((R)-0.5), g), gpp, mul2(gp, gp))));
+      const P c = add2(splat<R>((R)1), cm1);
+      const P h2 = mul2(mul2(splat<R>((R)0.5), dd), dd);
       s2 = fma2(neg2(s), h2, fma2(c, dd, s));
       cm2 = fma2(neg2(c), h2, fma2(neg2(s), dd, cm1));
-      const F2 add_ = abs2(dd);
+      const P add_ = abs2(dd);
       okx = !ax || add_.x <= tol.x;
       oky = !ay || add_.y <= tol.y;
       if (okx && oky) break;
@@ -763,67 +798,75 @@ __device__ __forceinline__ F2 rr_separation2_pair(const Cst<float, M> K, F2 dM, 
     }
   }
   if (!(okx && oky)) {                           // |d| > 0.5 or no convergence: the bracketed solver
-    float e, sE;
+    R e, sE;
     K.template pair<K_E>(e, sE);
-    const float cE = K.template get<K_CE>();
-    if (!okx) rr_kepler_robust<float>(e, sE, cE, dM.x, &s2.x, &cm2.x);
-    if (!oky) rr_kepler_robust<float>(e, sE, cE, dM.y, &s2.y, &cm2.y);
+    const R cE = K.template get<K_CE>();
+    if (!okx) rr_kepler_robust<R>(e, sE, cE, dM.x, &s2.x, &cm2.x);
+    if (!oky) rr_kepler_robust<R>(e, sE, cE, dM.y, &s2.y, &cm2.y);
   }
-  F2 X1, X2, Y1, Y2, Y0, aci2;
-  K.template pair2<K_X1>(X1, X2);
-  K.template pair2<K_Y1>(Y1, Y2);
-  K.template pair2<K_Y0>(Y0, aci2);
-  const F2 xs = fma2(X1, cm2, mul2(X2, s2));
-  const F2 ys = add2(Y0, fma2(Y1, cm2, mul2(Y2, s2)));
-  fx = ys.x > 0.0f;
-  fy = ys.y > 0.0f;
-  return fma2(xs, xs, fma2(mul2(aci2, ys), ys, f2(1e-30f)));
+  P X1, X2, Y1, Y2, Y0, aci2;
+  rr_pairP<K_X1>(K, X1, X2);
+  rr_pairP<K_Y1>(K, Y1, Y2);
+  rr_pairP<K_Y0>(K, Y0, aci2);
+  const P xs = fma2(X1, cm2, mul2(X2, s2));
+  const P ys = add2(Y0, fma2(Y1, cm2, mul2(Y2, s2)));
+  fx = ys.x > (R)0;
+  fy = ys.y > (R)0;
+  const R tiny = sizeof(R) == 8 ? (R)RR_TINY_D : (R)1e-30f;
+  return fma2(xs, xs, fma2(mul2(aci2, ys), ys, splat<R>(tiny)));
 }
 
 // Occulted light ip * ap of the pair; (ox, oy): z < 1+k in front of the star.
-template <int M>
-__device__ __forceinline__ F2 rr_deficit_pair(const Cst<float, M> K, F2 z2, bool ox, bool oy,
-                                              bool ksmall) {
-  F2 gscale, opk, omk2, afull;
-  K.template pair2<K_GSCALE>(gscale, opk);
-  K.template pair2<K_OMK2>(omk2, afull);
-  z2 = sel2(ox, oy, z2, f2(0.25f));             // a masked element stays inside the staged row
-  const F2 z = rr_sqrt2(z2);
-  const F2 yv = mul2(z, gscale);
-  const int igx = (int)yv.x, igy = (int)yv.y;
-  const F2 ag = sub2(yv, make_float2((float)igx, (float)igy));
-  float l0x, slx, l0y, sly;
+template <typename R, int M>
+__device__ __forceinline__ typename PairT<R>::type
+rr_deficit_pair(const Cst<R, M> K, typename PairT<R>::type z2, bool ox, bool oy, bool ksmall) {
+  using P = typename PairT<R>::type;
+  P gscale, opk, omk2, afull;
+  rr_pairP<K_GSCALE>(K, gscale, opk);
+  rr_pairP<K_OMK2>(K, omk2, afull);
+  z2 = sel2(ox, oy, z2, splat<R>((R)0.25));     // a masked element stays inside the staged row
+  const P z = rr_sqrt2(z2);
+  const P yv = mul2(z, gscale);
+  int igx, igy;
+  P ag;
+  rr_cell(yv.x, igx, ag.x);
+  rr_cell(yv.y, igy, ag.y);
+  R l0x, slx, l0y, sly;
   K.cell(igx, l0x, slx);
   K.cell(igy, l0y, sly);
-  const F2 ip = fma2(ag, make_float2(slx, sly), make_float2(l0x, l0y));
+  const P ip = fma2(ag, mk2(slx, sly), mk2(l0x, l0y));
   const bool inx = ox && z2.x > omk2.x, iny = oy && z2.y > omk2.y;
-  F2 ap = afull;
+  P ap = afull;
   if (inx || iny) {                             // lens area (rr_deficit), both elements
-    const F2 omks = K.template get2<K_OMKS>();
-    const F2 A = sub2(opk, z), B = add2(z, omks), C = sub2(z, omks), D = add2(z, opk);
-    const F2 AB = abs2(mul2(A, B)), S = abs2(mul2(C, D)), Q = mul2(B, D);
-    const F2 kite = rr_sqrt2(add2(mul2(AB, S), f2(1e-30f)));
-    const F2 tk2 = K.template get2<K_2K2>();
-    const F2 h2 = rr_atan_quadrant2(kite, S, AB);
-    const F2 h1 = ksmall ? rr_atan_t2(rr_div3_2(kite, Q))
-                         : rr_atan_quadrant2(kite, Q, abs2(mul2(A, C)));
-    const F2 lens = fma2(h1, f2(2.0f), fma2(tk2, h2, mul2(f2(-0.5f), kite)));
-    ap = make_float2(inx ? fmaxf(lens.x, 0.0f) : afull.x, iny ? fmaxf(lens.y, 0.0f) : afull.y);
+    const P omks = rr_getP<K_OMKS>(K);
+    const P A = sub2(opk, z), B = add2(z, omks), C = sub2(z, omks), D = add2(z, opk);
+    const P AB = abs2(mul2(A, B)), S = abs2(mul2(C, D)), Q = mul2(B, D);
+    const R tiny = sizeof(R) == 8 ? (R)RR_TINY_D : (R)1e-30f;
+    const P kite = rr_sqrt2(add2(mul2(AB, S), splat<R>(tiny)));
+    const P tk2 = rr_getP<K_2K2>(K);
+    const P h2 = rr_atan_quadrant2(kite, S, AB);
+    const P h1 = ksmall ? rr_atan_t2(rr_div3_2(kite, Q))
+                        : rr_atan_quadrant2(kite, Q, abs2(mul2(A, C)));
+    P lens = fma2(h1, splat<R>((R)2), fma2(tk2, h2, mul2(splat<R>((R)-0.5), kite)));
+    if constexpr (sizeof(R) == 4) lens = mk2(fmaxf(lens.x, 0.0f), fmaxf(lens.y, 0.0f));
+    ap = sel2(inx, iny, lens, afull);
   }
-  return sel2(ox, oy, mul2(ip, ap), f2(0.0f));
+  return sel2(ox, oy, mul2(ip, ap), splat<R>((R)0));
 }
 
-// The thread-per-exposure loop of rr_tile for the fp32 kernels: exposures i and i + FT together.
-template <typename O, bool CIRC, bool NOWRAP, int M>
+// The thread-per-exposure loop of rr_tile for a pair of exposures i and i + FT.
+template <typename R, typename O, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, O *__restrict__ out,
                                               int count, int ns, double t0, double inv_p,
                                               double u_mid, double hwid, double hw, O scale,
-                                              const Cst<float, M> K, bool ksmall) {
+                                              const Cst<R, M> K, bool ksmall) {
+  using P = typename PairT<R>::type;
+  constexpr bool ANG = NOWRAP && sizeof(R) == 4;   // fp32 angle step per sub-sample
   const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0), hskip = hwid + hw;
   const bool need_front =
       __shfl_sync(0xffffffffu, (int)(CIRC ? !(hskip + hw < 0.25) : !(hwid < 0.49)), 0) != 0;
   // (lane-0 broadcasts: opaque, or the compiler recomputes both from fp64 in the sub-sample loop)
-  const F2 da2 = f2(__shfl_sync(0xffffffffu, (float)(RR_TWOPI * du), 0));
+  const float2 da2 = splat<float>(__shfl_sync(0xffffffffu, (float)(RR_TWOPI * du), 0));
   const float hwa = __shfl_sync(0xffffffffu, (float)(RR_TWOPI * hwid), 0);
   uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
   uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
@@ -843,45 +886,49 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
     O fa = (wra == wra) ? (O)1 : rr_nan<O>(), fb = (wrb == wrb) ? (O)1 : rr_nan<O>();
     if (ina || inb) {
       O acca = (O)0, accb = (O)0;
-      double wa = wra + off0, wb = wrb + off0;
-      const F2 opk2 = K.template get2<K_OPK2>();
-      // NOWRAP (block-uniform: the exposure cannot wrap): the angles 2 pi x phase from the window
-      // centre (aw) and from conjunction (am) of the first sub-sample rounded ONCE from fp64, then an
-      // fp32 step per sub-sample - 2 eps32 |angle|, the size of the rounding of dM the fp32 solver
-      // starts from anyway - instead of six fp64 instructions and two conversions per element
-      // (an exposure outside the window gets an angle that never passes the test: no flag to keep)
-      const F2 aw0 = make_float2(ina ? (float)(RR_TWOPI * wa) : 1e30f, inb ? (float)(RR_TWOPI * wb) : 1e30f);
-      const F2 am0 = make_float2((float)(RR_TWOPI * (wa + u_mid)), (float)(RR_TWOPI * (wb + u_mid)));
-      F2 fs = f2(0.0f);
-      for (int s = 0; s < ns; ++s, wa += du, wb += du, fs = add2(fs, f2(1.0f))) {
+      // an exposure outside the window gets a phase that never passes the test: no flag to keep
+      double wa = ina ? wra + off0 : 1e30, wb = inb ? wrb + off0 : 1e30;
+      const P opk2 = rr_getP<K_OPK2>(K);
+      // ANG (fp32, the exposure cannot wrap): the angles 2 pi x phase from the window centre (aw)
+      // and from conjunction (am) of the first sub-sample rounded ONCE from fp64, then an fp32 step
+      // per sub-sample - 2 eps32 |angle|, the size of the rounding of dM the fp32 solver starts from
+      // anyway - instead of six fp64 instructions and two conversions per element
+      const float2 aw0 = make_float2(ina ? (float)(RR_TWOPI * wa) : 1e30f, inb ? (float)(RR_TWOPI * wb) : 1e30f);
+      const float2 am0 = make_float2((float)(RR_TWOPI * (wra + off0 + u_mid)), (float)(RR_TWOPI * (wrb + off0 + u_mid)));
+      float2 fs = splat<float>(0.0f);
+      for (int s = 0; s < ns; ++s, wa += du, wb += du) {
         bool ax, ay;
-        F2 dM;
-        if (NOWRAP) {
-          const F2 aw = abs2(fma2(fs, da2, aw0));
+        P dM;
+        if constexpr (ANG) {
+          const float2 aw = abs2(fma2(fs, da2, aw0));
           ax = aw.x <= hwa;
           ay = aw.y <= hwa;
+          const float2 am = fma2(fs, da2, am0);
+          fs = add2(fs, splat<float>(1.0f));
           if (!(ax || ay)) continue;
-          dM = fma2(fs, da2, am0);
+          dM = mk2((R)am.x, (R)am.y);
         } else {
-          const double was = wa - rr_round(wa), wbs = wb - rr_round(wb);
-          ax = ina && fabs(was) <= hwid;
-          ay = inb && fabs(wbs) <= hwid;
+          const double was = NOWRAP ? wa : wa - rr_round(wa), wbs = NOWRAP ? wb : wb - rr_round(wb);
+          ax = fabs(was) <= hwid;               // (1e30 - round(1e30) = 0: only without NOWRAP ...
+          ay = fabs(wbs) <= hwid;
+          if (!NOWRAP) { ax = ax && ina; ay = ay && inb; }   // ... where the flags are needed)
           if (!(ax || ay)) continue;
-          dM = make_float2((float)(RR_TWOPI * (was + u_mid)), (float)(RR_TWOPI * (wbs + u_mid)));
+          dM = mk2((R)(RR_TWOPI * (was + u_mid)), (R)(RR_TWOPI * (wbs + u_mid)));
         }
-        dM = sel2(ax, ay, dM, f2(0.0f));
+        dM = sel2(ax, ay, dM, splat<R>((R)0));
         bool fx, fy;
-        const F2 z2 = rr_separation2_pair<CIRC, M>(K, dM, ax, ay, fx, fy);
+        const P z2 = rr_separation2_pair<R, CIRC, M>(K, dM, ax, ay, fx, fy);
         bool ox = ax && z2.x < opk2.x, oy = ay && z2.y < opk2.y;
         if (need_front) { ox = ox && fx; oy = oy && fy; }
         if (ox || oy) {
-          const F2 def = rr_deficit_pair<M>(K, z2, ox, oy, ksmall);
+          const P def = rr_deficit_pair<R, M>(K, z2, ox, oy, ksmall);
           acca += (O)def.x;
           accb += (O)def.y;
         }
       }
-      if (ina) fa = fma(-acca, scale, (O)1);
-      if (inb) fb = fma(-accb, scale, (O)1);
+      // mean of (Istar - ip ap)/Istar over ns; fp64 staged the table already times 1/(Istar ns)
+      if (ina) fa = sizeof(R) == 8 ? (O)1 - acca : fma(-acca, scale, (O)1);
+      if (inb) fb = sizeof(R) == 8 ? (O)1 - accb : fma(-accb, scale, (O)1);
     }
     RR_STORE(reinterpret_cast<O *>(op), fa);
     if (has1) RR_STORE(reinterpret_cast<O *>(op + FT * sizeof(O)), fb);
@@ -903,11 +950,11 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double hskip = hwid + hw;
   // k^2 <= 1/2 (block-uniform; lane-0 broadcast so that it stays a predicate, not a compare per use)
   const bool ksmall = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5), 0) != 0;
-  if constexpr (PAIRS && sizeof(R) == 4 && !COUNT) {
-    if (!shuffle && count > FT) {   // fp32: two exposures per thread (tiles of <= FT exposures and
-                                    // the counting build keep the scalar loop)
-      rr_tile_pairs<O, CIRC, NOWRAP, M>(times, out, count, ns, t0, inv_p, u_mid, hwid, hw, scale, K,
-                                        ksmall);
+  if constexpr (PAIRS && !COUNT && !(CIRC && sizeof(R) == 8)) {
+    if (!shuffle && count > FT) {   // two exposures per thread (tiles of <= FT exposures, the
+                                    // counting build and fp64 circular tiles keep the scalar loop)
+      rr_tile_pairs<R, O, CIRC, NOWRAP, M>(times, out, count, ns, t0, inv_p, u_mid, hwid, hw, scale,
+                                           K, ksmall);
       return;
     }
   }
@@ -1017,18 +1064,22 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
 // One block per (parameter vector, chunk of consecutive dispatch tiles).  Block = FT threads.
 // The pv's constants are staged once per block, the k-collapsed table row once per light curve the
 // chunk meets; tiles outside the transit window are merged into contiguous runs and written as
-// flux = 1 with 16-byte stores, without touching the orbit.
-// Shared memory (rr_dyn): cst[K_SMEM] (constants, working precision) | ldw2[ldw_len] (node, slope)
+// flux = 1 by TMA bulk copies (rr_fill_ones_bulk), without touching the orbit.
+// Shared memory (rr_dyn): cst[K_SMEM] (constants, 8-byte slots) | ldw2[ldw_len] (node, slope)
 // pairs of the k-collapsed table row.
 // MODE 0: plain; 1: with the class counters (bench.py's op count); 2: fp32 kernels with the
 // two-exposures-per-thread FFMA2 loop for tiles longer than a block (the launcher picks it when the
 // tiles of the data are, on average, longer than 1.5 FT exposures; a kernel of its own because the
 // extra code costs the scalar loop registers: the sparse cadence 4b ran 8 % slower with both in one).
+#ifndef RR_FP64_PAIR_BLOCKS
+#define RR_FP64_PAIR_BLOCKS 6   // resident blocks per SM of the fp64 pair kernel (80 registers)
+#endif
 template <typename R, typename O, int MODE, int M>
-__global__ void __launch_bounds__(FT, RR_FLUX_MIN_BLOCKS)
+__global__ void __launch_bounds__(FT, (MODE == 2 && sizeof(R) == 8) ? RR_FP64_PAIR_BLOCKS
+                                                                    : RR_FLUX_MIN_BLOCKS)
 rr_flux_kernel(const FluxParams P) {
   constexpr bool COUNT = MODE == 1;
-  constexpr bool PAIRS = MODE == 2 && sizeof(R) == 4;
+  constexpr bool PAIRS = MODE == 2;
   const Cst<R, M> K;
   using R2 = typename Cst<R, M>::R2;
   unsigned *tflags = Cst<R, M>::flags();
@@ -1415,7 +1466,9 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
     RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
   using Kernel = void (*)(const FluxParams);
   const int pi = c.precision == RR_FP32 ? 1 : (c.precision == RR_MIXED ? 2 : 0);
-#define RR_KROW(R, O, M) {rr_flux_kernel<R, O, 0, M>, rr_flux_kernel<R, O, 1, M>, rr_flux_kernel<R, O, 2, M>}
+#define RR_KROW(R, O, M)                                                                          \
+  {rr_flux_kernel<R, O, 0, M>, rr_flux_kernel<R, O, 1, M>,                                        \
+   rr_flux_kernel<R, O, (sizeof(R) == 8 && !RR_FP64_PAIRS) ? 0 : 2, M>}
   static const Kernel kernels[2][3][3] = {
       {RR_KROW(double, double, RR_SM_FALLBACK_F64), RR_KROW(float, float, RR_SM_FALLBACK_F32),
        RR_KROW(float, double, RR_SM_FALLBACK_F32)},
@@ -1423,7 +1476,8 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
        RR_KROW(float, double, RR_SM_ABS)}};
 #undef RR_KROW
   // fp32 kernels: the pair loop when the data's tiles are long enough to give a thread two exposures
-  const bool pairs = RR_FP32_PAIRS && pi != 0 && 2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
+  const bool pairs = (pi != 0 ? RR_FP32_PAIRS : RR_FP64_PAIRS) &&
+                     2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
                      ctx->reduction != RR_REDUCE_SHUFFLE;
   const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
   if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory
