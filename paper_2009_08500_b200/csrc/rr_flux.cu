@@ -1074,9 +1074,13 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
 #ifndef RR_FP64_PAIR_BLOCKS
 #define RR_FP64_PAIR_BLOCKS 6   // resident blocks per SM of the fp64 pair kernel (80 registers)
 #endif
+#ifndef RR_FP32_PAIR_BLOCKS
+#define RR_FP32_PAIR_BLOCKS RR_FLUX_MIN_BLOCKS
+#endif
 template <typename R, typename O, int MODE, int M>
-__global__ void __launch_bounds__(FT, (MODE == 2 && sizeof(R) == 8) ? RR_FP64_PAIR_BLOCKS
-                                                                    : RR_FLUX_MIN_BLOCKS)
+__global__ void __launch_bounds__(FT, MODE != 2 ? RR_FLUX_MIN_BLOCKS
+                                                : (sizeof(R) == 8 ? RR_FP64_PAIR_BLOCKS
+                                                                  : RR_FP32_PAIR_BLOCKS))
 rr_flux_kernel(const FluxParams P) {
   constexpr bool COUNT = MODE == 1;
   constexpr bool PAIRS = MODE == 2;
