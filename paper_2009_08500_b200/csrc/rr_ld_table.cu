@@ -229,6 +229,7 @@ constexpr int RT = 256;
 template <typename TR>
 __global__ void __launch_bounds__(RT)
 rr_ld_rows_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
+                  const int2 *__restrict__ sup,
                   const RRPvBand *__restrict__ pvb, TR *__restrict__ rows, int npb, int nkpb,
                   int ng, int nz) {
   extern __shared__ double prof[];
@@ -243,10 +244,17 @@ rr_ld_rows_kernel(const TR *__restrict__ ldp, const double *__restrict__ W,
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const double *W0 = W + (int64_t)ik * ng * nz;
   const double *W1 = W0 + (int64_t)ng * nz;
-  for (int ig = warp; ig < ng; ig += RT / 32) {
+  // (gridDim.y blocks share a row's g nodes: with few rows every warp should have few nodes, each
+  // is two dependent rounds of L2 loads - one row in one block took 13 us)
+  for (int ig = blockIdx.y * (RT / 32) + warp; ig < ng; ig += (RT / 32) * gridDim.y) {
     const double *w0 = W0 + (int64_t)ig * nz, *w1 = W1 + (int64_t)ig * nz;
+    // only the support of the two weight rows (rr_support_kernel): the rest is exactly zero; lanes
+    // keep their j mod 32, so the sums are those of the full loop (1024 rows read 164 MB of W from
+    // L2 otherwise: config 1's rows took as long as its flux kernel)
+    const int2 a0 = sup[(int64_t)ik * ng + ig], a1 = sup[(int64_t)(ik + 1) * ng + ig];
+    const int jl = min(a0.x, a1.x) & ~31, jh = max(a0.y, a1.y);
     double s0 = 0.0, s1 = 0.0;
-    for (int j = lane; j < nz; j += 32) {
+    for (int j = jl + lane; j < jh; j += 32) {
       const double p = prof[j];
       s0 = fma(w0[j], p, s0);
       s1 = fma(w1[j], p, s1);
@@ -585,14 +593,17 @@ int rr_ld_rows_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, cudaStream_t st) {
     return RR_OK;
   }
   const size_t smem = sizeof(double) * ctx->nz;
+  const int gy_max = (c.ng + RT / 32 - 1) / (RT / 32);
+  const int gy = (int)std::max<int64_t>(1, std::min<int64_t>(gy_max, (2 * 8 * ctx->sm_count + M - 1) / M));
+  const dim3 grid((unsigned)M, (unsigned)gy);
   if (c.precision != RR_FP64)
-    rr_ld_rows_kernel<float><<<(unsigned)M, RT, smem, st>>>(
-        (const float *)wk->ldp_src, ctx->d_W, wk->pvb, (float *)wk->rows, c.npb, c.nkpb, c.ng,
-        ctx->nz);
+    rr_ld_rows_kernel<float><<<grid, RT, smem, st>>>(
+        (const float *)wk->ldp_src, ctx->d_W, (const int2 *)ctx->d_Wsup, wk->pvb, (float *)wk->rows,
+        c.npb, c.nkpb, c.ng, ctx->nz);
   else
-    rr_ld_rows_kernel<double><<<(unsigned)M, RT, smem, st>>>(
-        (const double *)wk->ldp_src, ctx->d_W, wk->pvb, (double *)wk->rows, c.npb, c.nkpb, c.ng,
-        ctx->nz);
+    rr_ld_rows_kernel<double><<<grid, RT, smem, st>>>(
+        (const double *)wk->ldp_src, ctx->d_W, (const int2 *)ctx->d_Wsup, wk->pvb, (double *)wk->rows,
+        c.npb, c.nkpb, c.ng, ctx->nz);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
