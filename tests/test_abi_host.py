@@ -171,3 +171,26 @@ def test_binding_refuses_unknown_handles_and_wrong_sizes_without_a_device():
                                 np.ones((2, 10), np.float32), np.zeros(2, np.int64))
     finally:
         rr._CTX.pop(999)
+
+
+def test_workload_4b_is_config_4_with_literal_cadence():
+    """SURVEY 8(d)'s labelled secondary workload: same population and LD draws as config 4, 10^5
+    exposures spaced two minutes apart (centred on t = 0)."""
+    import workloads
+    a = workloads.make_workload(4, npv=5, npt=1001)
+    b = workloads.make_workload("4b", npv=5, npt=1001)
+    assert b.name == "config4b-literal-cadence" and a.name == "config4-stress"
+    assert np.array_equal(a.pv, b.pv) and np.array_equal(a.ld_coeffs, b.ld_coeffs)
+    assert np.allclose(np.diff(b.times), 2.0 / 1440.0, rtol=0, atol=1e-15)
+    assert abs(b.times[500]) < 1e-15 and b.evaluations == a.evaluations
+
+
+def test_bench_reference_arm_takes_the_secondary_workload():
+    import json
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
+                          "--steps", "1", "--warmup", "0", "--config", "4b", "--npv", "4",
+                          "--npt", "700"], capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["config"]["workload"] == "config4b-literal-cadence" and line["value"] > 0
+    assert "every" in line["cpu_baseline"]["sample"] and line["cpu_baseline"]["cpu_model"]
