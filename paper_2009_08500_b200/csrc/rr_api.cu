@@ -24,6 +24,7 @@ void free_work(RRWork *w) {
   if (w->istar) cudaFree(w->istar);
   if (w->pvo) cudaFree(w->pvo);
   if (w->pvb) cudaFree(w->pvb);
+  if (w->lens) cudaFree(w->lens);
   if (w->ldp) cudaFree(w->ldp);
   if (w->rows) cudaFree(w->rows);
   if (w->bk) cudaFree(w->bk);

@@ -61,7 +61,7 @@ struct RRPvBand {
   double kw;           // radius ratio the LD weights are taken at: k, or the mean of the pv's k over
                        // the passbands (transmission-spectroscopy shortcut)
   int32_t ik;          // lower k row of kw, clamped to nk-2 (reading R10)
-  int32_t pad;
+  int32_t lens_ok;     // 1: the polynomial form of the lens area holds for this k (rr_lens_poly_kernel)
 };
 
 // Per-evaluation device buffers: one set for the device-pointer API, one per slot of the
@@ -83,8 +83,11 @@ struct RRWork {
   int32_t have_full;        // T holds the full table of the current profile
   RRPvOrbit *pvo;
   RRPvBand *pvb;
+  double *lens;             // [npv][nkpb][2][RR_LENS_PITCH]: lens-area polynomials (fp64 kernel)
   int64_t pv_cap;
 };
+#define RR_LENS_PITCH 14    // 13 coefficients + 1 pad: 16-byte multiples per half
+#define RR_LENS_KMAX 0.32   // radius ratios up to here take the polynomial form (error <= 2e-13)
 
 // ---- host context -----------------------------------------------------------------------------
 struct rr_ctx {

@@ -30,6 +30,7 @@
 
 #include "rr_common.cuh"
 #include "rr_math.cuh"
+#include "rr_lens_poly.cuh"
 
 // flux is written once and never re-read: streaming stores keep W, times and the rows in L2
 #define RR_STORE(p, v) __stcs((p), (v))
@@ -105,7 +106,7 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
     ik = min(max(ik, 0), nk - 2);
     b.ik = ik;
     b.ak = x - (double)ik;
-    b.pad = 0;
+    b.lens_ok = (k > 0.0 && k <= RR_LENS_KMAX) ? 1 : 0;
     pvb[v * nkpb + q] = b;
     kmax = fmax(kmax, k);
   }
@@ -206,6 +207,48 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   pvo[v] = po;
 }
 
+// ---- lens area between the contacts as two polynomials per (pv, radius ratio) -------------------------
+// For x = (z - (1-k)) / (2k) in (0, 1):  a(z) = pi k^2 - x^(3/2) g0(x) for x <= 1/2 and
+// a(z) = y^(3/2) g1(y), y = 1 - x, for x > 1/2, with g0, g1 analytic (the area is analytic in the angle
+// theta, x = sin^2(theta/2)): degree-12 interpolants at the Chebyshev nodes of [0, 1/2] reproduce the
+// area to 2e-13 for k <= 0.32 (tests/test_device_poly.py).  One warp per (pv, k): lanes 0..12 and
+// 13..25 evaluate the exact area (two sectors minus the kite, reading R9) at the nodes of the two
+// halves; the node values become monomial coefficients in w = 4x - 1 through the matrix RR_LENS_M.
+// The flux kernel then pays one square root and a Horner chain per ingress / egress sub-sample
+// instead of a square root, two divisions and two arctangents (60 -> 23 FP64 instructions).
+__global__ void rr_lens_poly_kernel(const RRPvBand *__restrict__ pvb, int64_t nrows,
+                                    double *__restrict__ lens) {
+  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (row >= nrows) return;
+  const RRPvBand b = pvb[row];
+  if (!b.lens_ok) return;                         // the flux kernel takes the exact form
+  const int half = lane >= RR_LENS_N ? 1 : 0, i = lane - half * RR_LENS_N;
+  double g = 0.0;
+  if (lane < 2 * RR_LENS_N) {
+    const double k = b.k, x = RR_LENS_X[i];
+    const double omks = 1.0 - k, opk = 1.0 + k;
+    const double z = half ? opk - 2.0 * k * x : omks + 2.0 * k * x;
+    const double A = opk - z, B = z + omks, C = z - omks, D = z + opk;
+    const double AB = fabs(A * B), S = fabs(C * D), Q = B * D;
+    const double kite = rr_sqrt3_pos(AB * S);
+    const double h1 = rr_atan_quadrant<double>(kite, Q, fabs(A * C));
+    const double h2 = rr_atan_quadrant<double>(kite, S, AB);
+    const double ap = fma(h1, 2.0, fma(2.0 * b.k2, h2, -0.5 * kite));
+    g = (half ? ap : b.afull - ap) * RR_LENS_XI15[i];
+  }
+  // coefficient j of this lane's half: sum_i M[j][i] g_i
+  double a = 0.0;
+#pragma unroll
+  for (int q = 0; q < RR_LENS_N; ++q) {
+    const double gq = __shfl_sync(0xffffffffu, g, half * RR_LENS_N + q);
+    if (lane < 2 * RR_LENS_N) a = fma(RR_LENS_M[i * RR_LENS_N + q], gq, a);
+  }
+  double *out = lens + (row * 2 + half) * RR_LENS_PITCH;
+  if (lane < 2 * RR_LENS_N) out[i] = a;
+  if (lane >= 2 * RR_LENS_N && lane < 2 * RR_LENS_N + 2) lens[(row * 2 + (lane - 2 * RR_LENS_N)) * RR_LENS_PITCH + RR_LENS_N] = 0.0;
+}
+
 // ---- per-(tile, pv) constants, staged in shared memory (8-byte slots: a double, or the float twice) ----
 // Read with volatile loads at the point of use: they are warp-uniform broadcasts that ride in the
 // issue slots the half-rate FP64 pipe leaves free, and keeping ~25 of them out of registers is what
@@ -230,11 +273,13 @@ enum {
   K_GSCALE, K_OPK,        // (ng-1)/(1+kw), 1+k (pair)
   K_OMKS, K_K2,           // 1-k (signed), k^2 (pair)
   K_2K2, K_SCALE,         // 2 k^2, 1/(Istar ns) (pair)
+  K_INV2K, K_XOFF,        // x = z K_INV2K + K_XOFF = (z - (1-k)) / (2k): lens polynomials (pair)
+  K_LENSOK, K_PAD1,       // != 0: the staged lens polynomials hold for this k
   K_TOTAL,
   K_COUNT = K_SCALE,      // entries rr_stage_constants writes
   K_SMEM = (K_TOTAL + 3) & ~3   // 16-byte multiple in both precisions
 };
-static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_E % 2 == 0 && K_OMK2 % 2 == 0 &&
+static_assert(K_CD % 2 == 0 && K_C4 % 2 == 0 && K_E % 2 == 0 && K_OMK2 % 2 == 0 && K_INV2K % 2 == 0 &&
               K_GSCALE % 2 == 0 && K_OMKS % 2 == 0 && K_2K2 % 2 == 0, "pairs");
 template <typename T> struct Vec2T;
 template <> struct Vec2T<double> { using type = double2; };
@@ -268,7 +313,8 @@ enum { RR_SM_SYMBOL = 0, RR_SM_HELD = 1, RR_SM_ABS = 2 };
 template <typename R, int M> struct Cst {
   static constexpr int ES = (int)sizeof(R);
   static constexpr int CS = 8;                       // bytes per constant slot
-  static constexpr int OFF_FLAGS = K_SMEM * CS, OFF_ROW = OFF_FLAGS + 16;
+  static constexpr int OFF_FLAGS = K_SMEM * CS, OFF_LENS = OFF_FLAGS + 16,
+                       OFF_ROW = OFF_LENS + 2 * RR_LENS_PITCH * 8;   // lens polynomials: 2 x 14 doubles
   static constexpr int AB = (M == RR_SM_ABS ? RR_SMEM_ABS : 0);
   unsigned sb;   // RR_SM_HELD: shared-window address of rr_dyn; RR_SM_ABS: 0
   __device__ __forceinline__ Cst() {
@@ -338,6 +384,18 @@ template <typename R, int M> struct Cst {
     a = x.x;
     b = y.x;
   }
+  // coefficients 2m, 2m+1 of the lens polynomial of the half at byte offset hoff (0 or 8 PITCH)
+  static __device__ __forceinline__ double *lens() { return reinterpret_cast<double *>(rr_dyn + OFF_LENS); }
+  template <int MM> __device__ __forceinline__ void lens2(unsigned hoff, double &a, double &b) const {
+    if constexpr (M == RR_SM_SYMBOL) {
+      const double2 v = reinterpret_cast<const double2 *>(rr_dyn + OFF_LENS + hoff)[MM];
+      a = v.x;
+      b = v.y;
+    } else {
+      asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b)
+                   : "r"(sb + hoff), "n"(AB + OFF_LENS + 16 * MM));
+    }
+  }
   // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
   using R2 = typename Vec2T<R>::type;
   static __device__ __forceinline__ R2 *row() { return reinterpret_cast<R2 *>(rr_dyn + OFF_ROW); }
@@ -363,7 +421,8 @@ __global__ void rr_smem_probe_kernel(unsigned *out) {
 }
 
 template <typename R>
-__device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRPvBand &b, double du) {
+__device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRPvBand &b, double du,
+                                                   bool lens_on = false) {
   const int t = threadIdx.x;
   double v = 0.0;
   switch (t) {
@@ -386,9 +445,11 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
     case K_K2: v = b.k2; break;         case K_GSCALE: v = b.gscale; break;
     case K_OMK2: v = b.omk * b.omk; break;
     case K_2K2: v = 2.0 * b.k2; break;
+    case K_INV2K: v = 0.5 / b.k; break;  case K_XOFF: v = -(1.0 - b.k) * (0.5 / b.k); break;
+    case K_LENSOK: v = lens_on ? 1.0 : 0.0; break;
     default: break;
   }
-  if (t < K_COUNT) Cst<R, RR_SM_SYMBOL>::store(t, v);
+  if (t < K_COUNT || (t >= K_INV2K && t <= K_LENSOK)) Cst<R, RR_SM_SYMBOL>::store(t, v);
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
@@ -524,8 +585,11 @@ __device__ __forceinline__ void rr_cell(float y, int &ig, float &ag) {
   ag = y - (float)ig;
 }
 
+// kmode (block-uniform, decided once per tile): bit 0: k^2 <= 1/2; bit 1: the staged lens
+// polynomials hold (fp64 kernel, k <= RR_LENS_KMAX).
 template <typename R, int M>
-__device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, bool ksmall) {
+__device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, int kmode) {
+  const bool ksmall = (kmode & 1) != 0;
   // the constants first: their shared-memory latency passes under the square root
   R gscale, opk, omk2, afull;
   K.template pair<K_GSCALE>(gscale, opk);
@@ -540,6 +604,30 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, 
   R ap;
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
+  } else if (sizeof(R) == 8 && (kmode & 2)) {
+    // Between the contacts, polynomial form (rr_lens_poly_kernel): x = (z - (1-k)) / (2k),
+    //   a = pi k^2 - x^(3/2) g0(4x - 1)  for x <= 1/2,   a = y^(3/2) g1(4y - 1), y = 1 - x, else.
+    if constexpr (sizeof(R) == 8) {
+      double inv2k, xoff;
+      K.template pair<K_INV2K>(inv2k, xoff);
+      const double x = fma(z, inv2k, xoff);
+      const bool lo = x <= 0.5;
+      const double xx = fabs(lo ? x : 1.0 - x);
+      const unsigned hoff = lo ? 0u : (unsigned)(RR_LENS_PITCH * 8);
+      const double w = fma(xx, 4.0, -1.0);
+      const double sq = rr_sqrt3_pos(xx);
+      double c0, c1, p;
+      K.template lens2<6>(hoff, p, c1);         // c12 (c13 = 0)
+      K.template lens2<5>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      K.template lens2<4>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      K.template lens2<3>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      K.template lens2<2>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      K.template lens2<1>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      K.template lens2<0>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      const double t = xx * sq;
+      ap = lo ? fma(-t, p, afull) : t * p;
+    }
+    ++ningress;
   } else {
     // Lens of the unit disc and the disc of radius k at distance z (reading R9): two sectors minus
     // the kite.  With A = 1+k-z, B = z+1-k, C = z-1+k, D = z+1+k (all >= 0 here):
@@ -582,6 +670,7 @@ struct FluxParams {
   const void *T;        // full table (RR_TABLE_FULL) or NULL
   const void *rows;     // collapsed rows ldw[npv][npb][ng] (RR_TABLE_LAZY) or NULL
   const void *istar;
+  const double *lens;   // lens-area polynomials [npv][nkpb][2][RR_LENS_PITCH] (fp64 kernel) or NULL
   void *flux;
   unsigned long long *counters;
   int64_t npt, npv, ntiles;
@@ -669,7 +758,7 @@ __device__ __forceinline__ void rr_fill_ones_bulk(O *out, int64_t count, unsigne
 // cnt: 0 skipped, 1 circular, 2 eccentric, 3 occulting, 4 ingress, 5 sincos evaluations of the solver
 template <typename R, bool COUNT, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_mid, double hwid,
-                                          bool need_front, bool ksmall, unsigned long long *cnt) {
+                                          bool need_front, int kmode, unsigned long long *cnt) {
   // NOWRAP (block-uniform): hwid + 2 hw < 1/2, so |w| < 1/2 already and the reduction is a no-op
   const double wr = NOWRAP ? w : w - rr_round(w);
   R def = (R)0;
@@ -682,7 +771,7 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
     bool occ = z2 < K.template get<K_OPK2>();
     if (need_front) occ = occ && front;
     if (occ) {
-      def = rr_deficit<R, M>(K, z2, ing, ksmall);
+      def = rr_deficit<R, M>(K, z2, ing, kmode);
       if (COUNT) { cnt[3]++; cnt[4] += ing; }
     }
     if (COUNT) { cnt[CIRC ? 1 : 2]++; cnt[5] += it; }
@@ -713,6 +802,9 @@ __device__ __forceinline__ double rr_ld_time(uintptr_t p) {
 // given the phase 0, computes along and is masked out; nothing here can fault on its values.
 #ifndef RR_FP32_PAIRS
 #define RR_FP32_PAIRS 1
+#endif
+#ifndef RR_LENS_POLY
+#define RR_LENS_POLY 1
 #endif
 #ifndef RR_FP64_PAIRS
 #define RR_FP64_PAIRS 0   // measured, 80 registers / 6 blocks per SM: config 4 5.09 -> 5.56 ms, config 3
@@ -949,7 +1041,9 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double off0 = hw * (1.0 / ns - 1.0);         // first sub-sample offset (reading R7)
   const double hskip = hwid + hw;
   // k^2 <= 1/2 (block-uniform; lane-0 broadcast so that it stays a predicate, not a compare per use)
-  const bool ksmall = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5), 0) != 0;
+  const int kmode = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5) |
+                                                 (K.template get<K_LENSOK>() != (R)0 ? 2 : 0), 0);
+  const bool ksmall = (kmode & 1) != 0;
   if constexpr (PAIRS && !COUNT && !(CIRC && sizeof(R) == 8)) {
     if (!shuffle && count > FT) {   // two exposures per thread (tiles of <= FT exposures, the
                                     // counting build and fp64 circular tiles keep the scalar loop)
@@ -1015,7 +1109,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
             sn = s1;
             if (occ) {
               int ing = 0;
-              acc += rr_deficit<R, M>(K, z2, ing, ksmall);
+              acc += rr_deficit<R, M>(K, z2, ing, kmode);
               if (COUNT) { cnt[3]++; cnt[4] += ing; }
             }
           }
@@ -1023,7 +1117,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
         } else {
           double w = wr + off0;
           for (int s = 0; s < ns; ++s, w += du)
-            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, need_front, ksmall, cnt);
+            acc += rr_subsample<R, COUNT, CIRC, NOWRAP, M>(K, w, u_mid, hwid, need_front, kmode, cnt);
         }
         // mean of (Istar - ip ap)/Istar over ns; fp64 staged the table already times 1/(Istar ns)
         f = sizeof(R) == 8 ? (O)1 - acc : fma(-acc, scale, (O)1);
@@ -1049,7 +1143,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
           const double w0 = wr + off0;
           for (int s = sl; s < ns; s += G)
             acc += rr_subsample<R, COUNT, CIRC, false, M>(K, fma(du, (double)s, w0), u_mid, hwid, true,
-                                                          ksmall, cnt);
+                                                          kmode, cnt);
         } else if (COUNT) {
           for (int s = sl; s < ns; s += G) cnt[0]++;
         }
@@ -1204,7 +1298,11 @@ rr_flux_kernel(const FluxParams P) {
             ldw2[ig] = c;
           }
         }
-        rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns);
+        const bool lens_on = sizeof(R) == 8 && P.lens != nullptr && pb.lens_ok != 0;
+        if (lens_on && threadIdx.x < 2 * RR_LENS_PITCH)
+          Cst<R, M>::lens()[threadIdx.x] =
+              P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) + threadIdx.x];
+        rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns, lens_on);
         if (threadIdx.x == K_SCALE) Cst<R, M>::store(K_SCALE, sc_d);
         __syncthreads();
         scale = (O)K.template get<K_SCALE>();
@@ -1397,8 +1495,11 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
     wk->pvo = nullptr;
     wk->pvb = nullptr;
     wk->pv_cap = 0;
+    if (wk->lens) cudaFree(wk->lens);
+    wk->lens = nullptr;
     if (cudaMalloc(&wk->pvo, sizeof(RRPvOrbit) * npv) != cudaSuccess ||
-        cudaMalloc(&wk->pvb, sizeof(RRPvBand) * npv * c.nkpb) != cudaSuccess) {
+        cudaMalloc(&wk->pvb, sizeof(RRPvBand) * npv * c.nkpb) != cudaSuccess ||
+        cudaMalloc(&wk->lens, sizeof(double) * 2 * RR_LENS_PITCH * npv * c.nkpb) != cudaSuccess) {
       cudaGetLastError();
       return RR_EALLOC;
     }
@@ -1429,6 +1530,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.T = wk->lazy ? nullptr : wk->T;
   P.rows = wk->lazy ? wk->rows : nullptr;
   P.istar = wk->istar;
+  P.lens = (c.precision == RR_FP64 && RR_LENS_POLY) ? wk->lens : nullptr;
   P.flux = d_flux;
   P.counters = ctx->d_counters;
   P.npt = ctx->npt;
@@ -1460,7 +1562,8 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  size_t smem = (size_t)K_SMEM * 8 + 16 + (size_t)2 * P.ldw_len * (c.precision != RR_FP64 ? 4 : 8);
+  size_t smem = (size_t)K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8 +
+                (size_t)2 * P.ldw_len * (c.precision != RR_FP64 ? 4 : 8);
   smem = (smem + 15) & ~(size_t)15;
   P.ones_off = (unsigned)smem;
 #if RR_BULK_FILL
@@ -1484,6 +1587,11 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
                      2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
                      ctx->reduction != RR_REDUCE_SHUFFLE;
   const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
+  if (P.lens) {             // fp64: the lens-area polynomials of every (pv, radius ratio)
+    const int64_t nrows = npv * c.nkpb;
+    rr_lens_poly_kernel<<<(unsigned)((nrows * 32 + 255) / 256), 256, 0, st>>>(wk->pvb, nrows, wk->lens);
+    RR_LAUNCH_CHECK(ctx);
+  }
   if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory
     RR_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   kern<<<grid, FT, smem, st>>>(P);
@@ -1497,10 +1605,10 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
   if (fp32_math)
-    rr_orbit_kernel<float><<<grid, FT, K_SMEM * 8 + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
+    rr_orbit_kernel<float><<<grid, FT, K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
                                                 ctx->ntiles, npv, ctx->nsub, d_z);
   else
-    rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
+    rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;

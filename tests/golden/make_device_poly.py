@@ -77,3 +77,53 @@ if __name__ == "__main__":
     for name, (_, n, ty) in TABLES.items():
         vals = ", ".join(literal(c, ty) for c in table(name))
         print(f"__constant__ {ty} {name}[{n}] = {{{vals}}};")
+
+
+# ---- lens area on the ingress / egress interval as two polynomials (rr_lens_poly.cuh) -----------------
+# For a planet of radius k at separation z between the contacts, x = (z - (1-k)) / (2k) in (0, 1):
+#   near the second contact  a(z) = pi k^2 - x^(3/2) g0(x),      x  in [0, 1/2]
+#   near the first contact   a(z) =         y^(3/2) g1(y),  y = 1 - x in [0, 1/2]
+# with g0, g1 analytic (the area is an analytic function of the angle theta, x = sin^2(theta/2)), so
+# they are interpolated by polynomials of degree LENS_DEG at the Chebyshev nodes of [0, 1/2].  The
+# kernel evaluates the exact area at those nodes once per (parameter vector, radius ratio) and turns
+# the node values into monomial coefficients in w = 4x - 1 with the matrix LENS_M below; every
+# ingress / egress sub-sample then costs one square root and a Horner chain instead of two
+# arctangents.  Tables: nodes x_i, x_i^(-3/2), and M = (Chebyshev -> monomial) . (values -> Chebyshev).
+LENS_DEG = 12
+
+
+def lens_tables(deg=LENS_DEG):
+    n = deg + 1
+    t = [mp.cos((2 * i + 1) * mp.pi / (2 * n)) for i in range(n)]          # nodes in [-1, 1]
+    x = [(ti + 1) / 4 for ti in t]                                         # nodes in [0, 1/2]
+    xi15 = [xi ** mp.mpf("-1.5") for xi in x]
+    C = mp.matrix(n, n)                                                    # values -> Chebyshev
+    for j in range(n):
+        for i in range(n):
+            C[j, i] = (1 if j == 0 else 2) * mp.chebyt(j, t[i]) / n
+    P = mp.matrix(n, n)                                                    # P[j, m]: coefficient of w^m in T_j
+    P[0, 0] = 1
+    if n > 1:
+        P[1, 1] = 1
+    for j in range(2, n):
+        for m in range(n):
+            P[j, m] = (2 * P[j - 1, m - 1] if m > 0 else 0) - P[j - 2, m]
+    M = P.T * C                                                            # monomial[m] = sum_i M[m, i] g_i
+    return x, xi15, M
+
+
+def lens_header(deg=LENS_DEG):
+    x, xi15, M = lens_tables(deg)
+    n = deg + 1
+    out = ["// rr_lens_poly.cuh - written by tests/golden/make_device_poly.py (mpmath); do not edit.",
+           "// Tables of the polynomial form of the lens area between the contacts (see the generator).",
+           "#pragma once",
+           f"#define RR_LENS_DEG {deg}",
+           f"#define RR_LENS_N {n}",
+           f"__constant__ double RR_LENS_X[{n}] = {{" + ", ".join(repr(float(v)) for v in x) + "};",
+           f"__constant__ double RR_LENS_XI15[{n}] = {{" + ", ".join(repr(float(v)) for v in xi15) + "};",
+           f"__device__ const double RR_LENS_M[{n * n}] = {{"]
+    for m in range(n):
+        out.append("    " + ", ".join(repr(float(M[m, i])) for i in range(n)) + ",")
+    out.append("};")
+    return "\n".join(out) + "\n"
