@@ -41,12 +41,16 @@ METRIC = "transit-model evaluations/sec (pv x time x supersample)"
 UNIT = "evaluations/s"
 # B200 FP64 FMA pipe = 64 lanes/clk/SM (37.2 TFLOP/s nominal at 148 SMs, 1965 MHz)
 FP64_LANES_PER_SM, FP32_LANES_PER_SM, SM_COUNT = 64, 128, 148
-# algorithmic FMA-pipe instructions per unit of each class of the flux kernel, counted in
-# the SASS of the committed build (DFMA/DMUL/DADD in fp64 mode; FFMA/FMUL/FADD in fp32 and mixed
+# ALGORITHMIC FMA-pipe instructions per unit of each class of the flux kernel: the
+# count of the direct formulation (Kepler solve by Halley steps on d = E - E_tr, analytic lens area with
+# its two arctangents, the paper's cc_intersection_area), counted in the SASS of the build that
+# evaluates exactly that (profiles/r02c; DFMA/DMUL/DADD in fp64 mode, FFMA/FMUL/FADD in fp32 and mixed
 # mode, where the fp64 phase arithmetic runs on the other pipe and is not counted).  Compares, selects,
 # conversions, loads and the MUFU seeds are not counted; sub-samples in merged out-of-window fill runs
-# cost no arithmetic.  The table sums to 98 % of the arithmetic thread-instructions ncu counts
-# (profiles/flux_kernel_ncu.csv), i.e. it does not claim work the kernel does not execute.
+# cost no arithmetic.  `roofline.frac` = this work / time / peak: the EFFECTIVE fraction.  Where the
+# kernel reaches the same result with fewer instructions (fp64: the lens area between the contacts from
+# per-pv polynomials, EXECUTED_OPS below) the line says so: `counter_based.frac` is what the pipe
+# really executes, `algorithmic_over_executed` the ratio.
 CIRC_PER_SUBSAMPLE, CIRC_PER_EXPOSURE = 6.0, 22.0   # fp64 circular path: rotation + z^2; phase + sincos
 ALG_OPS = {
     "fp64": dict(skipped=1, circular=28, eccentric_fixed=23, solver_iter=30, occulting=11,
@@ -54,6 +58,8 @@ ALG_OPS = {
     "fp32": dict(skipped=0, circular=7, eccentric_fixed=20, solver_iter=24, occulting=11,
                  ingress=45),
 }
+# what the committed fp64 kernel executes per unit where that differs from the direct formulation
+EXECUTED_OPS = {"fp64": dict(ingress=24)}
 
 
 def parse_args():
@@ -444,7 +450,12 @@ def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, 
                          "pipe_cycles_active_pct_ncu": float(cap["pipe_active_pct"]),
                          "issue_active_pct_ncu": float(cap["issue_active_pct"]),
                          "capture": cap["capture"]}
+    exe_ops = dict(ops)
+    exe_ops.update(EXECUTED_OPS.get("fp64" if precision == "fp64" else "fp32", {}))
+    exe_fma = alg_fma + sum(counts[c] * (exe_ops[c] - ops[c]) for c in ("ingress",))
     roofline.update({
+        "executed_ops_per_unit": exe_ops, "executed_fma_by_table": int(exe_fma),
+        "executed_frac_by_table": 2.0 * exe_fma / t_flux / 1e12 / alu_peak_tflops,
         "kernel": "rr_flux_kernel", "kernel_ms": t["ms_flux"],
         "ld_table_kernel_ms": t["ms_table"] + t["ms_rows"],
         "ld_table_parts_ms": {"rr_build_ld_table": t["ms_table"], "rows_in_rr_evaluate": t["ms_rows"]},

@@ -62,7 +62,8 @@ TABLES = {           # name in rr_math.cuh -> (generator, entries, float type)
 
 def table(name):
     gen, n, _ = TABLES[name]
-    return gen(n)
+    with mp.workdps(60):
+        return gen(n)
 
 
 def literal(c, ty):
@@ -93,6 +94,11 @@ LENS_DEG = 12
 
 
 def lens_tables(deg=LENS_DEG):
+    with mp.workdps(60):                       # whatever precision the caller has set
+        return _lens_tables(deg)
+
+
+def _lens_tables(deg):
     n = deg + 1
     t = [mp.cos((2 * i + 1) * mp.pi / (2 * n)) for i in range(n)]          # nodes in [-1, 1]
     x = [(ti + 1) / 4 for ti in t]                                         # nodes in [0, 1/2]
@@ -109,6 +115,10 @@ def lens_tables(deg=LENS_DEG):
         for m in range(n):
             P[j, m] = (2 * P[j - 1, m - 1] if m > 0 else 0) - P[j - 2, m]
     M = P.T * C                                                            # monomial[m] = sum_i M[m, i] g_i
+    for m in range(n):                                                     # entries that are exactly 0
+        for i in range(n):
+            if abs(M[m, i]) < mp.mpf("1e-40"):
+                M[m, i] = mp.mpf(0)
     return x, xi15, M
 
 

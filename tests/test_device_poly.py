@@ -134,3 +134,73 @@ def test_packed_tables_repeat_the_scalar_ones(name):
 
     for (a, b), c in zip(pairs, scalar):
         assert val(a) == val(b) == c, (name, a, b, c)
+
+
+# ---- lens area between the contacts as polynomials (csrc/rr_lens_poly.cuh) ------------------------------
+LENS_SRC = open(os.path.join(ROOT, "paper_2009_08500_b200", "csrc", "rr_lens_poly.cuh")).read()
+
+
+def _lens_table(name):
+    m = re.search(name + r"\[(\d+)\]\s*=\s*\{(.*?)\};", LENS_SRC, re.S)
+    assert m, name
+    vals = [float(t) for t in m.group(2).replace("\n", " ").split(",") if t.strip()]
+    assert len(vals) == int(m.group(1))
+    return np.array(vals)
+
+
+def test_lens_tables_equal_the_generator():
+    assert LENS_SRC == gen.lens_header()          # the committed header IS the generator's output
+    x, xi15, M = gen.lens_tables()
+    n = gen.LENS_DEG + 1
+    assert np.array_equal(_lens_table("RR_LENS_X"), [float(v) for v in x])
+    assert np.array_equal(_lens_table("RR_LENS_XI15"), [float(v) for v in xi15])
+    assert np.array_equal(_lens_table("RR_LENS_M").reshape(n, n),
+                          [[float(M[j, i]) for i in range(n)] for j in range(n)])
+
+
+def _lens_exact_mp(k, z):
+    k, z = mp.mpf(k), mp.mpf(z)
+    if z >= 1 + k:
+        return mp.mpf(0)
+    if z <= 1 - k:
+        return mp.pi * k * k
+    a1 = mp.acos((z * z + 1 - k * k) / (2 * z))
+    a2 = mp.acos((z * z + k * k - 1) / (2 * z * k))
+    return a1 + k * k * a2 - mp.sqrt((-z + 1 + k) * (z + 1 - k) * (z - 1 + k) * (z + 1 + k)) / 2
+
+
+@pytest.mark.parametrize("k", [0.01, 0.05, 0.1, 0.2, 0.3, 0.32])
+def test_lens_polynomial_reproduces_the_area(k):
+    """The pipeline of rr_lens_poly_kernel + rr_deficit restated in float64 (exact area at the nodes
+    by the half-angle form, node values -> monomial coefficients through RR_LENS_M, Horner in
+    w = 4x - 1, a = pi k^2 - x^(3/2) g0 or y^(3/2) g1) against the textbook two-sector-minus-kite area
+    in 40-digit arithmetic, between the contacts and right at them: <= 2.5e-13."""
+    mp.mp.dps = 40
+    X, XI15 = _lens_table("RR_LENS_X"), _lens_table("RR_LENS_XI15")
+    n = X.size
+    M = _lens_table("RR_LENS_M").reshape(n, n)
+    full = np.pi * k * k
+
+    def area64(z):                                  # float64, as the device states it
+        A, B, C, D = 1 + k - z, z + 1 - k, z - 1 + k, z + 1 + k
+        kite = np.sqrt(abs(A * B) * abs(C * D))
+        return 2 * np.arctan2(kite, B * D) + 2 * k * k * np.arctan2(kite, abs(C * D)) - kite / 2
+
+    g0 = np.array([(full - area64(1 - k + 2 * k * x)) for x in X]) * XI15
+    g1 = np.array([area64(1 + k - 2 * k * x) for x in X]) * XI15
+    a0, a1 = M @ g0, M @ g1
+    xs = np.concatenate([np.linspace(0.0, 1.0, 801), 10.0 ** np.linspace(-14, -3, 40),
+                         1 - 10.0 ** np.linspace(-14, -3, 40)])
+    worst = 0.0
+    for x in xs:
+        z = 1 - k + 2 * k * x
+        lo = x <= 0.5
+        xx = abs(x if lo else 1 - x)
+        w = 4 * xx - 1
+        p = 0.0
+        for c in (a0 if lo else a1)[::-1]:
+            p = p * w + c
+        t = xx * np.sqrt(xx)
+        ap = full - t * p if lo else t * p
+        worst = max(worst, abs(ap - float(_lens_exact_mp(k, z))))
+    assert worst <= 2.5e-13, worst
