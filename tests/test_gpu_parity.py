@@ -1218,3 +1218,39 @@ def test_step_is_cuda_graph_capturable(rr):
     assert np.max(np.abs(flux.cpu().numpy() - want2)) <= TOL64
     assert np.max(np.abs(want2 - want)) > 1e-5
     gm.close()
+
+
+def test_lens_polynomial_radius_ratio_edges(rr):
+    """The fp64 kernel takes the lens area between the contacts from per-pv polynomials for k <= 0.32
+    and from the two-arctangent form above: radius ratios from 0.005 to just past the switch, in the
+    direct model (any k > 0), ingress and egress densely sampled (2e-5 d steps), central to grazing
+    impact parameters; flux against the oracle, which only knows the arctangent form.  The observed
+    agreement is ~1e-14 on both sides of the switch."""
+    ks = np.array([0.005, 0.01, 0.05, 0.15, 0.3, 0.3199, 0.32, 0.3201, 0.35, 0.5])
+    n = ks.size
+    rng = np.random.default_rng(5)
+    e = np.where(np.arange(n) % 2 == 0, 0.0, rng.uniform(0.1, 0.5, n))
+    w = rng.uniform(0, 2 * np.pi, n)
+    a = rng.uniform(6.0, 12.0, n)
+    b = np.array([0.0, 0.5, 0.9, 0.3, 0.7, 0.1, 0.6, 0.95, 0.2, 1.2])
+    cosi = b * (1 + e * np.sin(w)) / (a * (1 - e * e))
+    pv = np.stack([ks, np.zeros(n), rng.uniform(2.5, 4.0, n), a, np.arccos(cosi), e, w], axis=1)
+    t1 = np.arange(-0.16, 0.16, 2e-5)
+    times = np.concatenate([t1, t1[::7]])
+    lc = np.concatenate([np.zeros(t1.size), np.ones(t1[::7].size)]).astype(np.int32)
+    pbs, nss, ets = [0, 0], [1, 3], [0.0, 0.002]
+    mc = workloads.ModelConfig()
+    coeffs = np.tile(np.array([[[0.35, 0.25]]]), (n, 1, 1))
+    om = oracle.OracleDirectModel.from_config(mc)
+    want, _ = om.evaluate(times, lc, pbs, nss, ets, pv,
+                          workloads.sample_profile("quadratic", coeffs, om.mu), nthreads=0)
+    gm = rr.RoadRunner.from_config(mc)
+    rr.rr_set_table_mode(gm.ctx, rr.RR_TABLE_DIRECT)
+    gm.set_data(times, lc, pbs, nss, ets)
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    got = gm.evaluate(pv).cpu().numpy()
+    err = np.max(np.abs(got - want), axis=1)
+    assert np.all((want < 1).sum(axis=1) > 1000)
+    assert np.max(err) <= TOL64, [float(f"{x:.1e}") for x in err]
+    assert np.max(err) <= 1e-12, [float(f"{x:.1e}") for x in err]      # what the arithmetic gives
+    gm.close()
