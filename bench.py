@@ -60,6 +60,7 @@ ALG_OPS = {
 }
 # what the committed fp64 kernel executes per unit where that differs from the direct formulation
 EXECUTED_OPS = {"fp64": dict(ingress=24)}
+ZPOLY_OPS = 15      # an eccentric sub-sample through the z^2 polynomials: t, w, Horner 12, |.| + tiny
 
 
 def parse_args():
@@ -357,12 +358,21 @@ class Case:
         return 1e3 * e0.elapsed_time(e1) / n
 
     def class_counts(self):
-        """Class counts of one evaluation (untimed launch with the kernel's counters on)."""
+        """Class counts of one evaluation (untimed launches with the kernel's counters on): those of
+        the direct formulation (every eccentric sub-sample solves Kepler's equation: the algorithmic
+        work) plus `eccentric_poly`, the sub-samples the committed kernel takes from the per-pv z^2
+        polynomials instead."""
         rr = self.rr
         rr.rr_enable_counters(self.ctx, True)
+        rr.rr_set_orbit_poly(self.ctx, False)
         rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
         counts = rr.rr_get_counters(self.ctx)
+        rr.rr_set_orbit_poly(self.ctx, True)
+        rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
+        as_run = rr.rr_get_counters(self.ctx)
         rr.rr_enable_counters(self.ctx, False)
+        counts["eccentric_poly"] = as_run["eccentric_poly"]
+        counts["solver_iters_as_run"] = as_run["solver_iters"]
         return counts
 
     def sample_error(self, n_pv=8, n_cols=600):
@@ -453,6 +463,10 @@ def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, 
     exe_ops = dict(ops)
     exe_ops.update(EXECUTED_OPS.get("fp64" if precision == "fp64" else "fp32", {}))
     exe_fma = alg_fma + sum(counts[c] * (exe_ops[c] - ops[c]) for c in ("ingress",))
+    if precision == "fp64" and counts.get("eccentric_poly"):
+        # sub-samples taken from the z^2 polynomials: ZPOLY_OPS instead of the fixed part and their solves
+        exe_fma += (counts["eccentric_poly"] * (ZPOLY_OPS - ops["eccentric_fixed"])
+                    - (counts["solver_iters"] - counts["solver_iters_as_run"]) * ops["solver_iter"])
     roofline.update({
         "executed_ops_per_unit": exe_ops, "executed_fma_by_table": int(exe_fma),
         "executed_frac_by_table": 2.0 * exe_fma / t_flux / 1e12 / alu_peak_tflops,

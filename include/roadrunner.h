@@ -173,6 +173,15 @@ int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on);
  * node).  k_threshold = 0 (default) switches it off.  Needs RR_TABLE_LAZY or RR_TABLE_DIRECT
  * (rr_evaluate returns RR_ESTATE on a full table).  Takes effect at the next rr_evaluate.        */
 int rr_set_small_planet(rr_ctx *ctx, double k_threshold);
+/* Orbit evaluation of the fp64 flux kernel for eccentric orbits (default on != 0): per parameter
+ * vector, z^2 over the two halves of its transit window is fitted once per rr_evaluate by two
+ * degree-12 polynomials through 26 exact Kepler solves, and every sub-sample
+ * evaluates the polynomial instead of solving Kepler's equation; a parameter vector whose polynomials
+ * have not converged (Chebyshev tail above 1e-12: wide windows of close-in, very eccentric orbits)
+ * and every fp32 / mixed kernel keep the per-sub-sample solve.  Difference to the per-sub-sample
+ * solve: <= ~1e-11 in z^2, ~1e-13 in flux (tested).  on = 0: always solve.  Takes effect at the next
+ * rr_evaluate.                                                                                    */
+int rr_set_orbit_poly(rr_ctx *ctx, int32_t on);
 /* Diagnostics: device pointers to the full table (built on demand in lazy mode; synchronous) and
  * Istar of the last rr_build_ld_table (ctx precision), or NULL.                                 */
 const void *rr_table_ptr(rr_ctx *ctx);
@@ -239,9 +248,9 @@ int rr_evaluate_host(rr_ctx *ctx, const void *h_ldp, const double *h_pv, int32_t
  * counted: total - [0] - [1] - [2]), [1] evaluated circular, [2] evaluated eccentric, [3] of those
  * with z < 1+k in front of the star, [4] of those in ingress/egress (lens area), [5] sincos
  * evaluations of the Kepler solver, [6] tiles (per pv) filled without evaluation, [7] tiles (per
- * pv) evaluated.  Synchronous. */
+ * pv) evaluated, [8] of [2] those evaluated through the orbit polynomials (no solve).  Synchronous. */
 int rr_enable_counters(rr_ctx *ctx, int32_t on);
-int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts /*[8]*/);
+int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts /*[9]*/);
 /* Number of kernel launches the library has made on this ctx since creation.                     */
 int64_t rr_launch_count(const rr_ctx *ctx);
 /* Device time of the kernels inside rr_evaluate, by CUDA events recorded on the caller's stream

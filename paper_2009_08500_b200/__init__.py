@@ -36,7 +36,7 @@ SYMBOLS = (
     "rr_set_reduction", "rr_evaluate_host", "rr_enable_counters", "rr_get_counters",
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
-    "rr_set_small_planet", "rr_build_ld_table_law", "rr_math_probe",
+    "rr_set_small_planet", "rr_build_ld_table_law", "rr_math_probe", "rr_set_orbit_poly",
 )
 PROBE_OPS = {"sqrt3": 0, "sqrt": 1, "div3": 2, "rcp": 3, "atan_t": 4, "atan_quadrant": 5,
              "atan2_pos": 6, "sincosm1": 7, "cell": 8}
@@ -100,6 +100,7 @@ def load() -> C.CDLL:
         "rr_set_table_mode": (C.c_int, [_VP, _I32]),
         "rr_get_rows": (C.c_int, [_VP, _VP]),
         "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
+        "rr_set_orbit_poly": (C.c_int, [_VP, _I32]),
         "rr_set_small_planet": (C.c_int, [_VP, _DBL]),
         "rr_build_ld_table_law": (C.c_int, [_VP, _I32, _VP, _I32, _I64, _VP]),
         "rr_math_probe": (C.c_int, [_I32, _I32, _VP, _VP, _I64, _VP, _VP, _VP]),
@@ -341,6 +342,10 @@ def rr_set_small_planet(ctx: int, k_threshold: float):
     _check(load().rr_set_small_planet(ctx, float(k_threshold)), "rr_set_small_planet")
 
 
+def rr_set_orbit_poly(ctx: int, on: bool):
+    _check(load().rr_set_orbit_poly(ctx, int(bool(on))), "rr_set_orbit_poly")
+
+
 def rr_set_mean_k_weights(ctx: int, on: bool):
     _check(load().rr_set_mean_k_weights(ctx, int(bool(on))), "rr_set_mean_k_weights")
 
@@ -403,11 +408,11 @@ def rr_enable_counters(ctx: int, on: bool):
 
 
 COUNTER_NAMES = ("skipped", "circular", "eccentric", "occulting", "ingress", "solver_iters",
-                 "tiles_filled", "tiles_evaluated")
+                 "tiles_filled", "tiles_evaluated", "eccentric_poly")
 
 
 def rr_get_counters(ctx: int) -> dict:
-    out = np.zeros(8, np.int64)
+    out = np.zeros(9, np.int64)
     _check(load().rr_get_counters(ctx, out.ctypes.data), "rr_get_counters")
     return dict(zip(COUNTER_NAMES, (int(x) for x in out)))
 

@@ -25,6 +25,7 @@ void free_work(RRWork *w) {
   if (w->pvo) cudaFree(w->pvo);
   if (w->pvb) cudaFree(w->pvb);
   if (w->lens) cudaFree(w->lens);
+  if (w->zpoly) cudaFree(w->zpoly);
   if (w->ldp) cudaFree(w->ldp);
   if (w->rows) cudaFree(w->rows);
   if (w->bk) cudaFree(w->bk);
@@ -107,12 +108,13 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   for (auto &w : ctx->work) w.table_npv = -1;
   ctx->reduction = RR_REDUCE_AUTO;
   ctx->table_mode = RR_TABLE_LAZY;
+  ctx->orbit_poly = 1;
   int rc = RR_OK;
   cudaError_t e = cudaGetDevice(&ctx->device);
   if (e == cudaSuccess)
     e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
-  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * 8);
-  if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, sizeof(unsigned long long) * 8);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * 16);
+  if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, sizeof(unsigned long long) * 16);
   if (e != cudaSuccess) rc = RR_ECUDA_BASE - (int)e;
   if (rc == RR_OK) rc = rr_smem_probe(&ctx->smem_abs);
   if (rc == RR_OK) rc = rr_geometry_build(ctx);
@@ -250,6 +252,12 @@ int rr_set_small_planet(rr_ctx *ctx, double k_threshold) {
 int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on) {
   if (!ctx) return RR_ENULL;
   ctx->mean_k = on ? 1 : 0;
+  return RR_OK;
+}
+
+int rr_set_orbit_poly(rr_ctx *ctx, int32_t on) {
+  if (!ctx) return RR_ENULL;
+  ctx->orbit_poly = on ? 1 : 0;
   return RR_OK;
 }
 
@@ -454,7 +462,7 @@ int rr_enable_counters(rr_ctx *ctx, int32_t on) {
 int rr_get_counters(const rr_ctx *ctx, int64_t *h_counts) {
   if (!ctx || !h_counts) return RR_ENULL;
   RR_CUDA(cudaDeviceSynchronize());
-  RR_CUDA(cudaMemcpy(h_counts, ctx->d_counters, sizeof(int64_t) * 8, cudaMemcpyDeviceToHost));
+  RR_CUDA(cudaMemcpy(h_counts, ctx->d_counters, sizeof(int64_t) * 9, cudaMemcpyDeviceToHost));
   return RR_OK;
 }
 

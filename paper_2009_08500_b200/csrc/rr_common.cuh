@@ -48,6 +48,8 @@ struct RRPvOrbit {
   double aci2;          // a^2 cos^2 i:  z^2 = x^2 + aci2 y^2
   int32_t status;       // RR_PV_* bits; != 0 -> NaN row
   int32_t circular;     // e == 0
+  int32_t zpoly_ok;     // 1: z^2 over the transit window from the fitted polynomials (rr_zpoly_kernel)
+  int32_t pad;
 };
 
 // Per (parameter vector, k-band): radius-ratio constants.
@@ -84,6 +86,7 @@ struct RRWork {
   RRPvOrbit *pvo;
   RRPvBand *pvb;
   double *lens;             // [npv][nkpb][2][RR_LENS_PITCH]: lens-area polynomials (fp64 kernel)
+  double *zpoly;            // [npv][2][RR_LENS_PITCH]: z^2 over the two halves of the transit window
   int64_t pv_cap;
 };
 #define RR_LENS_PITCH 14    // 13 coefficients + 1 pad: 16-byte multiples per half
@@ -115,6 +118,7 @@ struct rr_ctx {
   int32_t reduction;
   int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL | RR_TABLE_DIRECT
   int32_t mean_k;       // 1: LD weights at the mean k of the passbands
+  int32_t orbit_poly;   // 1 (default): fp64 kernel takes z^2 from per-pv polynomials where they hold
   double k_small;       // small-planet approximation for kw <= k_small; 0: off
   // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
   RRWork work[3];

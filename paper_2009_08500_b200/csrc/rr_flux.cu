@@ -204,6 +204,8 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
   }
   po.u_mid = 0.5 * (u_lo + u_hi);
   po.hwid = 0.5 * (u_hi - u_lo);
+  po.zpoly_ok = 0;
+  po.pad = 0;
   pvo[v] = po;
 }
 
@@ -274,7 +276,8 @@ enum {
   K_OMKS, K_K2,           // 1-k (signed), k^2 (pair)
   K_2K2, K_SCALE,         // 2 k^2, 1/(Istar ns) (pair)
   K_INV2K, K_XOFF,        // x = z K_INV2K + K_XOFF = (z - (1-k)) / (2k): lens polynomials (pair)
-  K_LENSOK, K_PAD1,       // != 0: the staged lens polynomials hold for this k
+  K_LENSOK, K_ZOK,        // != 0: the staged lens polynomials hold for this k / the z^2 polynomials for this pv
+  K_INVHW, K_PAD2,        // 1 / hwid
   K_TOTAL,
   K_COUNT = K_SCALE,      // entries rr_stage_constants writes
   K_SMEM = (K_TOTAL + 3) & ~3   // 16-byte multiple in both precisions
@@ -314,7 +317,8 @@ template <typename R, int M> struct Cst {
   static constexpr int ES = (int)sizeof(R);
   static constexpr int CS = 8;                       // bytes per constant slot
   static constexpr int OFF_FLAGS = K_SMEM * CS, OFF_LENS = OFF_FLAGS + 16,
-                       OFF_ROW = OFF_LENS + 2 * RR_LENS_PITCH * 8;   // lens polynomials: 2 x 14 doubles
+                       OFF_ZPOLY = OFF_LENS + 2 * RR_LENS_PITCH * 8,    // lens polynomials: 2 x 14 doubles
+                       OFF_ROW = OFF_ZPOLY + 2 * RR_LENS_PITCH * 8;    // z^2 polynomials: 2 x 14 doubles
   static constexpr int AB = (M == RR_SM_ABS ? RR_SMEM_ABS : 0);
   unsigned sb;   // RR_SM_HELD: shared-window address of rr_dyn; RR_SM_ABS: 0
   __device__ __forceinline__ Cst() {
@@ -386,15 +390,29 @@ template <typename R, int M> struct Cst {
   }
   // coefficients 2m, 2m+1 of the lens polynomial of the half at byte offset hoff (0 or 8 PITCH)
   static __device__ __forceinline__ double *lens() { return reinterpret_cast<double *>(rr_dyn + OFF_LENS); }
-  template <int MM> __device__ __forceinline__ void lens2(unsigned hoff, double &a, double &b) const {
+  template <int MM, int OFF = OFF_LENS>
+  __device__ __forceinline__ void lens2(unsigned hoff, double &a, double &b) const {
     if constexpr (M == RR_SM_SYMBOL) {
-      const double2 v = reinterpret_cast<const double2 *>(rr_dyn + OFF_LENS + hoff)[MM];
+      const double2 v = reinterpret_cast<const double2 *>(rr_dyn + OFF + hoff)[MM];
       a = v.x;
       b = v.y;
     } else {
       asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b)
-                   : "r"(sb + hoff), "n"(AB + OFF_LENS + 16 * MM));
+                   : "r"(sb + hoff), "n"(AB + OFF + 16 * MM));
     }
+  }
+  static __device__ __forceinline__ double *zpoly() { return reinterpret_cast<double *>(rr_dyn + OFF_ZPOLY); }
+  // degree-12 polynomial of the half at byte offset hoff of the region OFF (lens or z^2), at w
+  template <int OFF> __device__ __forceinline__ double poly12(unsigned hoff, double w) const {
+    double c0, c1, p;
+    lens2<6, OFF>(hoff, p, c1);               // c12 (c13 = 0)
+    lens2<5, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    lens2<4, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    lens2<3, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    lens2<2, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    lens2<1, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    lens2<0, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+    return p;
   }
   // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
   using R2 = typename Vec2T<R>::type;
@@ -422,7 +440,7 @@ __global__ void rr_smem_probe_kernel(unsigned *out) {
 
 template <typename R>
 __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRPvBand &b, double du,
-                                                   bool lens_on = false) {
+                                                   bool lens_on = false, bool zpoly_on = false) {
   const int t = threadIdx.x;
   double v = 0.0;
   switch (t) {
@@ -447,9 +465,11 @@ __device__ __forceinline__ void rr_stage_constants(const RRPvOrbit &o, const RRP
     case K_2K2: v = 2.0 * b.k2; break;
     case K_INV2K: v = 0.5 / b.k; break;  case K_XOFF: v = -(1.0 - b.k) * (0.5 / b.k); break;
     case K_LENSOK: v = lens_on ? 1.0 : 0.0; break;
+    case K_ZOK: v = zpoly_on ? 1.0 : 0.0; break;
+    case K_INVHW: v = 1.0 / o.hwid; break;
     default: break;
   }
-  if (t < K_COUNT || (t >= K_INV2K && t <= K_LENSOK)) Cst<R, RR_SM_SYMBOL>::store(t, v);
+  if (t < K_COUNT || (t >= K_INV2K && t <= K_INVHW)) Cst<R, RR_SM_SYMBOL>::store(t, v);
 }
 
 // ---- kernel 2, robust path: bracketed Halley / bisection for G(d) = 0, any dM ------------------------
@@ -486,6 +506,55 @@ __device__ RR_ROBUST_INLINE int rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out
   *s_out = s + c * dd - s * hdd2;
   *cm1_out = cm1 - s * dd - c * hdd2;
   return it;
+}
+
+// ---- z^2 over the transit window as two polynomials per parameter vector (fp64 kernel) ---------------
+// For an eccentric orbit with a transit window [u_mid - hwid, u_mid + hwid] the squared separation is
+// an analytic function of the phase; on each half of the window, t' = |w| / hwid in [0, 1], it is
+// interpolated by a degree-12 polynomial at the Chebyshev nodes (the tables of the lens polynomials:
+// nodes 2 RR_LENS_X, matrix RR_LENS_M).  One warp per parameter vector: lanes 0..12 / 13..25 solve
+// Kepler's equation exactly (bracketed Halley) at the nodes of the two halves.
+// The polynomials are used only if their Chebyshev tails |c12| + |c11| are below RR_ZPOLY_TAIL
+// (wide windows of close-in, very eccentric orbits do not converge: those pvs keep the per-sub-sample
+// solve).  Per sub-sample the flux kernel then pays 15 FP64 instructions instead of 53.
+#ifndef RR_ZPOLY_TAIL
+#define RR_ZPOLY_TAIL 1e-12
+#endif
+__global__ void rr_zpoly_kernel(RRPvOrbit *__restrict__ pvo, int64_t npv, double *__restrict__ zpoly) {
+  const int64_t v = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (v >= npv) return;
+  const RRPvOrbit po = pvo[v];
+  if (po.status || po.circular || !(po.hwid < 0.49)) return;     // (zpoly_ok stays 0)
+  const int half = lane >= RR_LENS_N ? 1 : 0, i = lane - half * RR_LENS_N;
+  double g = 0.0;
+  if (lane < 2 * RR_LENS_N) {
+    const double w = (half ? 2.0 : -2.0) * RR_LENS_X[i] * po.hwid;  // phase from the window centre
+    const double dM = RR_TWOPI * (w + po.u_mid);
+    double s, cm1;
+    rr_kepler_robust<double>(po.e, po.sE, po.cE, dM, &s, &cm1);
+    const double xs = fma(po.X1, cm1, po.X2 * s);
+    const double ys = po.Y0 + fma(po.Y1, cm1, po.Y2 * s);
+    g = fma(xs, xs, po.aci2 * ys * ys);
+  }
+  double a = 0.0;
+#pragma unroll
+  for (int q = 0; q < RR_LENS_N; ++q) {
+    const double gq = __shfl_sync(0xffffffffu, g, half * RR_LENS_N + q);
+    if (lane < 2 * RR_LENS_N) a = fma(RR_LENS_M[i * RR_LENS_N + q], gq, a);
+  }
+  // Chebyshev tail from the two leading monomial coefficients: c12 = a12 / 2^11, c11 = a11 / 2^10
+  double tail = 0.0;
+  if (lane < 2 * RR_LENS_N && i == RR_LENS_N - 1) tail = fabs(a) * (1.0 / 2048.0);
+  if (lane < 2 * RR_LENS_N && i == RR_LENS_N - 2) tail = fabs(a) * (1.0 / 1024.0);
+  if (!(a == a) || fabs(a) > 1e300) tail = 1.0;                   // not finite: no polynomial
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) tail += __shfl_xor_sync(0xffffffffu, tail, o);
+  double *out = zpoly + (v * 2 + half) * RR_LENS_PITCH;
+  if (lane < 2 * RR_LENS_N) out[i] = a;
+  if (lane >= 2 * RR_LENS_N && lane < 2 * RR_LENS_N + 2)
+    zpoly[(v * 2 + (lane - 2 * RR_LENS_N)) * RR_LENS_PITCH + RR_LENS_N] = 0.0;
+  if (lane == 0 && tail <= RR_ZPOLY_TAIL) pvo[v].zpoly_ok = 1;
 }
 
 // ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
@@ -616,14 +685,7 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, 
       const unsigned hoff = lo ? 0u : (unsigned)(RR_LENS_PITCH * 8);
       const double w = fma(xx, 4.0, -1.0);
       const double sq = rr_sqrt3_pos(xx);
-      double c0, c1, p;
-      K.template lens2<6>(hoff, p, c1);         // c12 (c13 = 0)
-      K.template lens2<5>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
-      K.template lens2<4>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
-      K.template lens2<3>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
-      K.template lens2<2>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
-      K.template lens2<1>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
-      K.template lens2<0>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
+      const double p = K.template poly12<Cst<R, M>::OFF_LENS>(hoff, w);
       const double t = xx * sq;
       ap = lo ? fma(-t, p, afull) : t * p;
     }
@@ -671,6 +733,7 @@ struct FluxParams {
   const void *rows;     // collapsed rows ldw[npv][npb][ng] (RR_TABLE_LAZY) or NULL
   const void *istar;
   const double *lens;   // lens-area polynomials [npv][nkpb][2][RR_LENS_PITCH] (fp64 kernel) or NULL
+  const double *zpoly;  // z^2 polynomials [npv][2][RR_LENS_PITCH] (fp64 kernel) or NULL
   void *flux;
   unsigned long long *counters;
   int64_t npt, npv, ntiles;
@@ -763,9 +826,20 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
   const double wr = NOWRAP ? w : w - rr_round(w);
   R def = (R)0;
   if (fabs(wr) <= hwid) {
-    bool front;
+    bool front = true;
     int it = 0, ing = 0;
-    R z2 = rr_separation2<R, CIRC, M>(K, wr + u_mid, front, it);
+    R z2;
+    if (!CIRC && sizeof(R) == 8 && (kmode & 4)) {
+      // z^2 from the pv's polynomials over its transit window (rr_zpoly_kernel): t' = |w| / hwid
+      if constexpr (!CIRC && sizeof(R) == 8) {
+        const double t = wr * K.template get<K_INVHW>();
+        const unsigned hoff = t < 0.0 ? 0u : (unsigned)(RR_LENS_PITCH * 8);
+        z2 = fabs(K.template poly12<Cst<R, M>::OFF_ZPOLY>(hoff, fma(fabs(t), 2.0, -1.0))) + RR_TINY_D;
+      }
+      if (COUNT) cnt[6]++;
+    } else {
+      z2 = rr_separation2<R, CIRC, M>(K, wr + u_mid, front, it);
+    }
     // inside a transit window (hwid < 1/2) the true anomaly is within a quarter turn of
     // conjunction: the planet is in front, and the test is only needed without a window
     bool occ = z2 < K.template get<K_OPK2>();
@@ -805,6 +879,9 @@ __device__ __forceinline__ double rr_ld_time(uintptr_t p) {
 #endif
 #ifndef RR_LENS_POLY
 #define RR_LENS_POLY 1
+#endif
+#ifndef RR_ZPOLY
+#define RR_ZPOLY 1
 #endif
 #ifndef RR_FP64_PAIRS
 #define RR_FP64_PAIRS 0   // measured, 80 registers / 6 blocks per SM: config 4 5.09 -> 5.56 ms, config 3
@@ -1042,7 +1119,8 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
   const double hskip = hwid + hw;
   // k^2 <= 1/2 (block-uniform; lane-0 broadcast so that it stays a predicate, not a compare per use)
   const int kmode = __shfl_sync(0xffffffffu, (int)(K.template get<K_K2>() <= (R)0.5) |
-                                                 (K.template get<K_LENSOK>() != (R)0 ? 2 : 0), 0);
+                                                 (K.template get<K_LENSOK>() != (R)0 ? 2 : 0) |
+                                                 (K.template get<K_ZOK>() != (R)0 ? 4 : 0), 0);
   const bool ksmall = (kmode & 1) != 0;
   if constexpr (PAIRS && !COUNT && !(CIRC && sizeof(R) == 8)) {
     if (!shuffle && count > FT) {   // two exposures per thread (tiles of <= FT exposures, the
@@ -1181,7 +1259,7 @@ rr_flux_kernel(const FluxParams P) {
   const Cst<R, M> K;
   using R2 = typename Cst<R, M>::R2;
   unsigned *tflags = Cst<R, M>::flags();
-  unsigned long long cnt[6] = {0, 0, 0, 0, 0, 0};
+  unsigned long long cnt[7] = {0, 0, 0, 0, 0, 0, 0};
   unsigned long long cfill = 0, ceval = 0;
 
 #if RR_BULK_FILL
@@ -1302,7 +1380,11 @@ rr_flux_kernel(const FluxParams P) {
         if (lens_on && threadIdx.x < 2 * RR_LENS_PITCH)
           Cst<R, M>::lens()[threadIdx.x] =
               P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) + threadIdx.x];
-        rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns, lens_on);
+        const bool zpoly_on = sizeof(R) == 8 && P.zpoly != nullptr && po.zpoly_ok != 0;
+        if (zpoly_on && threadIdx.x >= 32 && threadIdx.x < 32 + 2 * RR_LENS_PITCH)
+          Cst<R, M>::zpoly()[threadIdx.x - 32] =
+              P.zpoly[(int64_t)v * (2 * RR_LENS_PITCH) + threadIdx.x - 32];
+        rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns, lens_on, zpoly_on);
         if (threadIdx.x == K_SCALE) Cst<R, M>::store(K_SCALE, sc_d);
         __syncthreads();
         scale = (O)K.template get<K_SCALE>();
@@ -1333,10 +1415,10 @@ rr_flux_kernel(const FluxParams P) {
 #endif
   if (COUNT) {
 #pragma unroll
-    for (int q = 0; q < 6; ++q) {
+    for (int q = 0; q < 7; ++q) {
       unsigned long long x = cnt[q];
       for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-      if ((threadIdx.x & 31) == 0 && x) atomicAdd(P.counters + q, x);
+      if ((threadIdx.x & 31) == 0 && x) atomicAdd(P.counters + (q < 6 ? q : 8), x);
     }
     if (threadIdx.x == 0) {
       if (cfill) atomicAdd(P.counters + 6, cfill);
@@ -1497,9 +1579,12 @@ int rr_pv_prep_launch(rr_ctx *ctx, RRWork *wk, const double *d_pv, int64_t npv,
     wk->pv_cap = 0;
     if (wk->lens) cudaFree(wk->lens);
     wk->lens = nullptr;
+    if (wk->zpoly) cudaFree(wk->zpoly);
+    wk->zpoly = nullptr;
     if (cudaMalloc(&wk->pvo, sizeof(RRPvOrbit) * npv) != cudaSuccess ||
         cudaMalloc(&wk->pvb, sizeof(RRPvBand) * npv * c.nkpb) != cudaSuccess ||
-        cudaMalloc(&wk->lens, sizeof(double) * 2 * RR_LENS_PITCH * npv * c.nkpb) != cudaSuccess) {
+        cudaMalloc(&wk->lens, sizeof(double) * 2 * RR_LENS_PITCH * npv * c.nkpb) != cudaSuccess ||
+        cudaMalloc(&wk->zpoly, sizeof(double) * 2 * RR_LENS_PITCH * npv) != cudaSuccess) {
       cudaGetLastError();
       return RR_EALLOC;
     }
@@ -1562,7 +1647,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.nchunks = (unsigned)nchunks;
   P.chunk_len = (unsigned)chunk_len;
   const unsigned grid = (unsigned)(npv * nchunks);
-  size_t smem = (size_t)K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8 +
+  size_t smem = (size_t)K_SMEM * 8 + 16 + 4 * RR_LENS_PITCH * 8 +
                 (size_t)2 * P.ldw_len * (c.precision != RR_FP64 ? 4 : 8);
   smem = (smem + 15) & ~(size_t)15;
   P.ones_off = (unsigned)smem;
@@ -1570,7 +1655,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   smem += RR_ONES_BYTES;
 #endif
   if (ctx->counters_on)
-    RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 8, st));
+    RR_CUDA(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * 16, st));
   using Kernel = void (*)(const FluxParams);
   const int pi = c.precision == RR_FP32 ? 1 : (c.precision == RR_MIXED ? 2 : 0);
 #define RR_KROW(R, O, M)                                                                          \
@@ -1587,6 +1672,11 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
                      2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
                      ctx->reduction != RR_REDUCE_SHUFFLE;
   const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
+  P.zpoly = (c.precision == RR_FP64 && RR_ZPOLY && ctx->orbit_poly) ? wk->zpoly : nullptr;
+  if (P.zpoly) {            // fp64: z^2 over the transit window of every eccentric pv
+    rr_zpoly_kernel<<<(unsigned)((npv * 32 + 255) / 256), 256, 0, st>>>(wk->pvo, npv, wk->zpoly);
+    RR_LAUNCH_CHECK(ctx);
+  }
   if (P.lens) {             // fp64: the lens-area polynomials of every (pv, radius ratio)
     const int64_t nrows = npv * c.nkpb;
     rr_lens_poly_kernel<<<(unsigned)((nrows * 32 + 255) / 256), 256, 0, st>>>(wk->pvb, nrows, wk->lens);
@@ -1605,10 +1695,10 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   if (total <= 0) return RR_OK;
   const unsigned grid = rr_grid_for(total);
   if (fp32_math)
-    rr_orbit_kernel<float><<<grid, FT, K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
+    rr_orbit_kernel<float><<<grid, FT, K_SMEM * 8 + 16 + 4 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, wk->pvo,
                                                 ctx->ntiles, npv, ctx->nsub, d_z);
   else
-    rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16 + 2 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
+    rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16 + 4 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
