@@ -204,3 +204,51 @@ def test_lens_polynomial_reproduces_the_area(k):
         ap = full - t * p if lo else t * p
         worst = max(worst, abs(ap - float(_lens_exact_mp(k, z))))
     assert worst <= 2.5e-13, worst
+
+
+def test_orbit_polynomial_reproduces_z2_over_a_transit_window():
+    """rr_zpoly_kernel's construction restated in float64 on the CPU: z^2 of an eccentric orbit over
+    each half of its transit window, interpolated at the 13 Chebyshev nodes and converted to
+    monomials with RR_LENS_M, against the oracle's separation (a Newton solve per point): <= 5e-12 in
+    z^2 for config 4's eccentric parameter vectors whenever the kernel's tail test (|c12| + |c11| <=
+    1e-12) passes, which it does for most of them."""
+    import oracle
+    import workloads
+    X = _lens_table("RR_LENS_X")
+    n = X.size
+    M = _lens_table("RR_LENS_M").reshape(n, n)
+    wl = workloads.make_workload(4, npv=60, npt=10)
+    passed = worst = 0
+    total = 0
+    for row in wl.pv:
+        k, t0, p, e = row[0], row[1], row[2], row[5]
+        if e == 0.0:
+            continue
+        ts = t0 + np.linspace(-0.25 * p, 0.25 * p, 1601)
+        zz = np.array([z if front else 99.0 for z, front in (oracle.separation(t, *row[1:]) for t in ts)])
+        i0 = int(np.argmin(np.abs(ts - t0)))
+        if not zz[i0] < 1 + k:
+            continue
+        ia = ib = i0
+        while ia > 0 and zz[ia - 1] < 1 + k:
+            ia -= 1
+        while ib < ts.size - 1 and zz[ib + 1] < 1 + k:
+            ib += 1
+        c, h = 0.5 * (ts[ia] + ts[ib]), 0.5 * (ts[ib] - ts[ia]) * 1.03 + 1e-6
+        total += 1
+        tail = err = 0.0
+        for sgn in (-1.0, 1.0):
+            g = np.array([oracle.separation(c + sgn * h * 2 * x, *row[1:])[0] ** 2 for x in X])
+            a = M @ g
+            tail += abs(a[12]) / 2048 + abs(a[11]) / 1024
+            for tp in np.linspace(0, 1, 33):
+                w = 2 * tp - 1
+                q = 0.0
+                for cj in a[::-1]:
+                    q = q * w + cj
+                err = max(err, abs(q - oracle.separation(c + sgn * h * tp, *row[1:])[0] ** 2))
+        if tail <= 1e-12:
+            passed += 1
+            worst = max(worst, err)
+    assert total >= 20 and passed >= 0.7 * total, (passed, total)
+    assert worst <= 5e-12, worst

@@ -1254,3 +1254,45 @@ def test_lens_polynomial_radius_ratio_edges(rr):
     assert np.max(err) <= TOL64, [float(f"{x:.1e}") for x in err]
     assert np.max(err) <= 1e-12, [float(f"{x:.1e}") for x in err]      # what the arithmetic gives
     gm.close()
+
+
+def test_orbit_polynomials_against_the_per_subsample_solve(rr):
+    """rr_set_orbit_poly: the fp64 kernel takes z^2 of eccentric pvs from per-pv polynomials over the
+    transit window (fitted through 26 exact Kepler solves per evaluate) where they converge, and solves
+    Kepler's equation per sub-sample otherwise.  Both against the oracle (which always solves), the two
+    against each other, and the class counters: most of config 3's / 4's eccentric sub-samples go
+    through the polynomials, none with the switch off, none for e = 0.99 at periastron (no
+    convergence: the gate must send those to the solver)."""
+    for config in (3, 4):
+        wl = small_workload(config)
+        want, _ = oracle_flux(wl)
+        gm = gpu_model(rr, wl)
+        gm.build_ld_table(wl.ldp(gm.mu))
+        out = {}
+        for on in (True, False):
+            rr.rr_set_orbit_poly(gm.ctx, on)
+            rr.rr_enable_counters(gm.ctx, True)
+            out[on] = gm.evaluate(wl.pv).cpu().numpy()
+            cnt = rr.rr_get_counters(gm.ctx)
+            rr.rr_enable_counters(gm.ctx, False)
+            assert np.max(np.abs(out[on] - want)) <= 1e-12
+            if on:
+                assert cnt["eccentric_poly"] > 0.5 * cnt["eccentric"] > 0
+            else:
+                assert cnt["eccentric_poly"] == 0 and cnt["solver_iters"] >= cnt["eccentric"] > 0
+        assert 0 < np.max(np.abs(out[True] - out[False])) <= 1e-12
+        gm.close()
+    # gate: wide windows of close-in, very eccentric orbits do not converge
+    rng = np.random.default_rng(990)
+    pv = _eccentric_population(0.99, rng)
+    t1 = _multiscale_times()
+    mc = workloads.ModelConfig()
+    coeffs = np.tile(np.array([[[0.45, 0.15]]]), (pv.shape[0], 1, 1))
+    gm = rr.RoadRunner.from_config(mc)
+    gm.set_data(t1, np.zeros(t1.size, np.int32), [0], [1], [0.0])
+    gm.build_ld_table(workloads.sample_profile("quadratic", coeffs, gm.mu))
+    rr.rr_enable_counters(gm.ctx, True)
+    gm.evaluate(pv)
+    cnt = rr.rr_get_counters(gm.ctx)
+    assert 0 < cnt["eccentric"] and cnt["eccentric_poly"] < cnt["eccentric"]
+    gm.close()
