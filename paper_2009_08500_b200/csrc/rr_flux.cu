@@ -414,6 +414,27 @@ template <typename R, int M> struct Cst {
     lens2<0, OFF>(hoff, c0, c1); p = fma(p, w, c1); p = fma(p, w, c0);
     return p;
   }
+  // fp32 kernels: the same polynomial from coefficients staged as floats (16 per half, hoff 0 or 64)
+  template <int MM, int OFF> __device__ __forceinline__ float4 coef4f(unsigned hoff) const {
+    float4 v;
+    if constexpr (M == RR_SM_SYMBOL) {
+      v = reinterpret_cast<const float4 *>(rr_dyn + OFF + hoff)[MM];
+    } else {
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+                   : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                   : "r"(sb + hoff), "n"(AB + OFF + 16 * MM));
+    }
+    return v;
+  }
+  template <int OFF> __device__ __forceinline__ float poly12f(unsigned hoff, float w) const {
+    const float4 c3 = coef4f<3, OFF>(hoff), c2 = coef4f<2, OFF>(hoff), c1 = coef4f<1, OFF>(hoff),
+                 c0 = coef4f<0, OFF>(hoff);
+    float p = c3.x;                                  // c12
+    p = fmaf(p, w, c2.w); p = fmaf(p, w, c2.z); p = fmaf(p, w, c2.y); p = fmaf(p, w, c2.x);
+    p = fmaf(p, w, c1.w); p = fmaf(p, w, c1.z); p = fmaf(p, w, c1.y); p = fmaf(p, w, c1.x);
+    p = fmaf(p, w, c0.w); p = fmaf(p, w, c0.z); p = fmaf(p, w, c0.y); p = fmaf(p, w, c0.x);
+    return p;
+  }
   // table cell ig of the staged row: node ldw[ig] and slope ldw[ig+1] - ldw[ig], one load
   using R2 = typename Vec2T<R>::type;
   static __device__ __forceinline__ R2 *row() { return reinterpret_cast<R2 *>(rr_dyn + OFF_ROW); }
@@ -829,12 +850,16 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
     bool front = true;
     int it = 0, ing = 0;
     R z2;
-    if (!CIRC && sizeof(R) == 8 && (kmode & 4)) {
+    if (!CIRC && (kmode & 4)) {
       // z^2 from the pv's polynomials over its transit window (rr_zpoly_kernel): t' = |w| / hwid
       if constexpr (!CIRC && sizeof(R) == 8) {
         const double t = wr * K.template get<K_INVHW>();
         const unsigned hoff = t < 0.0 ? 0u : (unsigned)(RR_LENS_PITCH * 8);
         z2 = fabs(K.template poly12<Cst<R, M>::OFF_ZPOLY>(hoff, fma(fabs(t), 2.0, -1.0))) + RR_TINY_D;
+      } else if constexpr (!CIRC) {
+        const float t = (float)wr * K.template get<K_INVHW>();
+        z2 = fabsf(K.template poly12f<Cst<R, M>::OFF_ZPOLY>(t < 0.0f ? 0u : 64u,
+                                                             fmaf(fabsf(t), 2.0f, -1.0f))) + 1e-30f;
       }
       if (COUNT) cnt[6]++;
     } else {
@@ -1028,8 +1053,9 @@ template <typename R, typename O, bool CIRC, bool NOWRAP, int M>
 __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, O *__restrict__ out,
                                               int count, int ns, double t0, double inv_p,
                                               double u_mid, double hwid, double hw, O scale,
-                                              const Cst<R, M> K, bool ksmall) {
+                                              const Cst<R, M> K, int kmode) {
   using P = typename PairT<R>::type;
+  const bool ksmall = (kmode & 1) != 0;
   constexpr bool ANG = NOWRAP && sizeof(R) == 4;   // fp32 angle step per sub-sample
   const double du = 2.0 * hw / ns, off0 = hw * (1.0 / ns - 1.0), hskip = hwid + hw;
   const bool need_front =
@@ -1037,6 +1063,8 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
   // (lane-0 broadcasts: opaque, or the compiler recomputes both from fp64 in the sub-sample loop)
   const float2 da2 = splat<float>(__shfl_sync(0xffffffffu, (float)(RR_TWOPI * du), 0));
   const float hwa = __shfl_sync(0xffffffffu, (float)(RR_TWOPI * hwid), 0);
+  const float inv_hwa = __shfl_sync(0xffffffffu, (float)(1.0 / (RR_TWOPI * hwid)), 0);
+  const float inv_hw = __shfl_sync(0xffffffffu, (float)(1.0 / hwid), 0);
   uintptr_t tp = reinterpret_cast<uintptr_t>(times + threadIdx.x);
   uintptr_t op = reinterpret_cast<uintptr_t>(out + threadIdx.x);
   int left = count - (int)threadIdx.x;
@@ -1068,14 +1096,16 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
       for (int s = 0; s < ns; ++s, wa += du, wb += du) {
         bool ax, ay;
         P dM;
+        float2 tw = splat<float>(0.0f);        // fp32: phase from the window centre / hwid
         if constexpr (ANG) {
-          const float2 aw = abs2(fma2(fs, da2, aw0));
+          const float2 aws = fma2(fs, da2, aw0), aw = abs2(aws);
           ax = aw.x <= hwa;
           ay = aw.y <= hwa;
           const float2 am = fma2(fs, da2, am0);
           fs = add2(fs, splat<float>(1.0f));
           if (!(ax || ay)) continue;
           dM = mk2((R)am.x, (R)am.y);
+          tw = mk2(ax ? aws.x * inv_hwa : 0.0f, ay ? aws.y * inv_hwa : 0.0f);
         } else {
           const double was = NOWRAP ? wa : wa - rr_round(wa), wbs = NOWRAP ? wb : wb - rr_round(wb);
           ax = fabs(was) <= hwid;               // (1e30 - round(1e30) = 0: only without NOWRAP ...
@@ -1083,10 +1113,24 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
           if (!NOWRAP) { ax = ax && ina; ay = ay && inb; }   // ... where the flags are needed)
           if (!(ax || ay)) continue;
           dM = mk2((R)(RR_TWOPI * (was + u_mid)), (R)(RR_TWOPI * (wbs + u_mid)));
+          if constexpr (sizeof(R) == 4)
+            tw = mk2(ax ? (float)was * inv_hw : 0.0f, ay ? (float)wbs * inv_hw : 0.0f);
         }
         dM = sel2(ax, ay, dM, splat<R>((R)0));
-        bool fx, fy;
-        const P z2 = rr_separation2_pair<R, CIRC, M>(K, dM, ax, ay, fx, fy);
+        bool fx = true, fy = true;
+        P z2;
+        if (!CIRC && sizeof(R) == 4 && (kmode & 4)) {
+          // z^2 of both elements from the pv's polynomials (rr_zpoly_kernel), each in its own half
+          if constexpr (!CIRC && sizeof(R) == 4) {
+            const float px = K.template poly12f<Cst<R, M>::OFF_ZPOLY>(tw.x < 0.0f ? 0u : 64u,
+                                                                      fmaf(fabsf(tw.x), 2.0f, -1.0f));
+            const float py = K.template poly12f<Cst<R, M>::OFF_ZPOLY>(tw.y < 0.0f ? 0u : 64u,
+                                                                      fmaf(fabsf(tw.y), 2.0f, -1.0f));
+            z2 = mk2(fabsf(px) + 1e-30f, fabsf(py) + 1e-30f);
+          }
+        } else {
+          z2 = rr_separation2_pair<R, CIRC, M>(K, dM, ax, ay, fx, fy);
+        }
         bool ox = ax && z2.x < opk2.x, oy = ay && z2.y < opk2.y;
         if (need_front) { ox = ox && fx; oy = oy && fy; }
         if (ox || oy) {
@@ -1126,7 +1170,7 @@ __device__ __forceinline__ void rr_tile(const double *__restrict__ times, O *__r
     if (!shuffle && count > FT) {   // two exposures per thread (tiles of <= FT exposures, the
                                     // counting build and fp64 circular tiles keep the scalar loop)
       rr_tile_pairs<R, O, CIRC, NOWRAP, M>(times, out, count, ns, t0, inv_p, u_mid, hwid, hw, scale,
-                                           K, ksmall);
+                                           K, kmode);
       return;
     }
   }
@@ -1380,10 +1424,19 @@ rr_flux_kernel(const FluxParams P) {
         if (lens_on && threadIdx.x < 2 * RR_LENS_PITCH)
           Cst<R, M>::lens()[threadIdx.x] =
               P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) + threadIdx.x];
-        const bool zpoly_on = sizeof(R) == 8 && P.zpoly != nullptr && po.zpoly_ok != 0;
-        if (zpoly_on && threadIdx.x >= 32 && threadIdx.x < 32 + 2 * RR_LENS_PITCH)
-          Cst<R, M>::zpoly()[threadIdx.x - 32] =
-              P.zpoly[(int64_t)v * (2 * RR_LENS_PITCH) + threadIdx.x - 32];
+        const bool zpoly_on = P.zpoly != nullptr && po.zpoly_ok != 0;
+        if constexpr (sizeof(R) == 8) {
+          if (zpoly_on && threadIdx.x >= 32 && threadIdx.x < 32 + 2 * RR_LENS_PITCH)
+            Cst<R, M>::zpoly()[threadIdx.x - 32] =
+                P.zpoly[(int64_t)v * (2 * RR_LENS_PITCH) + threadIdx.x - 32];
+        } else {              // fp32 kernels: the coefficients rounded to fp32, 16 floats per half
+          if (zpoly_on && threadIdx.x >= 32 && threadIdx.x < 64) {
+            const int half = (threadIdx.x - 32) >> 4, j = threadIdx.x & 15;
+            reinterpret_cast<float *>(Cst<R, M>::zpoly())[threadIdx.x - 32] =
+                j < RR_LENS_N ? (float)P.zpoly[(int64_t)v * (2 * RR_LENS_PITCH) + half * RR_LENS_PITCH + j]
+                              : 0.0f;
+          }
+        }
         rr_stage_constants<R>(po, pb, 2.0 * hw / lc.ns, lens_on, zpoly_on);
         if (threadIdx.x == K_SCALE) Cst<R, M>::store(K_SCALE, sc_d);
         __syncthreads();
@@ -1672,8 +1725,8 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
                      2 * ctx->npt > 3 * (int64_t)FT * ctx->ntiles &&
                      ctx->reduction != RR_REDUCE_SHUFFLE;
   const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
-  P.zpoly = (c.precision == RR_FP64 && RR_ZPOLY && ctx->orbit_poly) ? wk->zpoly : nullptr;
-  if (P.zpoly) {            // fp64: z^2 over the transit window of every eccentric pv
+  P.zpoly = (RR_ZPOLY && ctx->orbit_poly) ? wk->zpoly : nullptr;   // (fitted in fp64 for every precision)
+  if (P.zpoly) {            // z^2 over the transit window of every eccentric pv
     rr_zpoly_kernel<<<(unsigned)((npv * 32 + 255) / 256), 256, 0, st>>>(wk->pvo, npv, wk->zpoly);
     RR_LAUNCH_CHECK(ctx);
   }
