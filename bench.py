@@ -58,8 +58,8 @@ ALG_OPS = {
     "fp32": dict(skipped=0, circular=7, eccentric_fixed=20, solver_iter=24, occulting=11,
                  ingress=45),
 }
-# what the committed fp64 kernel executes per unit where that differs from the direct formulation
-EXECUTED_OPS = {"fp64": dict(ingress=24)}
+# what the committed kernels execute per unit where that differs from the direct formulation
+EXECUTED_OPS = {"fp64": dict(ingress=24), "fp32": dict(ingress=24)}
 ZPOLY_OPS = 15      # an eccentric sub-sample through the z^2 polynomials: t, w, Horner 12, |.| + tiny
 
 
@@ -463,7 +463,7 @@ def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, 
     exe_ops = dict(ops)
     exe_ops.update(EXECUTED_OPS.get("fp64" if precision == "fp64" else "fp32", {}))
     exe_fma = alg_fma + sum(counts[c] * (exe_ops[c] - ops[c]) for c in ("ingress",))
-    if precision == "fp64" and counts.get("eccentric_poly"):
+    if counts.get("eccentric_poly"):
         # sub-samples taken from the z^2 polynomials: ZPOLY_OPS instead of the fixed part and their solves
         exe_fma += (counts["eccentric_poly"] * (ZPOLY_OPS - ops["eccentric_fixed"])
                     - (counts["solver_iters"] - counts["solver_iters_as_run"]) * ops["solver_iter"])

@@ -694,7 +694,7 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, 
   R ap;
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
-  } else if (sizeof(R) == 8 && (kmode & 2)) {
+  } else if (kmode & 2) {
     // Between the contacts, polynomial form (rr_lens_poly_kernel): x = (z - (1-k)) / (2k),
     //   a = pi k^2 - x^(3/2) g0(4x - 1)  for x <= 1/2,   a = y^(3/2) g1(4y - 1), y = 1 - x, else.
     if constexpr (sizeof(R) == 8) {
@@ -709,6 +709,15 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, 
       const double p = K.template poly12<Cst<R, M>::OFF_LENS>(hoff, w);
       const double t = xx * sq;
       ap = lo ? fma(-t, p, afull) : t * p;
+    } else {
+      float inv2k, xoff;
+      K.template pair<K_INV2K>(inv2k, xoff);
+      const float x = fmaf(z, inv2k, xoff);
+      const bool lo = x <= 0.5f;
+      const float xx = fabsf(lo ? x : 1.0f - x);
+      const float p = K.template poly12f<Cst<R, M>::OFF_LENS>(lo ? 0u : 64u, fmaf(xx, 4.0f, -1.0f));
+      const float t = xx * rr_sqrt_core(xx + 1e-30f);
+      ap = fmaxf(lo ? fmaf(-t, p, afull) : t * p, 0.0f);
     }
     ++ningress;
   } else {
@@ -1013,8 +1022,9 @@ rr_separation2_pair(const Cst<R, M> K, typename PairT<R>::type dM, bool ax, bool
 // Occulted light ip * ap of the pair; (ox, oy): z < 1+k in front of the star.
 template <typename R, int M>
 __device__ __forceinline__ typename PairT<R>::type
-rr_deficit_pair(const Cst<R, M> K, typename PairT<R>::type z2, bool ox, bool oy, bool ksmall) {
+rr_deficit_pair(const Cst<R, M> K, typename PairT<R>::type z2, bool ox, bool oy, int kmode) {
   using P = typename PairT<R>::type;
+  const bool ksmall = (kmode & 1) != 0;
   P gscale, opk, omk2, afull;
   rr_pairP<K_GSCALE>(K, gscale, opk);
   rr_pairP<K_OMK2>(K, omk2, afull);
@@ -1031,7 +1041,24 @@ rr_deficit_pair(const Cst<R, M> K, typename PairT<R>::type z2, bool ox, bool oy,
   const P ip = fma2(ag, mk2(slx, sly), mk2(l0x, l0y));
   const bool inx = ox && z2.x > omk2.x, iny = oy && z2.y > omk2.y;
   P ap = afull;
-  if (inx || iny) {                             // lens area (rr_deficit), both elements
+  if ((inx || iny) && sizeof(R) == 4 && (kmode & 2)) {
+    // lens polynomials (rr_deficit, fp32): each element with the coefficients of its own half, two
+    // scalar chains (packing the coefficients of two different halves costs more than it saves)
+    if constexpr (sizeof(R) == 4) {
+      P inv2k, xoff;
+      rr_pairP<K_INV2K>(K, inv2k, xoff);
+      const P x = fma2(z, inv2k, xoff);
+      const bool lox = x.x <= 0.5f, loy = x.y <= 0.5f;
+      const P xx = abs2(sel2(lox, loy, x, sub2(splat<R>(1.0f), x)));
+      const P w = fma2(xx, splat<R>(4.0f), splat<R>(-1.0f));
+      const P t = mul2(xx, rr_sqrt2(add2(xx, splat<R>(1e-30f))));
+      const float px = K.template poly12f<Cst<R, M>::OFF_LENS>(lox ? 0u : 64u, w.x);
+      const float py = K.template poly12f<Cst<R, M>::OFF_LENS>(loy ? 0u : 64u, w.y);
+      const float lx = lox ? fmaf(-t.x, px, afull.x) : t.x * px;
+      const float ly = loy ? fmaf(-t.y, py, afull.y) : t.y * py;
+      ap = mk2(inx ? fmaxf(lx, 0.0f) : afull.x, iny ? fmaxf(ly, 0.0f) : afull.y);
+    }
+  } else if (inx || iny) {                      // lens area (rr_deficit), both elements
     const P omks = rr_getP<K_OMKS>(K);
     const P A = sub2(opk, z), B = add2(z, omks), C = sub2(z, omks), D = add2(z, opk);
     const P AB = abs2(mul2(A, B)), S = abs2(mul2(C, D)), Q = mul2(B, D);
@@ -1134,7 +1161,7 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
         bool ox = ax && z2.x < opk2.x, oy = ay && z2.y < opk2.y;
         if (need_front) { ox = ox && fx; oy = oy && fy; }
         if (ox || oy) {
-          const P def = rr_deficit_pair<R, M>(K, z2, ox, oy, ksmall);
+          const P def = rr_deficit_pair<R, M>(K, z2, ox, oy, kmode);
           acca += (O)def.x;
           accb += (O)def.y;
         }
@@ -1420,10 +1447,19 @@ rr_flux_kernel(const FluxParams P) {
             ldw2[ig] = c;
           }
         }
-        const bool lens_on = sizeof(R) == 8 && P.lens != nullptr && pb.lens_ok != 0;
-        if (lens_on && threadIdx.x < 2 * RR_LENS_PITCH)
-          Cst<R, M>::lens()[threadIdx.x] =
-              P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) + threadIdx.x];
+        const bool lens_on = P.lens != nullptr && pb.lens_ok != 0;
+        if constexpr (sizeof(R) == 8) {
+          if (lens_on && threadIdx.x < 2 * RR_LENS_PITCH)
+            Cst<R, M>::lens()[threadIdx.x] =
+                P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) + threadIdx.x];
+        } else {              // fp32 kernels: the coefficients rounded to fp32, 16 floats per half
+          if (lens_on && threadIdx.x < 32) {
+            const int half = threadIdx.x >> 4, j = threadIdx.x & 15;
+            reinterpret_cast<float *>(Cst<R, M>::lens())[threadIdx.x] =
+                j < RR_LENS_N ? (float)P.lens[((int64_t)v * P.nkpb + kb) * (2 * RR_LENS_PITCH) +
+                                              half * RR_LENS_PITCH + j] : 0.0f;
+          }
+        }
         const bool zpoly_on = P.zpoly != nullptr && po.zpoly_ok != 0;
         if constexpr (sizeof(R) == 8) {
           if (zpoly_on && threadIdx.x >= 32 && threadIdx.x < 32 + 2 * RR_LENS_PITCH)
@@ -1668,7 +1704,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.T = wk->lazy ? nullptr : wk->T;
   P.rows = wk->lazy ? wk->rows : nullptr;
   P.istar = wk->istar;
-  P.lens = (c.precision == RR_FP64 && RR_LENS_POLY) ? wk->lens : nullptr;
+  P.lens = RR_LENS_POLY ? wk->lens : nullptr;   // (fitted in fp64 for every precision)
   P.flux = d_flux;
   P.counters = ctx->d_counters;
   P.npt = ctx->npt;
