@@ -25,7 +25,9 @@
 // exposure, one plane rotation per further sub-sample.
 // Round 2: out-of-window runs of flux = 1 go out as TMA bulk copies from a block-resident buffer of
 // ones (rr_fill_ones_bulk); the fp32 and mixed kernels take two exposures per thread with packed
-// FFMA2 arithmetic (rr_tile_pairs) when the tiles are longer than a block.
+// FFMA2 arithmetic (rr_tile_pairs) when the tiles are longer than a block; the lens area between the
+// contacts (rr_lens_poly_kernel) and z^2 over the transit window of an eccentric pv (rr_zpoly_kernel)
+// come from per-pv degree-12 polynomials fitted through exact evaluations once per rr_evaluate.
 #include <algorithm>
 
 #include "rr_common.cuh"
