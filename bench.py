@@ -84,6 +84,9 @@ def parse_args():
     ap.add_argument("--ld-law", default=None, choices=["quadratic"],
                     help="time the step with rr_build_ld_table_law (the law evaluated on the device "
                          "from its coefficients, PAPER.md:143-156) instead of rr_build_ld_table")
+    ap.add_argument("--no-orbit-poly", action="store_true",
+                    help="solve Kepler's equation per eccentric sub-sample (rr_set_orbit_poly(ctx, 0)) "
+                         "instead of evaluating the per-pv z^2 polynomials")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true",
@@ -271,15 +274,17 @@ DTYPE_NAME = {"fp64": "f64", "fp32": "f32", "mixed": "f32 (sum and flux f64)"}
 class Case:
     """One workload in one precision, resident on the device: ctx, inputs, output buffers."""
 
-    def __init__(self, rr, wl, precision: str, table_mode: str, dev, ld_law=None):
+    def __init__(self, rr, wl, precision: str, table_mode: str, dev, ld_law=None, orbit_poly=True):
         import torch
         self.rr, self.wl, self.precision, self.dev = rr, wl, precision, dev
+        self.orbit_poly = orbit_poly
         code = PRECISIONS[precision]
         self.npdt = np.float32 if code != rr.RR_FP64 else np.float64
         self.model = rr.RoadRunner.from_config(wl.model, code)
         self.ctx = self.model.ctx
         rr.rr_set_table_mode(self.ctx, {"lazy": rr.RR_TABLE_LAZY, "full": rr.RR_TABLE_FULL,
                                         "direct": rr.RR_TABLE_DIRECT}[table_mode])
+        rr.rr_set_orbit_poly(self.ctx, orbit_poly)
         self.model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
                             wl.exposure_time)
         self.ldp_h = np.ascontiguousarray(wl.ldp(self.model.mu), dtype=self.npdt)
@@ -367,7 +372,7 @@ class Case:
         rr.rr_set_orbit_poly(self.ctx, False)
         rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
         counts = rr.rr_get_counters(self.ctx)
-        rr.rr_set_orbit_poly(self.ctx, True)
+        rr.rr_set_orbit_poly(self.ctx, self.orbit_poly)
         rr.rr_evaluate(self.ctx, self.pv, self.flux, self.status)
         as_run = rr.rr_get_counters(self.ctx)
         rr.rr_enable_counters(self.ctx, False)
@@ -555,7 +560,8 @@ def run_ours(args):
         wl.pv = np.ascontiguousarray(np.roll(wl.pv, sh, axis=0))
         wl.ld_coeffs = np.ascontiguousarray(np.roll(wl.ld_coeffs, sh, axis=0))
 
-    case = Case(rr, wl, args.precision, args.table_mode, dev, ld_law=args.ld_law)
+    case = Case(rr, wl, args.precision, args.table_mode, dev, ld_law=args.ld_law,
+                orbit_poly=not args.no_orbit_poly)
     ctx, model = case.ctx, case.model
     steps, warm = max(1, args.steps), max(3, args.warmup)
 
@@ -637,7 +643,9 @@ def run_ours(args):
               "no flush needed" if wl.npv * wl.npt * es > 2 ** 28 else
               "working set fits L2: small config, latency-bound, no roofline claim",
         "invalid_pv": n_bad,
-        "ld_table_call": "rr_build_ld_table_law" if args.ld_law else "rr_build_ld_table"})
+        "ld_table_call": "rr_build_ld_table_law" if args.ld_law else "rr_build_ld_table",
+        "orbit": "Kepler solve per eccentric sub-sample" if args.no_orbit_poly else
+                 "per-pv z^2 polynomials over the transit window where they converge, else the solve"})
     case.close()
     del case
     torch.cuda.empty_cache()
