@@ -23,6 +23,11 @@
  *     before anything was launched; <= -1000 = CUDA error (-1000 - cudaError_t).
  *     rr_error_string() names any code.  No exception crosses the ABI.
  *   - There is no CPU fallback: without a CUDA device every compute call fails with a CUDA error.
+ *   - A ctx is not thread-safe and keeps ONE set of per-evaluation buffers for the device-pointer
+ *     API: calls on the same ctx must be issued from one host thread at a time and, if they go to
+ *     different streams, ordered by the caller (two evaluations in flight need two contexts).  In
+ *     steady state (same npv, same data) rr_build_ld_table* and rr_evaluate allocate nothing and
+ *     synchronise nothing, so a step can be captured into a CUDA graph.
  *
  * Per-parameter-vector validity (reading R12): a parameter vector whose k is outside [k0,k1] (in
  * RR_TABLE_DIRECT mode: k <= 0), whose
