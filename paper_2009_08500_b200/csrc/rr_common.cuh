@@ -48,7 +48,7 @@ struct RRPvOrbit {
   double aci2;          // a^2 cos^2 i:  z^2 = x^2 + aci2 y^2
   int32_t status;       // RR_PV_* bits; != 0 -> NaN row
   int32_t circular;     // e == 0
-  int32_t zpoly_ok;     // 1: z^2 over the transit window from the fitted polynomials (rr_zpoly_kernel)
+  int32_t zpoly_ok;     // 1: z^2 over the transit window from the fitted polynomials (rr_zpoly_fit)
   int32_t pad;
 };
 
@@ -63,7 +63,7 @@ struct RRPvBand {
   double kw;           // radius ratio the LD weights are taken at: k, or the mean of the pv's k over
                        // the passbands (transmission-spectroscopy shortcut)
   int32_t ik;          // lower k row of kw, clamped to nk-2 (reading R10)
-  int32_t lens_ok;     // 1: the polynomial form of the lens area holds for this k (rr_lens_poly_kernel)
+  int32_t lens_ok;     // 1: the polynomial form of the lens area holds for this k (rr_lens_fit)
 };
 
 // Per-evaluation device buffers: one set for the device-pointer API, one per slot of the

@@ -26,7 +26,7 @@
 // Round 2: out-of-window runs of flux = 1 go out as TMA bulk copies from a block-resident buffer of
 // ones (rr_fill_ones_bulk); the fp32 and mixed kernels take two exposures per thread with packed
 // FFMA2 arithmetic (rr_tile_pairs) when the tiles are longer than a block; the lens area between the
-// contacts (rr_lens_poly_kernel) and z^2 over the transit window of an eccentric pv (rr_zpoly_kernel)
+// contacts (rr_lens_fit) and z^2 over the transit window of an eccentric pv (rr_zpoly_fit)
 // come from per-pv degree-12 polynomials fitted through exact evaluations once per rr_evaluate.
 #include <algorithm>
 
@@ -215,16 +215,13 @@ __global__ void rr_pv_prep_kernel(const double *__restrict__ pv, int64_t npv, in
 // For x = (z - (1-k)) / (2k) in (0, 1):  a(z) = pi k^2 - x^(3/2) g0(x) for x <= 1/2 and
 // a(z) = y^(3/2) g1(y), y = 1 - x, for x > 1/2, with g0, g1 analytic (the area is analytic in the angle
 // theta, x = sin^2(theta/2)): degree-12 interpolants at the Chebyshev nodes of [0, 1/2] reproduce the
-// area to 2e-13 for k <= 0.32 (tests/test_device_poly.py).  One warp per (pv, k): lanes 0..12 and
+// area to 2e-13 for k <= 0.32 (tests/test_device_poly.py).  One warp per (pv, k) (rr_poly_fit_kernel): lanes 0..12 and
 // 13..25 evaluate the exact area (two sectors minus the kite, reading R9) at the nodes of the two
 // halves; the node values become monomial coefficients in w = 4x - 1 through the matrix RR_LENS_M.
 // The flux kernel then pays one square root and a Horner chain per ingress / egress sub-sample
 // instead of a square root, two divisions and two arctangents (60 -> 23 FP64 instructions).
-__global__ void rr_lens_poly_kernel(const RRPvBand *__restrict__ pvb, int64_t nrows,
-                                    double *__restrict__ lens) {
-  const int64_t row = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (row >= nrows) return;
+__device__ __forceinline__ void rr_lens_fit(const RRPvBand *__restrict__ pvb, int64_t row, int lane,
+                                            double *__restrict__ lens) {
   const RRPvBand b = pvb[row];
   if (!b.lens_ok) return;                         // the flux kernel takes the exact form
   const int half = lane >= RR_LENS_N ? 1 : 0, i = lane - half * RR_LENS_N;
@@ -543,10 +540,8 @@ __device__ RR_ROBUST_INLINE int rr_kepler_robust(R e, R sE, R cE, R dM, R *s_out
 #ifndef RR_ZPOLY_TAIL
 #define RR_ZPOLY_TAIL 1e-12
 #endif
-__global__ void rr_zpoly_kernel(RRPvOrbit *__restrict__ pvo, int64_t npv, double *__restrict__ zpoly) {
-  const int64_t v = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (v >= npv) return;
+__device__ __forceinline__ void rr_zpoly_fit(RRPvOrbit *__restrict__ pvo, int64_t v, int lane,
+                                             double *__restrict__ zpoly) {
   const RRPvOrbit po = pvo[v];
   if (po.status || po.circular || !(po.hwid < 0.49)) return;     // (zpoly_ok stays 0)
   const int half = lane >= RR_LENS_N ? 1 : 0, i = lane - half * RR_LENS_N;
@@ -578,6 +573,18 @@ __global__ void rr_zpoly_kernel(RRPvOrbit *__restrict__ pvo, int64_t npv, double
   if (lane >= 2 * RR_LENS_N && lane < 2 * RR_LENS_N + 2)
     zpoly[(v * 2 + (lane - 2 * RR_LENS_N)) * RR_LENS_PITCH + RR_LENS_N] = 0.0;
   if (lane == 0 && tail <= RR_ZPOLY_TAIL) pvo[v].zpoly_ok = 1;
+}
+
+// One launch for both fits: warps [0, nrows) take the lens polynomials of the (pv, k) rows, warps
+// [nrows, nrows + npv) the z^2 polynomials of the parameter vectors (either part may be absent).
+__global__ void rr_poly_fit_kernel(const RRPvBand *__restrict__ pvb, int64_t nrows,
+                                   double *__restrict__ lens, RRPvOrbit *__restrict__ pvo, int64_t npv,
+                                   double *__restrict__ zpoly) {
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  const int64_t nl = lens ? nrows : 0;
+  if (w < nl) rr_lens_fit(pvb, w, lane, lens);
+  else if (zpoly && w - nl < npv) rr_zpoly_fit(pvo, w - nl, lane, zpoly);
 }
 
 // ---- kernel 2 core: squared separation at reduced phase ur (turns, relative to t0) ----------------------
@@ -697,7 +704,7 @@ __device__ __forceinline__ R rr_deficit(const Cst<R, M> K, R z2, int &ningress, 
   if (z2 <= omk2) {
     ap = afull;                             // planet (or star) fully inside the other disc
   } else if (kmode & 2) {
-    // Between the contacts, polynomial form (rr_lens_poly_kernel): x = (z - (1-k)) / (2k),
+    // Between the contacts, polynomial form (rr_lens_fit): x = (z - (1-k)) / (2k),
     //   a = pi k^2 - x^(3/2) g0(4x - 1)  for x <= 1/2,   a = y^(3/2) g1(4y - 1), y = 1 - x, else.
     if constexpr (sizeof(R) == 8) {
       double inv2k, xoff;
@@ -862,7 +869,7 @@ __device__ __forceinline__ R rr_subsample(const Cst<R, M> K, double w, double u_
     int it = 0, ing = 0;
     R z2;
     if (!CIRC && (kmode & 4)) {
-      // z^2 from the pv's polynomials over its transit window (rr_zpoly_kernel): t' = |w| / hwid
+      // z^2 from the pv's polynomials over its transit window (rr_zpoly_fit): t' = |w| / hwid
       if constexpr (!CIRC && sizeof(R) == 8) {
         const double t = wr * K.template get<K_INVHW>();
         const unsigned hoff = t < 0.0 ? 0u : (unsigned)(RR_LENS_PITCH * 8);
@@ -1149,7 +1156,7 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
         bool fx = true, fy = true;
         P z2;
         if (!CIRC && sizeof(R) == 4 && (kmode & 4)) {
-          // z^2 of both elements from the pv's polynomials (rr_zpoly_kernel), each in its own half
+          // z^2 of both elements from the pv's polynomials (rr_zpoly_fit), each in its own half
           if constexpr (!CIRC && sizeof(R) == 4) {
             const float px = K.template poly12f<Cst<R, M>::OFF_ZPOLY>(tw.x < 0.0f ? 0u : 64u,
                                                                       fmaf(fabsf(tw.x), 2.0f, -1.0f));
@@ -1764,13 +1771,10 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
                      ctx->reduction != RR_REDUCE_SHUFFLE;
   const Kernel kern = kernels[ctx->smem_abs ? 1 : 0][pi][ctx->counters_on ? 1 : (pairs ? 2 : 0)];
   P.zpoly = (RR_ZPOLY && ctx->orbit_poly) ? wk->zpoly : nullptr;   // (fitted in fp64 for every precision)
-  if (P.zpoly) {            // z^2 over the transit window of every eccentric pv
-    rr_zpoly_kernel<<<(unsigned)((npv * 32 + 255) / 256), 256, 0, st>>>(wk->pvo, npv, wk->zpoly);
-    RR_LAUNCH_CHECK(ctx);
-  }
-  if (P.lens) {             // fp64: the lens-area polynomials of every (pv, radius ratio)
-    const int64_t nrows = npv * c.nkpb;
-    rr_lens_poly_kernel<<<(unsigned)((nrows * 32 + 255) / 256), 256, 0, st>>>(wk->pvb, nrows, wk->lens);
+  if (P.zpoly || P.lens) {  // the per-pv polynomials (lens area, z^2 over the transit window): one launch
+    const int64_t nrows = npv * c.nkpb, nw = (P.lens ? nrows : 0) + (P.zpoly ? npv : 0);
+    rr_poly_fit_kernel<<<(unsigned)((nw * 32 + 255) / 256), 256, 0, st>>>(
+        wk->pvb, nrows, P.lens ? wk->lens : nullptr, wk->pvo, npv, P.zpoly ? wk->zpoly : nullptr);
     RR_LAUNCH_CHECK(ctx);
   }
   if (smem > 48 * 1024)     // large ng, or mean-k padding: opt in to more dynamic shared memory

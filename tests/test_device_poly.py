@@ -171,7 +171,7 @@ def _lens_exact_mp(k, z):
 
 @pytest.mark.parametrize("k", [0.01, 0.05, 0.1, 0.2, 0.3, 0.32])
 def test_lens_polynomial_reproduces_the_area(k):
-    """The pipeline of rr_lens_poly_kernel + rr_deficit restated in float64 (exact area at the nodes
+    """The pipeline of rr_lens_fit + rr_deficit restated in float64 (exact area at the nodes
     by the half-angle form, node values -> monomial coefficients through RR_LENS_M, Horner in
     w = 4x - 1, a = pi k^2 - x^(3/2) g0 or y^(3/2) g1) against the textbook two-sector-minus-kite area
     in 40-digit arithmetic, between the contacts and right at them: <= 2.5e-13."""
@@ -207,7 +207,7 @@ def test_lens_polynomial_reproduces_the_area(k):
 
 
 def test_orbit_polynomial_reproduces_z2_over_a_transit_window():
-    """rr_zpoly_kernel's construction restated in float64 on the CPU: z^2 of an eccentric orbit over
+    """rr_zpoly_fit's construction restated in float64 on the CPU: z^2 of an eccentric orbit over
     each half of its transit window, interpolated at the 13 Chebyshev nodes and converted to
     monomials with RR_LENS_M, against the oracle's separation (a Newton solve per point): <= 5e-12 in
     z^2 for config 4's eccentric parameter vectors whenever the kernel's tail test (|c12| + |c11| <=
