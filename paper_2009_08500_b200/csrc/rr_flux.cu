@@ -927,9 +927,9 @@ __device__ __forceinline__ double rr_ld_time(uintptr_t p) {
 #define RR_ZPOLY 1
 #endif
 #ifndef RR_FP64_PAIRS
-#define RR_FP64_PAIRS 0   // measured, 80 registers / 6 blocks per SM: config 4 5.09 -> 5.56 ms, config 3
-                          // 7.56 -> 9.04: the FP64 pipe is the limit there, the pair shares everything
-                          // but the FP64 arithmetic and costs occupancy; kept as a build option
+#define RR_FP64_PAIRS 0   // measured twice: with the direct formulation (80 registers, 6 blocks per SM)
+                          // config 4 5.09 -> 5.56 ms, config 3 7.56 -> 9.04; with the polynomial paths
+                          // 3.85 -> 4.22 ms at 6, 7 or 8 blocks per SM.  Kept as a build option.
 #endif
 // two neighbouring constants as pairs (c, c): fp32 from the doubled slots, fp64 splat in registers
 template <int I, typename R, int M>
@@ -948,6 +948,13 @@ template <int I, typename R, int M>
 __device__ __forceinline__ typename PairT<R>::type rr_getP(const Cst<R, M> K) {
   if constexpr (sizeof(R) == 4) return K.template get2<I>();
   else return splat<R>(K.template get<I>());
+}
+
+// degree-12 polynomial of the first (lo) or second half of the region OFF, in the working precision
+template <int OFF, typename R, int M>
+__device__ __forceinline__ R rr_polyR(const Cst<R, M> K, bool lo, R w) {
+  if constexpr (sizeof(R) == 8) return K.template poly12<OFF>(lo ? 0u : (unsigned)(RR_LENS_PITCH * 8), w);
+  else return K.template poly12f<OFF>(lo ? 0u : 64u, w);
 }
 
 // The phases come as dM = 2 pi ur in the working precision (rr_tile_pairs).
@@ -1050,23 +1057,23 @@ rr_deficit_pair(const Cst<R, M> K, typename PairT<R>::type z2, bool ox, bool oy,
   const P ip = fma2(ag, mk2(slx, sly), mk2(l0x, l0y));
   const bool inx = ox && z2.x > omk2.x, iny = oy && z2.y > omk2.y;
   P ap = afull;
-  if ((inx || iny) && sizeof(R) == 4 && (kmode & 2)) {
-    // lens polynomials (rr_deficit, fp32): each element with the coefficients of its own half, two
-    // scalar chains (packing the coefficients of two different halves costs more than it saves)
-    if constexpr (sizeof(R) == 4) {
-      P inv2k, xoff;
-      rr_pairP<K_INV2K>(K, inv2k, xoff);
-      const P x = fma2(z, inv2k, xoff);
-      const bool lox = x.x <= 0.5f, loy = x.y <= 0.5f;
-      const P xx = abs2(sel2(lox, loy, x, sub2(splat<R>(1.0f), x)));
-      const P w = fma2(xx, splat<R>(4.0f), splat<R>(-1.0f));
-      const P t = mul2(xx, rr_sqrt2(add2(xx, splat<R>(1e-30f))));
-      const float px = K.template poly12f<Cst<R, M>::OFF_LENS>(lox ? 0u : 64u, w.x);
-      const float py = K.template poly12f<Cst<R, M>::OFF_LENS>(loy ? 0u : 64u, w.y);
-      const float lx = lox ? fmaf(-t.x, px, afull.x) : t.x * px;
-      const float ly = loy ? fmaf(-t.y, py, afull.y) : t.y * py;
-      ap = mk2(inx ? fmaxf(lx, 0.0f) : afull.x, iny ? fmaxf(ly, 0.0f) : afull.y);
-    }
+  if ((inx || iny) && (kmode & 2)) {
+    // lens polynomials (rr_deficit): each element with the coefficients of its own half, two scalar
+    // chains (packing the coefficients of two different halves costs more than it saves)
+    P inv2k, xoff;
+    rr_pairP<K_INV2K>(K, inv2k, xoff);
+    const P x = fma2(z, inv2k, xoff);
+    const bool lox = x.x <= (R)0.5, loy = x.y <= (R)0.5;
+    const P xx = abs2(sel2(lox, loy, x, sub2(splat<R>((R)1), x)));
+    const P w = fma2(xx, splat<R>((R)4), splat<R>((R)-1));
+    const R tiny = sizeof(R) == 8 ? (R)RR_TINY_D : (R)1e-30f;
+    const P t = mul2(xx, rr_sqrt2(add2(xx, splat<R>(tiny))));
+    const R px = rr_polyR<Cst<R, M>::OFF_LENS>(K, lox, w.x);
+    const R py = rr_polyR<Cst<R, M>::OFF_LENS>(K, loy, w.y);
+    R lx = lox ? fma(-t.x, px, afull.x) : t.x * px;
+    R ly = loy ? fma(-t.y, py, afull.y) : t.y * py;
+    if constexpr (sizeof(R) == 4) { lx = fmaxf(lx, 0.0f); ly = fmaxf(ly, 0.0f); }
+    ap = mk2(inx ? lx : afull.x, iny ? ly : afull.y);
   } else if (inx || iny) {                      // lens area (rr_deficit), both elements
     const P omks = rr_getP<K_OMKS>(K);
     const P A = sub2(opk, z), B = add2(z, omks), C = sub2(z, omks), D = add2(z, opk);
@@ -1132,7 +1139,7 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
       for (int s = 0; s < ns; ++s, wa += du, wb += du) {
         bool ax, ay;
         P dM;
-        float2 tw = splat<float>(0.0f);        // fp32: phase from the window centre / hwid
+        P tw = splat<R>((R)0);                  // phase from the window centre / hwid
         if constexpr (ANG) {
           const float2 aws = fma2(fs, da2, aw0), aw = abs2(aws);
           ax = aw.x <= hwa;
@@ -1141,7 +1148,7 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
           fs = add2(fs, splat<float>(1.0f));
           if (!(ax || ay)) continue;
           dM = mk2((R)am.x, (R)am.y);
-          tw = mk2(ax ? aws.x * inv_hwa : 0.0f, ay ? aws.y * inv_hwa : 0.0f);
+          tw = mk2((R)(ax ? aws.x * inv_hwa : 0.0f), (R)(ay ? aws.y * inv_hwa : 0.0f));
         } else {
           const double was = NOWRAP ? wa : wa - rr_round(wa), wbs = NOWRAP ? wb : wb - rr_round(wb);
           ax = fabs(was) <= hwid;               // (1e30 - round(1e30) = 0: only without NOWRAP ...
@@ -1149,20 +1156,21 @@ __device__ __forceinline__ void rr_tile_pairs(const double *__restrict__ times, 
           if (!NOWRAP) { ax = ax && ina; ay = ay && inb; }   // ... where the flags are needed)
           if (!(ax || ay)) continue;
           dM = mk2((R)(RR_TWOPI * (was + u_mid)), (R)(RR_TWOPI * (wbs + u_mid)));
-          if constexpr (sizeof(R) == 4)
-            tw = mk2(ax ? (float)was * inv_hw : 0.0f, ay ? (float)wbs * inv_hw : 0.0f);
+          if (kmode & 4) {
+            const R invhw = K.template get<K_INVHW>();
+            tw = mk2(ax ? (R)was * invhw : (R)0, ay ? (R)wbs * invhw : (R)0);
+          }
         }
         dM = sel2(ax, ay, dM, splat<R>((R)0));
         bool fx = true, fy = true;
         P z2;
-        if (!CIRC && sizeof(R) == 4 && (kmode & 4)) {
+        if (!CIRC && (kmode & 4)) {
           // z^2 of both elements from the pv's polynomials (rr_zpoly_fit), each in its own half
-          if constexpr (!CIRC && sizeof(R) == 4) {
-            const float px = K.template poly12f<Cst<R, M>::OFF_ZPOLY>(tw.x < 0.0f ? 0u : 64u,
-                                                                      fmaf(fabsf(tw.x), 2.0f, -1.0f));
-            const float py = K.template poly12f<Cst<R, M>::OFF_ZPOLY>(tw.y < 0.0f ? 0u : 64u,
-                                                                      fmaf(fabsf(tw.y), 2.0f, -1.0f));
-            z2 = mk2(fabsf(px) + 1e-30f, fabsf(py) + 1e-30f);
+          if constexpr (!CIRC) {
+            const R tiny = sizeof(R) == 8 ? (R)RR_TINY_D : (R)1e-30f;
+            const R px = rr_polyR<Cst<R, M>::OFF_ZPOLY>(K, tw.x < (R)0, fma(fabs(tw.x), (R)2, (R)-1));
+            const R py = rr_polyR<Cst<R, M>::OFF_ZPOLY>(K, tw.y < (R)0, fma(fabs(tw.y), (R)2, (R)-1));
+            z2 = mk2(fabs(px) + tiny, fabs(py) + tiny);
           }
         } else {
           z2 = rr_separation2_pair<R, CIRC, M>(K, dM, ax, ay, fx, fy);
