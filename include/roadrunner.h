@@ -58,6 +58,7 @@ extern "C" {
 #define RR_EINDEX       -4   /* lc_index / passband_index / supersampling out of range         */
 #define RR_ESTATE       -5   /* call order: evaluate before set_data / build_ld_table, or npv  */
 #define RR_EALLOC       -6   /* device or host allocation failed                               */
+#define RR_ESCRATCH     -7   /* rr_orbit_z_noalloc: problem exceeds the static scratch array   */
 #define RR_ECUDA_BASE   -1000
 
 /* status bits written per parameter vector (reading R12) */
@@ -224,6 +225,22 @@ int rr_evaluate_flat(rr_ctx *ctx, const double *d_times, const int32_t *d_lc_ind
  * rr_set_data; not rr_build_ld_table.                                                           */
 int rr_orbit_z(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, double *d_z,
                int32_t fp32_math, void *stream);
+/* The same WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it).  rr_orbit_z keeps its scratch - the per-pv
+ * orbit and radius-ratio constants its prep kernel writes - in buffers the ctx grows with cudaMalloc
+ * when a larger npv arrives; this call keeps it in ONE static device array of
+ * RR_NOALLOC_SCRATCH_BYTES (2 MiB; every GPU that loads the library holds it until exit) and calls
+ * no cudaMalloc, cudaFree or allocating library routine.  Arguments, output and arithmetic are those
+ * of rr_orbit_z (same kernels).  Limit: 256-aligned(200 npv) + 72 npv nkpb <= RR_NOALLOC_SCRATCH_BYTES,
+ * i.e. npv <= 7709 with one radius ratio per parameter vector; beyond it the call returns RR_ESCRATCH
+ * and launches nothing.  Must be called with the ctx's device current (RR_ESTATE otherwise).  The
+ * array is shared by every call on that device and keeps the last call's contents; nothing in it
+ * needs clearing (each call writes the entries it reads before it reads them), but calls that overlap
+ * on the GPU - different streams, or several contexts on one device - race on it: serialise them.
+ * Asynchronous on `stream`.  Needs rr_set_data.                                                   */
+#define RR_NOALLOC_SCRATCH_BYTES (2 << 20)
+int rr_orbit_z_noalloc(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, double *d_z,
+                       int32_t fp32_math, void *stream);
 int64_t rr_num_subsamples(const rr_ctx *ctx);   /* < 0: no data set */
 int64_t rr_num_tiles(const rr_ctx *ctx);        /* dispatch tiles of the current data; < 0: none */
 

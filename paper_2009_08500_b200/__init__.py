@@ -37,6 +37,7 @@ SYMBOLS = (
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
     "rr_set_small_planet", "rr_build_ld_table_law", "rr_math_probe", "rr_set_orbit_poly",
+    "rr_orbit_z_noalloc",
 )
 PROBE_OPS = {"sqrt3": 0, "sqrt": 1, "div3": 2, "rcp": 3, "atan_t": 4, "atan_quadrant": 5,
              "atan2_pos": 6, "sincosm1": 7, "cell": 8}
@@ -88,6 +89,7 @@ def load() -> C.CDLL:
         "rr_evaluate_flat": (C.c_int, [_VP, _VP, _VP, _I64, _VP, _VP, _VP, _I32, _VP, _I32, _I64,
                                        _VP, _VP, _VP]),
         "rr_orbit_z": (C.c_int, [_VP, _VP, _I32, _I64, _VP, _I32, _VP]),
+        "rr_orbit_z_noalloc": (C.c_int, [_VP, _VP, _I32, _I64, _VP, _I32, _VP]),
         "rr_num_subsamples": (_I64, [_VP]),
         "rr_num_tiles": (_I64, [_VP]),
         "rr_get_tiles": (C.c_int, [_VP, _VP, _VP, _VP, _VP, _VP]),
@@ -309,6 +311,23 @@ def rr_orbit_z(ctx: int, pv, z, fp32_math=False, stream=None):
         _numel(z, npv * nsub, "z [npv][nsub]", "rr_orbit_z")
     _check(load().rr_orbit_z(ctx, _dev(pv, torch.float64, "pv"), npar, npv, pz,
                              int(bool(fp32_math)), _stream(stream)), "rr_orbit_z")
+
+
+RR_ESCRATCH = -7
+RR_NOALLOC_SCRATCH_BYTES = 2 << 20
+
+
+def rr_orbit_z_noalloc(ctx: int, pv, z, fp32_math=False, stream=None):
+    """rr_orbit_z without any allocation (scratch in a static 2 MiB device array shared by all calls
+    on the device: do not overlap calls); RoadRunnerError code RR_ESCRATCH beyond its limit."""
+    import torch
+    npv, npar = pv.shape
+    pz = _dev(z, torch.float64, "z")
+    nsub = rr_num_subsamples(ctx)
+    if nsub >= 0:
+        _numel(z, npv * nsub, "z [npv][nsub]", "rr_orbit_z_noalloc")
+    _check(load().rr_orbit_z_noalloc(ctx, _dev(pv, torch.float64, "pv"), npar, npv, pz,
+                                     int(bool(fp32_math)), _stream(stream)), "rr_orbit_z_noalloc")
 
 
 def rr_num_subsamples(ctx: int) -> int:

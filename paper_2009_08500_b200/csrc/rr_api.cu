@@ -83,6 +83,9 @@ const char *rr_error_string(int code) {
     case RR_EINDEX: return "lc_index / passband_index / supersampling / exposure_time out of range";
     case RR_ESTATE: return "call order: set_data / build_ld_table first, with the same npv";
     case RR_EALLOC: return "allocation failed";
+    case RR_ESCRATCH:
+      return "problem too large for the static scratch of the allocation-free entry point "
+             "(RR_NOALLOC_SCRATCH_BYTES): use rr_orbit_z";
     default: break;
   }
   if (code <= RR_ECUDA_BASE) return cudaGetErrorString((cudaError_t)(RR_ECUDA_BASE - code));
@@ -117,6 +120,7 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, sizeof(unsigned long long) * 16);
   if (e != cudaSuccess) rc = RR_ECUDA_BASE - (int)e;
   if (rc == RR_OK) rc = rr_smem_probe(&ctx->smem_abs);
+  if (rc == RR_OK) rc = rr_noalloc_setup(ctx);   // address of the no-alloc scratch on this device
   if (rc == RR_OK) rc = rr_geometry_build(ctx);
   if (rc != RR_OK) {
     cudaGetLastError();
@@ -364,6 +368,14 @@ int rr_orbit_z(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, doubl
   int rc = rr_pv_prep_launch(ctx, &ctx->work[0], d_pv, npv, nullptr, fp32_math != 0, st);
   if (rc != RR_OK) return rc;
   return rr_orbit_launch(ctx, &ctx->work[0], npv, d_z, fp32_math, st);
+}
+
+int rr_orbit_z_noalloc(rr_ctx *ctx, const double *d_pv, int32_t npar, int64_t npv, double *d_z,
+                       int32_t fp32_math, void *stream) {
+  if (!ctx || !d_pv || !d_z) return RR_ENULL;
+  if (npv <= 0 || npar != ctx->cfg.nkpb + 6) return RR_ESIZE;
+  if (ctx->ntiles < 0) return RR_ESTATE;
+  return rr_orbit_noalloc_launch(ctx, d_pv, npv, d_z, fp32_math, (cudaStream_t)stream);
 }
 
 int64_t rr_num_subsamples(const rr_ctx *ctx) { return ctx ? ctx->nsub : -1; }

@@ -99,6 +99,7 @@ struct rr_ctx {
   int device;
   int sm_count;
   int smem_abs;         // 1: the flux kernels may address shared memory absolutely (rr_smem_probe)
+  void *noalloc_scratch; // device address of the static scratch of rr_orbit_z_noalloc on ctx's device
   // geometry (a0)
   double *d_ze, *d_zm, *d_mu, *d_q, *d_W;
   void *d_Wsup;         // int2 [nk][ng]: non-zero range [jlo, jhi) of every weight row
@@ -171,5 +172,8 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
                     cudaStream_t st);
 int rr_fma_peak_launch(int precision, double *h_fma_per_s, cudaStream_t st);   // rr_flux.cu
 int rr_smem_probe(int *abs_ok);                                                // rr_flux.cu
+int rr_noalloc_setup(rr_ctx *ctx);                                             // rr_flux.cu
+int rr_orbit_noalloc_launch(rr_ctx *ctx, const double *d_pv, int64_t npv, double *d_z,
+                            int fp32_math, cudaStream_t st);                   // rr_flux.cu
 int rr_math_probe_launch(int op, int fp32, const double *d_a, const double *d_b, int64_t n,
                          double *d_o0, double *d_o1, cudaStream_t st);         // rr_flux.cu

@@ -29,6 +29,7 @@
 // contacts (rr_lens_fit) and z^2 over the transit window of an eccentric pv (rr_zpoly_fit)
 // come from per-pv degree-12 polynomials fitted through exact evaluations once per rr_evaluate.
 #include <algorithm>
+#include <mutex>
 
 #include "rr_common.cuh"
 #include "rr_math.cuh"
@@ -1803,6 +1804,69 @@ int rr_orbit_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, double *d_z, int fp32_
   else
     rr_orbit_kernel<double><<<grid, FT, K_SMEM * 8 + 16 + 4 * RR_LENS_PITCH * 8, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc,
                                                  wk->pvo, ctx->ntiles, npv, ctx->nsub, d_z);
+  RR_LAUNCH_CHECK(ctx);
+  return RR_OK;
+}
+
+// ---- allocation-free entry point (rr_orbit_z_noalloc): kernel 2 alone, scratch in a static array ----
+// Some callers cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+// that forbid it).  rr_orbit_z's scratch - the per-pv orbit and radius-ratio constants the prep kernel
+// writes and the orbit kernel reads - normally lives in buffers the ctx grows with cudaMalloc; here it
+// lives in ONE file-scope device array of RR_NOALLOC_SCRATCH_BYTES (2 MiB), which every GPU that loads
+// the library holds until exit.  Layout: RRPvOrbit[npv] | (256-byte aligned) RRPvBand[npv nkpb].
+// In host code `rr_noalloc_scratch` is a host-side stand-in, not a device address: its device address
+// is taken once per device with cudaGetSymbolAddress (rr_noalloc_setup, from rr_create, with the
+// ctx's device current) and handed to the kernels.  Every call on a device shares the array, which
+// keeps the last call's contents: nothing in it needs to start at zero (the prep kernel writes every
+// entry the orbit kernel reads, for exactly the npv rows of this call, before it reads them, on the
+// same stream), but two calls that overlap on the GPU (different streams, or different contexts on
+// one device) race on it.
+static_assert(sizeof(RRPvOrbit) == 200 && sizeof(RRPvBand) == 72,
+              "roadrunner.h states the no-alloc limit with these sizes");
+static __device__ __align__(256) unsigned char rr_noalloc_scratch[RR_NOALLOC_SCRATCH_BYTES];
+
+int rr_noalloc_setup(rr_ctx *ctx) {
+  static std::mutex mu;
+  static void *addr[64] = {nullptr};               // device address of the array, per device
+  std::lock_guard<std::mutex> lock(mu);
+  const int d = ctx->device;                       // the current device (rr_create)
+  void *p = (d >= 0 && d < 64) ? addr[d] : nullptr;
+  if (!p) {
+    RR_CUDA(cudaGetSymbolAddress(&p, rr_noalloc_scratch));
+    if (d >= 0 && d < 64) addr[d] = p;
+  }
+  ctx->noalloc_scratch = p;
+  return RR_OK;
+}
+
+// As rr_pv_prep_launch + rr_orbit_launch with pvo / pvb in the static scratch.  No allocation.
+int rr_orbit_noalloc_launch(rr_ctx *ctx, const double *d_pv, int64_t npv, double *d_z, int fp32_math,
+                            cudaStream_t st) {
+  const rr_config &c = ctx->cfg;
+  const uint64_t off_b = ((uint64_t)sizeof(RRPvOrbit) * (uint64_t)npv + 255u) & ~(uint64_t)255u;
+  const uint64_t need = off_b + (uint64_t)sizeof(RRPvBand) * (uint64_t)npv * (uint64_t)c.nkpb;
+  if (npv > (1 << 24) || need > (uint64_t)RR_NOALLOC_SCRATCH_BYTES) return RR_ESCRATCH;
+  int dev = -1;
+  RR_CUDA(cudaGetDevice(&dev));
+  if (!ctx->noalloc_scratch || dev != ctx->device) return RR_ESTATE;   // the address is per device
+  RRPvOrbit *pvo = reinterpret_cast<RRPvOrbit *>(ctx->noalloc_scratch);
+  RRPvBand *pvb = reinterpret_cast<RRPvBand *>(static_cast<unsigned char *>(ctx->noalloc_scratch) + off_b);
+  const RRWork *wk = &ctx->work[0];                // table mode of the device-pointer API (k limits)
+  const bool direct = wk->lazy == 2;
+  rr_pv_prep_kernel<<<(unsigned)((npv + 127) / 128), 128, 0, st>>>(
+      d_pv, npv, c.nkpb, c.nk, c.k0, c.k1, direct ? 1e-300 : c.k0, direct ? 1e300 : c.k1, c.ng,
+      fp32_math != 0, ctx->mean_k, rr_row_pad(ctx, wk), pvo, pvb, nullptr);
+  RR_LAUNCH_CHECK(ctx);
+  const int64_t total = ctx->ntiles * npv;
+  if (total <= 0) return RR_OK;
+  const unsigned grid = rr_grid_for(total);
+  const size_t smem = K_SMEM * 8 + 16 + 4 * RR_LENS_PITCH * 8;
+  if (fp32_math)
+    rr_orbit_kernel<float><<<grid, FT, smem, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, pvo,
+                                                   ctx->ntiles, npv, ctx->nsub, d_z);
+  else
+    rr_orbit_kernel<double><<<grid, FT, smem, st>>>(ctx->d_times, ctx->d_tiles, ctx->d_lc, pvo,
+                                                    ctx->ntiles, npv, ctx->nsub, d_z);
   RR_LAUNCH_CHECK(ctx);
   return RR_OK;
 }
