@@ -87,6 +87,10 @@ def parse_args():
     ap.add_argument("--no-orbit-poly", action="store_true",
                     help="solve Kepler's equation per eccentric sub-sample (rr_set_orbit_poly(ctx, 0)) "
                          "instead of evaluating the per-pv z^2 polynomials")
+    ap.add_argument("--direct-formulation", action="store_true",
+                    help="the direct formulation throughout: a Kepler solve per eccentric sub-sample and "
+                         "the two-arctangent lens area per ingress sub-sample (rr_set_orbit_poly(ctx, 0), "
+                         "rr_set_lens_poly(ctx, 0)): executed work = algorithmic work")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true",
@@ -274,10 +278,11 @@ DTYPE_NAME = {"fp64": "f64", "fp32": "f32", "mixed": "f32 (sum and flux f64)"}
 class Case:
     """One workload in one precision, resident on the device: ctx, inputs, output buffers."""
 
-    def __init__(self, rr, wl, precision: str, table_mode: str, dev, ld_law=None, orbit_poly=True):
+    def __init__(self, rr, wl, precision: str, table_mode: str, dev, ld_law=None, orbit_poly=True,
+                 lens_poly=True):
         import torch
         self.rr, self.wl, self.precision, self.dev = rr, wl, precision, dev
-        self.orbit_poly = orbit_poly
+        self.orbit_poly, self.lens_poly = orbit_poly, lens_poly
         code = PRECISIONS[precision]
         self.npdt = np.float32 if code != rr.RR_FP64 else np.float64
         self.model = rr.RoadRunner.from_config(wl.model, code)
@@ -285,6 +290,7 @@ class Case:
         rr.rr_set_table_mode(self.ctx, {"lazy": rr.RR_TABLE_LAZY, "full": rr.RR_TABLE_FULL,
                                         "direct": rr.RR_TABLE_DIRECT}[table_mode])
         rr.rr_set_orbit_poly(self.ctx, orbit_poly)
+        rr.rr_set_lens_poly(self.ctx, lens_poly)
         self.model.set_data(wl.times, wl.lc_index, wl.passband_index, wl.supersampling,
                             wl.exposure_time)
         self.ldp_h = np.ascontiguousarray(wl.ldp(self.model.mu), dtype=self.npdt)
@@ -378,6 +384,7 @@ class Case:
         rr.rr_enable_counters(self.ctx, False)
         counts["eccentric_poly"] = as_run["eccentric_poly"]
         counts["solver_iters_as_run"] = as_run["solver_iters"]
+        counts["lens_poly"] = int(bool(self.lens_poly))
         return counts
 
     def sample_error(self, n_pv=8, n_cols=600):
@@ -414,7 +421,8 @@ class Case:
         self.ldp = self.pv = self.flux = self.status = self.ldc = None
 
 
-def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, clocks, peaks):
+def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, clocks, peaks,
+                capture_key=None):
     """algorithmic bytes and FMA-pipe instructions per launch of rr_flux_kernel against
     the HBM and ALU peaks; the larger time bound names the binding roofline."""
     code = PRECISIONS[precision]
@@ -451,7 +459,7 @@ def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, 
                     "unit": "TFLOP/s", "frac": alu_achieved / alu_peak_tflops, "traffic": None,
                     "peak_source": f"{lanes} FMA lanes/clk/SM x {SM_COUNT} SMs x {sm_max:.0f} MHz "
                                    "x 2 (DESIGN.md s7)"}
-    cap = ncu_capture(wl.name, precision)
+    cap = ncu_capture(wl.name, capture_key or precision)
     counter_based = None
     if cap is not None:
         roofline["traffic"] = int(cap["dram_read_bytes"]) + int(cap["dram_write_bytes"])
@@ -466,7 +474,8 @@ def roofline_of(rr, wl, precision: str, t: dict, counts: dict, table_mode: str, 
                          "issue_active_pct_ncu": float(cap["issue_active_pct"]),
                          "capture": cap["capture"]}
     exe_ops = dict(ops)
-    exe_ops.update(EXECUTED_OPS.get("fp64" if precision == "fp64" else "fp32", {}))
+    if counts.get("lens_poly", 1):
+        exe_ops.update(EXECUTED_OPS.get("fp64" if precision == "fp64" else "fp32", {}))
     exe_fma = alg_fma + sum(counts[c] * (exe_ops[c] - ops[c]) for c in ("ingress",))
     if counts.get("eccentric_poly"):
         # sub-samples taken from the z^2 polynomials: ZPOLY_OPS instead of the fixed part and their solves
@@ -561,7 +570,8 @@ def run_ours(args):
         wl.ld_coeffs = np.ascontiguousarray(np.roll(wl.ld_coeffs, sh, axis=0))
 
     case = Case(rr, wl, args.precision, args.table_mode, dev, ld_law=args.ld_law,
-                orbit_poly=not args.no_orbit_poly)
+                orbit_poly=not (args.no_orbit_poly or args.direct_formulation),
+                lens_poly=not args.direct_formulation)
     ctx, model = case.ctx, case.model
     steps, warm = max(1, args.steps), max(3, args.warmup)
 
@@ -626,7 +636,8 @@ def run_ours(args):
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except (OSError, ValueError):
         pass
-    roofline = roofline_of(rr, wl, args.precision, t, counts, args.table_mode, clocks, peaks)
+    roofline = roofline_of(rr, wl, args.precision, t, counts, args.table_mode, clocks, peaks,
+                           capture_key=args.precision + "-direct" if args.direct_formulation else None)
     roofline["fma_peak_measured_live_tflops"] = 2.0 * rr.rr_measure_fma_peak(precision) / 1e12
     roofline["note"] = ("kernel_ms = CUDA events recorded by the library around rr_flux_kernel on the "
                         "launching stream, inside the timed region, mean over the timed steps; frac = "
@@ -644,7 +655,9 @@ def run_ours(args):
               "working set fits L2: small config, latency-bound, no roofline claim",
         "invalid_pv": n_bad,
         "ld_table_call": "rr_build_ld_table_law" if args.ld_law else "rr_build_ld_table",
-        "orbit": "Kepler solve per eccentric sub-sample" if args.no_orbit_poly else
+        "lens_area": "two arctangents per ingress sub-sample" if args.direct_formulation else
+                     "per-(pv, k) polynomials between the contacts for k <= 0.32, else the exact form",
+        "orbit": "Kepler solve per eccentric sub-sample" if (args.no_orbit_poly or args.direct_formulation) else
                  "per-pv z^2 polynomials over the transit window where they converge, else the solve"})
     case.close()
     del case

@@ -37,7 +37,7 @@ SYMBOLS = (
     "rr_launch_count", "rr_measure_fma_peak", "rr_set_table_mode", "rr_enable_kernel_timing",
     "rr_get_kernel_times", "rr_get_rows", "rr_set_mean_k_weights",
     "rr_set_small_planet", "rr_build_ld_table_law", "rr_math_probe", "rr_set_orbit_poly",
-    "rr_orbit_z_noalloc",
+    "rr_orbit_z_noalloc", "rr_set_lens_poly",
 )
 PROBE_OPS = {"sqrt3": 0, "sqrt": 1, "div3": 2, "rcp": 3, "atan_t": 4, "atan_quadrant": 5,
              "atan2_pos": 6, "sincosm1": 7, "cell": 8}
@@ -103,6 +103,7 @@ def load() -> C.CDLL:
         "rr_get_rows": (C.c_int, [_VP, _VP]),
         "rr_set_mean_k_weights": (C.c_int, [_VP, _I32]),
         "rr_set_orbit_poly": (C.c_int, [_VP, _I32]),
+        "rr_set_lens_poly": (C.c_int, [_VP, _I32]),
         "rr_set_small_planet": (C.c_int, [_VP, _DBL]),
         "rr_build_ld_table_law": (C.c_int, [_VP, _I32, _VP, _I32, _I64, _VP]),
         "rr_math_probe": (C.c_int, [_I32, _I32, _VP, _VP, _I64, _VP, _VP, _VP]),
@@ -363,6 +364,10 @@ def rr_set_small_planet(ctx: int, k_threshold: float):
 
 def rr_set_orbit_poly(ctx: int, on: bool):
     _check(load().rr_set_orbit_poly(ctx, int(bool(on))), "rr_set_orbit_poly")
+
+
+def rr_set_lens_poly(ctx: int, on: bool):
+    _check(load().rr_set_lens_poly(ctx, int(bool(on))), "rr_set_lens_poly")
 
 
 def rr_set_mean_k_weights(ctx: int, on: bool):

@@ -112,6 +112,7 @@ int rr_create(const rr_config *cfg, rr_ctx **out) {
   ctx->reduction = RR_REDUCE_AUTO;
   ctx->table_mode = RR_TABLE_LAZY;
   ctx->orbit_poly = 1;
+  ctx->lens_poly = 1;
   int rc = RR_OK;
   cudaError_t e = cudaGetDevice(&ctx->device);
   if (e == cudaSuccess)
@@ -262,6 +263,12 @@ int rr_set_mean_k_weights(rr_ctx *ctx, int32_t on) {
 int rr_set_orbit_poly(rr_ctx *ctx, int32_t on) {
   if (!ctx) return RR_ENULL;
   ctx->orbit_poly = on ? 1 : 0;
+  return RR_OK;
+}
+
+int rr_set_lens_poly(rr_ctx *ctx, int32_t on) {
+  if (!ctx) return RR_ENULL;
+  ctx->lens_poly = on ? 1 : 0;
   return RR_OK;
 }
 

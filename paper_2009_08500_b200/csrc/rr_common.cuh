@@ -119,7 +119,8 @@ struct rr_ctx {
   int32_t reduction;
   int32_t table_mode;   // RR_TABLE_LAZY | RR_TABLE_FULL | RR_TABLE_DIRECT
   int32_t mean_k;       // 1: LD weights at the mean k of the passbands
-  int32_t orbit_poly;   // 1 (default): fp64 kernel takes z^2 from per-pv polynomials where they hold
+  int32_t orbit_poly;   // 1 (default): z^2 of eccentric pvs from per-pv polynomials where they hold
+  int32_t lens_poly;    // 1 (default): lens area between the contacts from per-pv polynomials
   double k_small;       // small-planet approximation for kw <= k_small; 0: off
   // table (kernel 1) and per-pv prep: [0] device API, [1],[2] host-path slots
   RRWork work[3];

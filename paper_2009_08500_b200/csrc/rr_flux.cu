@@ -1722,7 +1722,7 @@ int rr_flux_launch(rr_ctx *ctx, RRWork *wk, int64_t npv, void *d_flux, cudaStrea
   P.T = wk->lazy ? nullptr : wk->T;
   P.rows = wk->lazy ? wk->rows : nullptr;
   P.istar = wk->istar;
-  P.lens = RR_LENS_POLY ? wk->lens : nullptr;   // (fitted in fp64 for every precision)
+  P.lens = (RR_LENS_POLY && ctx->lens_poly) ? wk->lens : nullptr;   // (fitted in fp64 for every precision)
   P.flux = d_flux;
   P.counters = ctx->d_counters;
   P.npt = ctx->npt;

@@ -1296,3 +1296,21 @@ def test_orbit_polynomials_against_the_per_subsample_solve(rr):
     cnt = rr.rr_get_counters(gm.ctx)
     assert 0 < cnt["eccentric"] and cnt["eccentric_poly"] < cnt["eccentric"]
     gm.close()
+
+
+@pytest.mark.parametrize("precision", [0, 1])
+def test_lens_polynomials_against_the_exact_lens_area(rr, precision):
+    """rr_set_lens_poly: the area between the contacts from per-(pv, k) polynomials (default) or from
+    the two-arctangent form per sub-sample; both against the oracle and against each other."""
+    wl = small_workload(4)
+    want, _ = oracle_flux(wl)
+    gm = gpu_model(rr, wl, precision)
+    gm.build_ld_table(wl.ldp(gm.mu))
+    out = {}
+    for on in (True, False):
+        rr.rr_set_lens_poly(gm.ctx, on)
+        out[on] = gm.evaluate(wl.pv).cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(out[on] - want)) <= (TOL32 if precision else 1e-12)
+    d = np.max(np.abs(out[True] - out[False]))
+    assert 0 < d <= (2e-7 if precision else 1e-12)
+    gm.close()
