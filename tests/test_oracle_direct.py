@@ -186,3 +186,34 @@ def test_named_law_disc_integrals():
         assert abs(float(truth.istar_mp(f)) - ist) < 1e-14, name
     f, ist = truth.law("exponential", [0.5, 0.01])
     assert ist is None and float(f(0.5)) < 1.0
+
+
+def test_rows_from_parameter_vectors_pick_the_right_radius_ratio():
+    """oracle_direct_rows_pv (row selection of readings R12 / R13, in C since round 2): row (pv, pb)
+    is built at the pv's k of that passband, or at the mean of the pv's radius ratios with
+    mean_k_weights; a pv with a non-finite or non-positive k gets NaN rows.  Against rows built one
+    at a time with the k chosen here (weights pinned elsewhere: to L1 on the g nodes)."""
+    mc = workloads.ModelConfig(npb=3, nkpb=3, nzin=20, nzlimb=20, ng=17)
+    om = oracle.OracleDirectModel.from_config(mc)
+    rng = np.random.default_rng(2)
+    npv = 5
+    pv = np.zeros((npv, 9))
+    pv[:, :3] = rng.uniform(0.05, 0.2, (npv, 3))
+    pv[:, 3:] = [0.0, 3.0, 8.0, 1.5, 0.1, 0.3]
+    pv[3, 1] = -0.1                                   # invalid rows
+    pv[4, 2] = np.nan
+    ldp = workloads.sample_profile("quadratic", rng.uniform(0.1, 0.4, (npv, 3, 2)), om.mu)
+    one = oracle.OracleDirectModel(mc.nzin, mc.nzlimb, mc.zcut, mc.ng, npb=1, nkpb=1)
+    for mean in (False, True):
+        rows, _ = om.rows(ldp, pv, mean_k_weights=mean)
+        assert rows.shape == (npv, 3, mc.ng)
+        assert np.isnan(rows[3:]).all() and not np.isnan(rows[:3]).any()
+        for v in range(3):
+            for b in range(3):
+                k = pv[v, :3].mean() if mean else pv[v, b]
+                pv1 = np.array([[k, 0.0, 3.0, 8.0, 1.5, 0.1, 0.3]])
+                want, _ = one.rows(ldp[v, b][None, None, :], pv1)
+                assert np.array_equal(rows[v, b], want[0, 0])
+    a, _ = om.rows(ldp, pv, mean_k_weights=False)
+    b_, _ = om.rows(ldp, pv, mean_k_weights=True)
+    assert np.max(np.abs(a[:3] - b_[:3])) > 1e-6      # the two selections differ
