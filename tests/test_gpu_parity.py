@@ -1314,3 +1314,41 @@ def test_lens_polynomials_against_the_exact_lens_area(rr, precision):
     d = np.max(np.abs(out[True] - out[False]))
     assert 0 < d <= (2e-7 if precision else 1e-12)
     gm.close()
+
+
+def test_bench_line_contract(rr):
+    """bench.py prints ONE JSON line with the keys the driver reads (a small population here; the
+    default run uses config 4 at full size)."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "3", "--npv", "96",
+                          "--npt", "6000", "--steps", "3", "--warmup", "3", "--no-all-configs"],
+                         capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.strip().splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step",
+                "higher_is_better", "scaling", "vs_baseline", "dtype", "data", "config", "clocks",
+                "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert key in d, key
+    assert d["unit"] == "evaluations/s" and d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] == 3
+    assert d["higher_is_better"] is True and d["vs_baseline"] is None and d["dtype"] == "f64"
+    assert d["config"]["workload"] == "config3-heterogeneous" and d["data"] == "synthetic"
+    assert d["value"] > 0 and d["gpu_launches"] >= 3 * 5
+    assert abs(d["value"] - d["config"]["evaluations_per_step_per_gpu"] / (d["ms_per_step"] * 1e-3)) \
+        <= 1e-6 * d["value"]
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] >= 96 * 6000 * 8
+    r = d["roofline"]
+    for key in ("bound", "achieved", "peak", "unit", "frac", "traffic", "kernel_ms", "counter_based",
+                "executed_frac_by_table", "class_counts"):
+        assert key in r, key
+    assert r["bound"] in ("hbm", "alu") and 0 < r["frac"] and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["value"] > 0 and c["cores"] >= 1 and c["sample"]
+    assert c["one_thread"] > 0 and c["all_cores"] > 0 and c["cpu_model"]
+    assert d["max_abs_err_vs_oracle_sample"]["value"] <= TOL64
